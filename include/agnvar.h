@@ -1,0 +1,164 @@
+/*
+ * agnvar.h -- C ABI of the B200-native light-curve generator (hot path of Sartori et al. 2019,
+ * arXiv:1909.06374): batched light curves with a prescribed PSD (bending power law, Eq. 3) and a
+ * prescribed value distribution (the ERDF, Eq. 1-2), by Timmer & Koenig + Emmanoulopoulos-style
+ * iterative amplitude adjustment (sec. 2.1, sec. 3.2.2).
+ *
+ * Citations "PAPER.md:<line>" are to the paper text; "Qn"/"On" are the readings listed in DESIGN.md.
+ *
+ * Conventions (all calls)
+ *   - d_* are DEVICE pointers owned by the caller; h_* are HOST pointers, read before the call returns.
+ *   - The library never allocates or frees device memory.  Scratch space is the caller's d_ws of
+ *     ws_bytes >= agnvar_workspace_bytes(...), 256-byte aligned.
+ *   - Every call only enqueues work on `stream` (a cudaStream_t passed as void*; NULL = default
+ *     stream) and returns without synchronising.
+ *   - Every call returns an agnvar_status; nothing throws or aborts.  AGNVAR_EINVAL is returned
+ *     before any launch.  AGNVAR_ECUDA wraps a failed launch (sticky CUDA errors are not cleared).
+ *   - Arrays are row-major [B][N], one light curve contiguous.  N is a power of two,
+ *     4 <= N <= 2^27 (the paper's own cap).
+ *   - dtype selects the arithmetic AND storage type of series, spectra and sort keys (float or
+ *     double).  PSD values, the ERDF table and the inverse-CDF arithmetic are always fp64.
+ *   - Random numbers: Philox4x32-10, key = (seed lo, seed hi), counter = (i lo, i hi, curve b, tag);
+ *     tag 0 = TK normals (i = frequency index j), tag 1 = ERDF uniforms (i = n >> 1).  A curve's
+ *     numbers depend on (seed, b0 + row) only, never on B or on the launch shape (b0 = `curve0`).
+ */
+#ifndef AGNVAR_H
+#define AGNVAR_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    AGNVAR_OK = 0,
+    AGNVAR_EINVAL = 1,       /* bad argument (see each call) */
+    AGNVAR_EWORKSPACE = 2,   /* ws_bytes too small or d_ws NULL / misaligned */
+    AGNVAR_ECUDA = 3,        /* a CUDA launch or API call failed */
+    AGNVAR_EUNSUPPORTED = 4  /* valid request this build does not implement (e.g. oversample*N > 2^28) */
+} agnvar_status;
+
+typedef enum { AGNVAR_F32 = 0, AGNVAR_F64 = 1 } agnvar_dtype;
+typedef enum { AGNVAR_ERDF_BPL = 0, AGNVAR_ERDF_LOGNORMAL = 1 } agnvar_erdf_kind;
+typedef enum {
+    AGNVAR_OP_ERDF_SAMPLE_SORTED = 1,
+    AGNVAR_OP_TK_GENERATE = 2,
+    AGNVAR_OP_E13_ITERATE = 3,
+    AGNVAR_OP_PERIODOGRAM = 4
+} agnvar_op;
+
+/* Eq. 3: PSD(f) = A [ (f/f_b)^alpha_low + (f/f_b)^alpha_high ]^-1.
+ * A <= 0 asks agnvar_tk_generate for the unit-variance normalisation (Q4):
+ * A = M^2 / (2 sum_{1<=j<M/2} s_j + s_{M/2}), s_j the bracket at f_j = j/(M dt). */
+typedef struct {
+    double A, f_b, alpha_low, alpha_high;
+} agnvar_psd;
+
+/* Eq. 1, kind BPL:  xi(lambda) ~ [ (lambda/lam_star)^delta1 + (lambda/lam_star)^delta2 ]^-1
+ * Eq. 2, kind LOGNORMAL: xi ~ exp(-(log10 lambda - mu_log10)^2 / (2 sigma_log10^2)).
+ * xi is dN/dlog(lambda); the sampled density of u = log10(lambda) is proportional to xi(10^u) on
+ * [log10 lam_min, log10 lam_max]  (Q10). */
+typedef struct {
+    int kind;
+    int reserved;
+    double lam_star, delta1, delta2;
+    double mu_log10, sigma_log10;
+    double lam_min, lam_max;
+} agnvar_erdf;
+
+/* Bytes of scratch the given op needs.  `oversample` matters for AGNVAR_OP_TK_GENERATE only
+ * (pass 1 otherwise); `aux` = grid_points for ERDF_SAMPLE_SORTED, nbins for PERIODOGRAM, else 0.
+ * Returns 0 for invalid arguments. */
+size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int oversample, int64_t aux);
+
+/* S0 -- Eq. 3 at n given frequencies (fp64 in, fp64 out; d_out[i] = A * bracket(d_f[i])).
+ * The unit of f is the unit of f_b (Q9).  A is used as given (must be finite).
+ * EINVAL: n < 0, NULL pointer with n > 0, non-finite parameter, f_b <= 0. */
+int agnvar_psd_bpl(const double* d_f, int64_t n, const agnvar_psd* h_p, double* d_out, void* stream);
+
+/* S1 -- the random draw from the ERDF, sorted ("a random draw from the PDF";
+ * PAPER.md:124).  Per curve b: table u_k = u_lo + k D (k < grid_points), p_k = xi(10^u_k),
+ * C = normalised trapezoid cumulative; sample n: U from Philox (tag 1), k with C_k <= U < C_{k+1},
+ * u = u_k + (U - C_k)/(C_{k+1} - C_k) D, lambda = 10^u rounded to dtype (O4).  Then a stable
+ * ascending sort of the N draws carrying the draw index.
+ *   h_erdf      n_erdf structs, n_erdf = 1 (shared) or B (one per curve)
+ *   curve0      Philox curve number of row 0 (lets a caller shard a batch across GPUs)
+ *   d_sorted    out [B][N] dtype: the draw in ascending order
+ *   d_perm0     out [B][N] u32 or NULL: d_perm0[b][r] = draw (time) index of the r-th smallest (Q15:
+ *               the first x_sim is the draw in draw order, x_sim[perm0[r]] = sorted[r])
+ *   d_draw      out [B][N] dtype or NULL: the draw in draw order
+ * EINVAL: bad B/N/dtype, n_erdf not 1 or B, grid_points < 2 or > 65536, NULL h_erdf/d_sorted,
+ * non-finite parameter, lam_min <= 0, lam_min >= lam_max, sigma <= 0 (log-normal), lam_star <= 0 (BPL). */
+int agnvar_erdf_sample_sorted(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t B, int64_t N, int dtype,
+                              uint64_t seed, uint32_t curve0, int grid_points, void* d_sorted,
+                              uint32_t* d_perm0, void* d_draw, void* d_ws, size_t ws_bytes, void* stream);
+
+/* S2 -- Timmer & Koenig series and its amplitudes.  M = oversample * N;
+ * X_0 = 0; X_j = sqrt(S_j/2)(g_re + i g_im), 1 <= j < M/2; X_{M/2} = sqrt(S_{M/2}) g_re;
+ * S_j = Eq. 3 at f_j = j/(M dt), fp64; g from Philox tag 0, Box-Muller (O1, O3);
+ * x = inverse real DFT of length M with 1/M; x_norm = the central N samples
+ * x[(M-N)/2 ... (M-N)/2+N-1] (oversampling, Q3); A_norm_j = |DFT_N(x_norm)_j|,
+ * j = 0..N/2 (Q2: the amplitudes of the TK realisation are the target of the adjustment).
+ *   h_psd       n_psd structs, n_psd = 1 or B
+ *   oversample  one of 1, 2, 4, 8, 10, 16, 20
+ *   d_xnorm     out [B][N] dtype or NULL
+ *   d_anorm     out [B][N/2+1] dtype or NULL
+ * EINVAL: bad B/N/dtype/oversample, n_psd not 1 or B, dt <= 0, f_b <= 0, non-finite parameter,
+ * NULL h_psd, both outputs NULL.  EUNSUPPORTED: oversample * N > 2^28. */
+int agnvar_tk_generate(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_t N, double dt, int oversample,
+                       int dtype, uint64_t seed, uint32_t curve0, void* d_xnorm, void* d_anorm, void* d_ws,
+                       size_t ws_bytes, void* stream);
+
+/* L1-L6 -- the iteration (steps O6).  Per curve, k = 1..max_iter:
+ *   X = DFT_N(x_sim);  X'_j = A_norm_j X_j / |X_j|  (X'_j = A_norm_j if |X_j| = 0; DC and Nyquist
+ *   real);  x_adj = IDFT_N(X') with 1/N, -0 -> +0;  idx_new = stable ascending argsort of x_adj
+ *   (ties: lower time index first);  changed = #{r : idx_new[r] != idx_old[r]};
+ *   x_sim[idx_new[r]] = sorted[r].
+ * A curve is converged at the first k with changed = 0 (iters_used = k); a converged state is a fixed
+ * point, so later iterations of a batch leave it unchanged (Q18).  Not converging within max_iter is
+ * not an error: iters_used = max_iter.
+ *   d_anorm        in  [B][N/2+1] dtype  target amplitudes (natural order, j = 0..N/2)
+ *   d_sorted       in  [B][N] dtype      ascending values (the draw)
+ *   d_perm         in/out [B][N] u32     in: idx_old of the first iteration (perm0); out: final permutation.
+ *                                        Feeding the output back resumes the run.
+ *   d_x            out [B][N] dtype      final x_sim  (x[perm[r]] = sorted[r])
+ *   d_iters_used   out [B] i32 or NULL
+ *   d_changed_hist out [B][max_iter] i64 or NULL: changed count of every iteration
+ *   d_xadj_dbg     out [B][N] dtype or NULL: x_adj of the last iteration (for lock-step checks: call
+ *                  with max_iter = 1 to step the product kernels one iteration at a time)
+ * EINVAL: bad B/N/dtype, max_iter < 1, NULL d_anorm/d_sorted/d_perm/d_x. */
+int agnvar_e13_iterate(int64_t B, int64_t N, int dtype, const void* d_anorm, const void* d_sorted,
+                       uint32_t* d_perm, void* d_x, int max_iter, int32_t* d_iters_used,
+                       int64_t* d_changed_hist, void* d_xadj_dbg, void* d_ws, size_t ws_bytes, void* stream);
+
+/* P -- periodogram (Appendix A), bins j = 1..N/2 (DC excluded):
+ *   norm 0 (Eq. A2):  P_j = (2/N^2) |DFT_j|^2
+ *   norm 1 (Eq. A4):  P_j = (2 dt / (mu^2 N)) |DFT_j|^2,  mu = sample mean.
+ * nbins = 0: d_out [B][N/2] fp64, d_out[b][j-1] = P_j.
+ * nbins > 0 (Q19): h_bin_edges_j holds nbins+1 increasing integers j_0 >= 1 ... j_nb <= N/2+1; bin e is
+ * the arithmetic mean of P_j over j_e <= j < j_{e+1}, the last bin closed at N/2; d_out [B][nbins] fp64;
+ * d_counts [nbins] i64 or NULL receives the number of j per bin.  Sums are accumulated in fp64.
+ * EINVAL: bad B/N/dtype/norm, dt <= 0, nbins < 0 or > 4096, edges not increasing or out of range, NULL d_x/d_out. */
+int agnvar_periodogram(int64_t B, int64_t N, int dtype, const void* d_x, double dt, int norm, int nbins,
+                       const int64_t* h_bin_edges_j, double* d_out, int64_t* d_counts, void* d_ws,
+                       size_t ws_bytes, void* stream);
+
+/* O1 -- the raw random words every other call consumes (for bit-exact checks of the generator):
+ * d_out[4 i + w] = word w of Philox4x32-10 with counter (lo(i0+i), hi(i0+i), curve, tag) and key
+ * (seed lo, seed hi), 0 <= i < n.  The paper only names cuRAND; the stream layout is
+ * reading O1 of DESIGN.md.  EINVAL: n < 0, NULL d_out with n > 0. */
+int agnvar_philox_u32(uint64_t seed, uint64_t i0, int64_t n, uint32_t curve, uint32_t tag, uint32_t* d_out,
+                      void* stream);
+
+/* Static, never NULL. */
+const char* agnvar_strerror(int status);
+
+/* Library version string and the GPU architecture it was compiled for ("sm_100a"). */
+const char* agnvar_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AGNVAR_H */

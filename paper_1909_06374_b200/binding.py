@@ -1,0 +1,237 @@
+"""Thin ctypes binding of include/agnvar.h (libagnvar.so).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels behind the C ABI.
+PyTorch is used for device memory (tensors own every buffer, including the workspace) and for the
+current CUDA stream.  There is no CPU fallback: if the library is missing or cannot be loaded the
+import of a symbol raises.
+"""
+import ctypes as C
+import os
+
+import torch
+
+from . import _build
+
+AGNVAR_F32, AGNVAR_F64 = 0, 1
+AGNVAR_ERDF_BPL, AGNVAR_ERDF_LOGNORMAL = 0, 1
+OP_ERDF_SAMPLE_SORTED, OP_TK_GENERATE, OP_E13_ITERATE, OP_PERIODOGRAM = 1, 2, 3, 4
+
+EXPORTS = (
+    "agnvar_workspace_bytes", "agnvar_psd_bpl", "agnvar_erdf_sample_sorted", "agnvar_tk_generate",
+    "agnvar_e13_iterate", "agnvar_periodogram", "agnvar_philox_u32", "agnvar_strerror", "agnvar_version",
+)
+
+
+class AgnvarError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        super().__init__(f"{where}: agnvar status {status} ({strerror(status)})")
+
+
+class agnvar_psd(C.Structure):
+    _fields_ = [("A", C.c_double), ("f_b", C.c_double), ("alpha_low", C.c_double), ("alpha_high", C.c_double)]
+
+
+class agnvar_erdf(C.Structure):
+    _fields_ = [("kind", C.c_int), ("reserved", C.c_int), ("lam_star", C.c_double), ("delta1", C.c_double),
+                ("delta2", C.c_double), ("mu_log10", C.c_double), ("sigma_log10", C.c_double),
+                ("lam_min", C.c_double), ("lam_max", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libagnvar.so (building it with nvcc first if the sources are newer). Raises if impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    try:
+        path = _build.build()
+    except Exception as exc:  # no nvcc on this machine: use the shipped .so if there is one
+        if not os.path.exists(path):
+            raise RuntimeError(f"libagnvar.so is missing and could not be built: {exc}") from exc
+    L = C.CDLL(path)
+    vp, i64, u64, u32, i32, dbl, sz = C.c_void_p, C.c_int64, C.c_uint64, C.c_uint32, C.c_int, C.c_double, C.c_size_t
+    L.agnvar_workspace_bytes.restype = sz
+    L.agnvar_workspace_bytes.argtypes = [i32, i64, i64, i32, i32, i64]
+    L.agnvar_psd_bpl.restype = i32
+    L.agnvar_psd_bpl.argtypes = [vp, i64, C.POINTER(agnvar_psd), vp, vp]
+    L.agnvar_erdf_sample_sorted.restype = i32
+    L.agnvar_erdf_sample_sorted.argtypes = [C.POINTER(agnvar_erdf), i64, i64, i64, i32, u64, u32, i32, vp, vp, vp,
+                                            vp, sz, vp]
+    L.agnvar_tk_generate.restype = i32
+    L.agnvar_tk_generate.argtypes = [C.POINTER(agnvar_psd), i64, i64, i64, dbl, i32, i32, u64, u32, vp, vp, vp, sz,
+                                     vp]
+    L.agnvar_e13_iterate.restype = i32
+    L.agnvar_e13_iterate.argtypes = [i64, i64, i32, vp, vp, vp, vp, i32, vp, vp, vp, vp, sz, vp]
+    L.agnvar_periodogram.restype = i32
+    L.agnvar_periodogram.argtypes = [i64, i64, i32, vp, dbl, i32, i32, C.POINTER(i64), vp, vp, vp, sz, vp]
+    L.agnvar_philox_u32.restype = i32
+    L.agnvar_philox_u32.argtypes = [u64, u64, i64, u32, u32, vp, vp]
+    L.agnvar_strerror.restype = C.c_char_p
+    L.agnvar_strerror.argtypes = [i32]
+    L.agnvar_version.restype = C.c_char_p
+    L.agnvar_version.argtypes = []
+    _lib = L
+    return L
+
+
+def strerror(status):
+    return lib().agnvar_strerror(int(status)).decode()
+
+
+def version():
+    return lib().agnvar_version().decode()
+
+
+# ---- marshalling helpers --------------------------------------------------------------------------
+def _dt(dtype):
+    if dtype in (AGNVAR_F32, torch.float32, "f32", "float32"):
+        return AGNVAR_F32, torch.float32
+    if dtype in (AGNVAR_F64, torch.float64, "f64", "float64"):
+        return AGNVAR_F64, torch.float64
+    raise ValueError(f"dtype {dtype!r}: use float32 or float64")
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _check(st, where):
+    if st != 0:
+        raise AgnvarError(st, where)
+
+
+def _psd_array(psd):
+    """psd: one (A, f_b, alpha_low, alpha_high) tuple/dict or a sequence of them."""
+    items = [psd] if isinstance(psd, (dict, tuple)) else list(psd)
+    arr = (agnvar_psd * len(items))()
+    for i, p in enumerate(items):
+        if isinstance(p, dict):
+            p = (p.get("A", 0.0), p["f_b"], p["alpha_low"], p["alpha_high"])
+        arr[i] = agnvar_psd(float(p[0]), float(p[1]), float(p[2]), float(p[3]))
+    return arr, len(items)
+
+
+def _erdf_array(erdf):
+    """erdf: one dict (kind, lam_star, delta1, delta2 | mu_log10, sigma_log10, lam_min, lam_max) or a sequence."""
+    items = [erdf] if isinstance(erdf, dict) else list(erdf)
+    arr = (agnvar_erdf * len(items))()
+    for i, e in enumerate(items):
+        arr[i] = agnvar_erdf(int(e["kind"]), 0, float(e.get("lam_star", 1.0)), float(e.get("delta1", 0.0)),
+                             float(e.get("delta2", 0.0)), float(e.get("mu_log10", 0.0)),
+                             float(e.get("sigma_log10", 1.0)), float(e["lam_min"]), float(e["lam_max"]))
+    return arr, len(items)
+
+
+_ws_cache = {}
+
+
+def workspace_bytes(op, B, N, dtype, oversample=1, aux=0):
+    return int(lib().agnvar_workspace_bytes(int(op), int(B), int(N), _dt(dtype)[0], int(oversample), int(aux)))
+
+
+def workspace(nbytes, device=None):
+    """A cached uint8 device tensor of at least nbytes (one per device; grown on demand)."""
+    device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+    cur = _ws_cache.get(device)
+    if cur is None or cur.numel() < nbytes:
+        _ws_cache[device] = None
+        cur = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+        _ws_cache[device] = cur
+    return cur
+
+
+def free_workspace():
+    _ws_cache.clear()
+
+
+# ---- the calls of include/agnvar.h ----------------------------------------------------------------
+def agnvar_philox_u32(seed, i0, n, curve, tag, device="cuda"):
+    """O1: raw Philox4x32-10 words [n][4] (int32 tensor holding the u32 bit patterns)."""
+    out = torch.empty((n, 4), dtype=torch.int32, device=device)
+    _check(lib().agnvar_philox_u32(int(seed), int(i0), int(n), int(curve), int(tag), _ptr(out), _stream()),
+           "agnvar_philox_u32")
+    return out
+
+
+def agnvar_psd_bpl(f, psd, out=None):
+    """S0: Eq. 3 at the fp64 device tensor f. psd = (A, f_b, alpha_low, alpha_high)."""
+    arr, _ = _psd_array(psd)
+    if out is None:
+        out = torch.empty_like(f)
+    _check(lib().agnvar_psd_bpl(_ptr(f), f.numel(), arr, _ptr(out), _stream()), "agnvar_psd_bpl")
+    return out
+
+
+def agnvar_erdf_sample_sorted(erdf, B, N, dtype, seed, curve0=0, grid_points=4096, want_perm0=True,
+                              want_draw=False, device="cuda"):
+    """S1: returns (sorted [B][N], perm0 [B][N] u32-as-int32 | None, draw [B][N] | None)."""
+    code, tdt = _dt(dtype)
+    arr, n = _erdf_array(erdf)
+    srt = torch.empty((B, N), dtype=tdt, device=device)
+    perm0 = torch.empty((B, N), dtype=torch.int32, device=device) if want_perm0 else None
+    draw = torch.empty((B, N), dtype=tdt, device=device) if want_draw else None
+    nb = workspace_bytes(OP_ERDF_SAMPLE_SORTED, B, N, code, 1, grid_points)
+    ws = workspace(nb, srt.device)
+    _check(lib().agnvar_erdf_sample_sorted(arr, n, B, N, code, int(seed), int(curve0), int(grid_points), _ptr(srt),
+                                           _ptr(perm0), _ptr(draw), _ptr(ws), ws.numel(), _stream()),
+           "agnvar_erdf_sample_sorted")
+    return srt, perm0, draw
+
+
+def agnvar_tk_generate(psd, B, N, dt, oversample, dtype, seed, curve0=0, want_xnorm=True, want_anorm=True,
+                       device="cuda"):
+    """S2: returns (x_norm [B][N] | None, A_norm [B][N/2+1] | None)."""
+    code, tdt = _dt(dtype)
+    arr, n = _psd_array(psd)
+    xn = torch.empty((B, N), dtype=tdt, device=device) if want_xnorm else None
+    an = torch.empty((B, N // 2 + 1), dtype=tdt, device=device) if want_anorm else None
+    nb = workspace_bytes(OP_TK_GENERATE, B, N, code, oversample, 0)
+    ws = workspace(nb, device)
+    _check(lib().agnvar_tk_generate(arr, n, B, N, float(dt), int(oversample), code, int(seed), int(curve0),
+                                    _ptr(xn), _ptr(an), _ptr(ws), ws.numel(), _stream()), "agnvar_tk_generate")
+    return xn, an
+
+
+def agnvar_e13_iterate(anorm, sorted_vals, perm, max_iter, x=None, want_hist=False, want_xadj=False):
+    """L1-L6. perm is updated IN PLACE (in: idx_old of the first iteration, out: final permutation).
+    Returns dict(x, perm, iters_used, changed_hist | None, x_adj | None)."""
+    B, N = sorted_vals.shape
+    code, tdt = _dt(sorted_vals.dtype)
+    dev = sorted_vals.device
+    assert anorm.dtype == tdt and anorm.shape == (B, N // 2 + 1) and anorm.is_contiguous()
+    assert perm.dtype == torch.int32 and perm.shape == (B, N) and perm.is_contiguous() and sorted_vals.is_contiguous()
+    if x is None:
+        x = torch.empty((B, N), dtype=tdt, device=dev)
+    iters = torch.empty((B,), dtype=torch.int32, device=dev)
+    hist = torch.empty((B, max_iter), dtype=torch.int64, device=dev) if want_hist else None
+    xadj = torch.empty((B, N), dtype=tdt, device=dev) if want_xadj else None
+    nb = workspace_bytes(OP_E13_ITERATE, B, N, code, 1, 0)
+    ws = workspace(nb, dev)
+    _check(lib().agnvar_e13_iterate(B, N, code, _ptr(anorm), _ptr(sorted_vals), _ptr(perm), _ptr(x), int(max_iter),
+                                    _ptr(iters), _ptr(hist), _ptr(xadj), _ptr(ws), ws.numel(), _stream()),
+           "agnvar_e13_iterate")
+    return {"x": x, "perm": perm, "iters_used": iters, "changed_hist": hist, "x_adj": xadj}
+
+
+def agnvar_periodogram(x, dt, norm=0, bin_edges=None):
+    """P: x [B][N] -> P [B][N/2] fp64, or (Pbin [B][nbins] fp64, counts [nbins] i64) with integer bin edges."""
+    B, N = x.shape
+    code, _ = _dt(x.dtype)
+    dev = x.device
+    nbins = 0 if bin_edges is None else len(bin_edges) - 1
+    out = torch.empty((B, nbins if nbins else N // 2), dtype=torch.float64, device=dev)
+    counts = torch.empty((nbins,), dtype=torch.int64, device=dev) if nbins else None
+    edges = (C.c_int64 * (nbins + 1))(*[int(e) for e in bin_edges]) if nbins else None
+    nb = workspace_bytes(OP_PERIODOGRAM, B, N, code, 1, nbins)
+    ws = workspace(nb, dev)
+    _check(lib().agnvar_periodogram(B, N, code, _ptr(x), float(dt), int(norm), nbins, edges, _ptr(out), _ptr(counts),
+                                    _ptr(ws), ws.numel(), _stream()), "agnvar_periodogram")
+    return out if not nbins else (out, counts)

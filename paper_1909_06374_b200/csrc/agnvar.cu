@@ -1,0 +1,432 @@
+// agnvar.cu -- C ABI (include/agnvar.h) of the B200-native E13 light-curve generator.
+// Host side: argument validation, workspace carving, kernel sequencing on the caller's stream.
+// Every step of the path runs in the kernels of fft.cuh / sort.cuh / kernels.cuh; there is no CPU
+// fallback and no vendor FFT / sort library call.
+#include "../../include/agnvar.h"
+#include "common.cuh"
+#include "fft.cuh"
+#include "sort.cuh"
+#include "kernels.cuh"
+
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+using namespace agn;
+
+namespace {
+
+struct Carver {
+    unsigned char* base;
+    size_t off;
+    explicit Carver(void* p) : base((unsigned char*)p), off(0) {}
+    template <typename U> U* take(size_t count) {
+        U* r = base ? (U*)(base + off) : nullptr;
+        off += align_up(count * sizeof(U), 256);
+        return r;
+    }
+};
+
+inline bool is_pow2(int64_t n) { return n > 0 && (n & (n - 1)) == 0; }
+inline bool valid_BN(int64_t B, int64_t N) {
+    return B >= 1 && B <= (int64_t)1 << 30 && is_pow2(N) && N >= 4 && N <= ((int64_t)1 << 27);
+}
+inline bool valid_dtype(int d) { return d == AGNVAR_F32 || d == AGNVAR_F64; }
+inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
+inline bool valid_oversample(int o) { return o == 1 || o == 2 || o == 4 || o == 8 || o == 10 || o == 16 || o == 20; }
+
+bool g_attrs_done[16] = {false};
+template <typename T> cudaError_t ensure_attrs() {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    int slot = (dev & 7) * 2 + (sizeof(T) == 8 ? 1 : 0);
+    if (g_attrs_done[slot]) return cudaSuccess;
+    e = fft_set_attrs<T>();
+    if (e != cudaSuccess) return e;
+    e = sort_set_attrs<T>();
+    if (e != cudaSuccess) return e;
+    g_attrs_done[slot] = true;
+    return cudaSuccess;
+}
+
+inline unsigned cdiv(long long a, long long b) { return (unsigned)((a + b - 1) / b); }
+
+// ---- workspace sizes -----------------------------------------------------------------------------
+template <typename T> size_t ws_e13(int64_t B, int64_t N) {
+    typedef typename Cx<T>::type C;
+    Carver c(nullptr);
+    c.take<C>(FftPlan<T>::table_elems());
+    c.take<T>((size_t)B * N);                 // Z / x_adj
+    c.take<T>((size_t)B * (N / 2 + 1));       // A_norm in position order
+    c.take<uint32_t>((size_t)B * N);          // permutation ping-pong
+    c.take<unsigned long long>((size_t)B);    // changed counters
+    c.take<int>((size_t)B);                   // first_zero
+    return c.off + sort_ws_bytes<T>(B, N);
+}
+template <typename T> size_t ws_tk(int64_t B, int64_t N, int os) {
+    typedef typename Cx<T>::type C;
+    Carver c(nullptr);
+    const int64_t M = N * os;
+    c.take<C>(FftPlan<T>::table_elems());     // tables, length-M transform
+    c.take<C>(FftPlan<T>::table_elems());     // tables, length-N transform
+    c.take<PsdDev>((size_t)B);
+    c.take<double>((size_t)B * 1024);         // partial sums
+    if (os % 5 == 0) c.take<C>((size_t)B * 3 * (M / 5));
+    else c.take<T>((size_t)B * M);
+    c.take<T>((size_t)B * N);                 // x_norm
+    c.take<T>((size_t)B * N);                 // spectrum of x_norm
+    return c.off;
+}
+template <typename T> size_t ws_erdf(int64_t B, int64_t N, int64_t G) {
+    Carver c(nullptr);
+    c.take<ErdfDev>((size_t)B);
+    c.take<double>((size_t)B * G);
+    c.take<T>((size_t)B * N);                 // the draw in draw order
+    return c.off + sort_ws_bytes<T>(B, N);
+}
+template <typename T> size_t ws_pgram(int64_t B, int64_t N, int64_t nbins) {
+    typedef typename Cx<T>::type C;
+    Carver c(nullptr);
+    c.take<C>(FftPlan<T>::table_elems());
+    c.take<T>((size_t)B * N);
+    c.take<double>((size_t)B);
+    c.take<double>((size_t)B * (N / 2));
+    c.take<long long>((size_t)nbins + 1);
+    return c.off;
+}
+
+inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? AGNVAR_OK : AGNVAR_ECUDA; }
+
+// real forward FFT of B series of length N held in `Z` (in place, viewed as [B][N/2] complex);
+// result in position order.
+template <typename T> void rfft_inplace(const FftPlan<T>& p, T* Z, int64_t B, cudaStream_t st) {
+    typedef typename Cx<T>::type C;
+    const long long L = 1ll << p.dg.logL;
+    fft_forward<T>(p, (const C*)Z, (C*)Z, L, L, (int)B, st);
+}
+
+// ---- E13 -------------------------------------------------------------------------------------------
+template <typename T>
+int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, uint32_t* d_perm, void* d_x,
+             int max_iter, int32_t* d_iters_used, int64_t* d_changed_hist, void* d_xadj_dbg, void* d_ws,
+             size_t ws_bytes, cudaStream_t st) {
+    typedef typename Cx<T>::type C;
+    if (ws_bytes < ws_e13<T>(B, N) || !d_ws || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
+    if (ensure_attrs<T>() != cudaSuccess) return AGNVAR_ECUDA;
+    const int logL = ilog2_u64((uint64_t)N) - 1;
+    const long long L = N / 2;
+    Carver c(d_ws);
+    C* tables = c.take<C>(FftPlan<T>::table_elems());
+    T* Z = c.take<T>((size_t)B * N);
+    T* Ap = c.take<T>((size_t)B * (N / 2 + 1));
+    uint32_t* P1 = c.take<uint32_t>((size_t)B * N);
+    unsigned long long* changed = c.take<unsigned long long>((size_t)B);
+    int* first_zero = c.take<int>((size_t)B);
+    void* sort_ws = (unsigned char*)d_ws + c.off;
+    T* x = (T*)d_x;
+    const T* sorted = (const T*)d_sorted;
+
+    FftPlan<T> plan = fft_plan_init<T>(logL, tables, st);
+    TwLevel<T> rlv = real_level<T>(plan);
+    cudaMemsetAsync(changed, 0, (size_t)B * sizeof(unsigned long long), st);
+    cudaMemsetAsync(first_zero, 0, (size_t)B * sizeof(int), st);
+    perm_anorm_kernel<T><<<bgrid(cdiv(L + 1, 256), B), 256, 0, st>>>((const T*)d_anorm, Ap, plan.dg, (int)B);
+    const unsigned sg = (unsigned)std::min<long long>((N + 1023) / 1024, 148 * 16);
+    // first x_sim: the draw in draw order (Q15)
+    scatter_count_kernel<T, false><<<bgrid(sg, B), 256, 0, st>>>(d_perm, nullptr, sorted, x, N, nullptr, (int)B);
+    uint32_t* cur = d_perm;
+    uint32_t* nxt = P1;
+    for (int k = 1; k <= max_iter; ++k) {
+        // L1 forward FFT (x_sim -> Z, position order)
+        fft_forward<T>(plan, (const C*)x, (C*)Z, L, L, (int)B, st);
+        // L2 amplitude replace
+        replace_kernel<T><<<bgrid(cdiv(L, 256), B), 256, 0, st>>>((C*)Z, Ap, plan.dg, rlv, (int)B);
+        // L3 inverse FFT (Z -> x_adj, natural order, 1/L)
+        fft_inverse<T>(plan, (const C*)Z, (C*)Z, L, L, (int)B, (T)(1.0 / (double)L), st);
+        // L4 segmented stable argsort
+        cudaError_t e = seg_argsort<T>(Z, nxt, nullptr, B, N, sort_ws, st);
+        if (e != cudaSuccess) return AGNVAR_ECUDA;
+        // L5 rank scatter + change count
+        scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(nxt, cur, sorted, x, N, changed, (int)B);
+        // L6 bookkeeping
+        post_iter_kernel<<<cdiv(B, 256), 256, 0, st>>>(changed, first_zero, k, (long long*)d_changed_hist, max_iter, (int)B);
+        std::swap(cur, nxt);
+    }
+    if (cur != d_perm) cudaMemcpyAsync(d_perm, cur, (size_t)B * N * 4, cudaMemcpyDeviceToDevice, st);
+    if (d_xadj_dbg)
+        copy_canon_kernel<T><<<cdiv(B * N, 256), 256, 0, st>>>(Z, (T*)d_xadj_dbg, (long long)B * N);
+    if (d_iters_used) finalize_iters_kernel<<<cdiv(B, 256), 256, 0, st>>>(first_zero, d_iters_used, max_iter, (int)B);
+    return cuda_status(cudaGetLastError());
+}
+
+// ---- TK ----------------------------------------------------------------------------------------------
+template <typename T>
+int tk_impl(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_t N, double dt, int os, uint64_t seed,
+            uint32_t curve0, void* d_xnorm, void* d_anorm, void* d_ws, size_t ws_bytes, cudaStream_t st) {
+    typedef typename Cx<T>::type C;
+    if (ws_bytes < ws_tk<T>(B, N, os) || !d_ws || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
+    if (ensure_attrs<T>() != cudaSuccess) return AGNVAR_ECUDA;
+    const int64_t M = N * os;
+    const bool five = (os % 5 == 0);
+    Carver c(d_ws);
+    C* tabM = c.take<C>(FftPlan<T>::table_elems());
+    C* tabN = c.take<C>(FftPlan<T>::table_elems());
+    PsdDev* psd = c.take<PsdDev>((size_t)B);
+    double* partial = c.take<double>((size_t)B * 1024);
+    T* ZM = five ? (T*)c.take<C>((size_t)B * 3 * (M / 5)) : c.take<T>((size_t)B * M);
+    T* xn = c.take<T>((size_t)B * N);
+    T* ZN = c.take<T>((size_t)B * N);
+
+    std::vector<PsdDev> hp((size_t)B);
+    bool need_norm = false;
+    for (int64_t b = 0; b < B; ++b) {
+        const agnvar_psd& p = h_psd[n_psd == 1 ? 0 : b];
+        hp[(size_t)b] = PsdDev{p.A, p.f_b, p.alpha_low, p.alpha_high};
+        if (!(p.A > 0.0)) need_norm = true;
+    }
+    // pageable host -> device: the copy is staged before the call returns
+    if (cudaMemcpyAsync(psd, hp.data(), (size_t)B * sizeof(PsdDev), cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return AGNVAR_ECUDA;
+    if (need_norm) {
+        long long half = M / 2;
+        int nchunks = (int)std::min<long long>(1024, (half + 4095) / 4096);
+        int chunk = (int)((half + nchunks - 1) / nchunks);
+        psd_norm_partial_kernel<<<bgrid(nchunks, B), 256, 0, st>>>(psd, M, dt, chunk, partial, nchunks, (int)B);
+        psd_norm_final_kernel<<<(unsigned)B, 256, 0, st>>>(psd, partial, nchunks, M);
+    }
+    T* xsrc;   // where x_norm ends up
+    if (five) {
+        const int64_t Mp = M / 5;
+        const int logMp = ilog2_u64((uint64_t)Mp);
+        FftPlan<T> pm = fft_plan_init<T>(logMp, tabM, st);
+        tk_fill5_kernel<T><<<bgrid(cdiv(Mp, 256), 3 * B), 256, 0, st>>>((C*)ZM, psd, pm.dg, dt, seed, curve0, (int)B);
+        fft_inverse<T>(pm, (const C*)ZM, (C*)ZM, Mp, Mp, (int)(3 * B), (T)1, st);
+        tk_combine5_kernel<T><<<bgrid(cdiv(N, 256), B), 256, 0, st>>>((const C*)ZM, xn, Mp, N, (M - N) / 2, (int)B);
+        xsrc = xn;
+    } else {
+        const int logLM = ilog2_u64((uint64_t)M) - 1;
+        const long long LM = M / 2;
+        FftPlan<T> pm = fft_plan_init<T>(logLM, tabM, st);
+        tk_fill_kernel<T><<<bgrid(cdiv(LM, 256), B), 256, 0, st>>>((C*)ZM, psd, pm.dg, dt, seed, curve0, (int)B);
+        fft_inverse<T>(pm, (const C*)ZM, (C*)ZM, LM, LM, (int)B, (T)(1.0 / (double)LM), st);
+        if (os == 1) xsrc = ZM;
+        else {
+            crop_kernel<T><<<bgrid(cdiv(N, 256), B), 256, 0, st>>>(ZM, M, (M - N) / 2, xn, N, (int)B);
+            xsrc = xn;
+        }
+    }
+    if (d_xnorm) cudaMemcpyAsync(d_xnorm, xsrc, (size_t)B * N * sizeof(T), cudaMemcpyDeviceToDevice, st);
+    if (d_anorm) {
+        const int logL = ilog2_u64((uint64_t)N) - 1;
+        const long long L = N / 2;
+        FftPlan<T> pn = fft_plan_init<T>(logL, tabN, st);
+        fft_forward<T>(pn, (const C*)xsrc, (C*)ZN, L, L, (int)B, st);
+        untangle_out_kernel<T, 0><<<bgrid(cdiv(L, 256), B), 256, 0, st>>>((const C*)ZN, pn.dg, real_level<T>(pn),
+                                                                          (T*)d_anorm, nullptr, nullptr, (int)B);
+    }
+    return cuda_status(cudaGetLastError());
+}
+
+// ---- ERDF ----------------------------------------------------------------------------------------------
+template <typename T>
+int erdf_impl(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t B, int64_t N, uint64_t seed, uint32_t curve0,
+              int G, void* d_sorted, uint32_t* d_perm0, void* d_draw, void* d_ws, size_t ws_bytes, cudaStream_t st) {
+    if (ws_bytes < ws_erdf<T>(B, N, G) || !d_ws || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
+    if (ensure_attrs<T>() != cudaSuccess) return AGNVAR_ECUDA;
+    Carver c(d_ws);
+    ErdfDev* erdf = c.take<ErdfDev>((size_t)B);
+    double* Ctab = c.take<double>((size_t)B * G);
+    T* draw = c.take<T>((size_t)B * N);
+    void* sort_ws = (unsigned char*)d_ws + c.off;
+    if (d_draw) draw = (T*)d_draw;
+    std::vector<ErdfDev> he((size_t)n_erdf);
+    for (int64_t i = 0; i < n_erdf; ++i) {
+        const agnvar_erdf& e = h_erdf[i];
+        he[(size_t)i] = ErdfDev{e.kind, 0, e.lam_star, e.delta1, e.delta2, e.mu_log10, e.sigma_log10,
+                                std::log10(e.lam_min), std::log10(e.lam_max)};
+    }
+    if (cudaMemcpyAsync(erdf, he.data(), (size_t)n_erdf * sizeof(ErdfDev), cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return AGNVAR_ECUDA;
+    erdf_table_kernel<<<(unsigned)n_erdf, 256, 0, st>>>(erdf, G, Ctab);
+    erdf_sample_kernel<T><<<bgrid(cdiv(N / 2, 256), B), 256, 0, st>>>(erdf, n_erdf == 1 ? 0 : 1, Ctab, G, N, seed,
+                                                                      curve0, draw, (int)B);
+    // stable ascending sort carrying the draw index; perm0 is needed internally even if the caller
+    // does not want it -> use the tail of the sort workspace? no: sort straight into d_perm0 or a scratch
+    uint32_t* perm = d_perm0;
+    if (!perm) return AGNVAR_EINVAL;   // guarded by the caller (scratch provided there)
+    cudaError_t e = seg_argsort<T>(draw, perm, (T*)d_sorted, B, N, sort_ws, st);
+    if (e != cudaSuccess) return AGNVAR_ECUDA;
+    return cuda_status(cudaGetLastError());
+}
+
+// ---- periodogram -----------------------------------------------------------------------------------------
+template <typename T>
+int pgram_impl(int64_t B, int64_t N, const void* d_x, double dt, int norm, int nbins, const int64_t* h_edges,
+               double* d_out, int64_t* d_counts, void* d_ws, size_t ws_bytes, cudaStream_t st) {
+    typedef typename Cx<T>::type C;
+    if (ws_bytes < ws_pgram<T>(B, N, nbins) || !d_ws || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
+    if (ensure_attrs<T>() != cudaSuccess) return AGNVAR_ECUDA;
+    Carver c(d_ws);
+    C* tables = c.take<C>(FftPlan<T>::table_elems());
+    T* Z = c.take<T>((size_t)B * N);
+    double* scale = c.take<double>((size_t)B);
+    double* P = c.take<double>((size_t)B * (N / 2));
+    long long* edges = c.take<long long>((size_t)nbins + 1);
+    const int logL = ilog2_u64((uint64_t)N) - 1;
+    const long long L = N / 2;
+    FftPlan<T> plan = fft_plan_init<T>(logL, tables, st);
+    pgram_scale_kernel<T><<<(unsigned)B, 256, 0, st>>>((const T*)d_x, N, dt, norm, scale);
+    fft_forward<T>(plan, (const C*)d_x, (C*)Z, L, L, (int)B, st);
+    double* Pout = nbins > 0 ? P : d_out;
+    untangle_out_kernel<T, 1><<<bgrid(cdiv(L, 256), B), 256, 0, st>>>((const C*)Z, plan.dg, real_level<T>(plan), nullptr,
+                                                                      Pout, scale, (int)B);
+    if (nbins > 0) {
+        if (cudaMemcpyAsync(edges, h_edges, (size_t)(nbins + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st) != cudaSuccess)
+            return AGNVAR_ECUDA;
+        pgram_bin_kernel<<<bgrid((unsigned)nbins, B), 256, 0, st>>>(P, L, edges, nbins, d_out, (long long*)d_counts, (int)B);
+    }
+    return cuda_status(cudaGetLastError());
+}
+
+}  // namespace
+
+// =====================================================================================================
+// C ABI
+// =====================================================================================================
+extern "C" {
+
+const char* agnvar_strerror(int status) {
+    switch (status) {
+        case AGNVAR_OK: return "ok";
+        case AGNVAR_EINVAL: return "invalid argument";
+        case AGNVAR_EWORKSPACE: return "workspace too small, NULL or misaligned";
+        case AGNVAR_ECUDA: return "CUDA launch or API failure";
+        case AGNVAR_EUNSUPPORTED: return "unsupported configuration";
+        default: return "unknown status";
+    }
+}
+
+const char* agnvar_version(void) { return "agnvar 0.1 (sm_100a)"; }
+
+size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int oversample, int64_t aux) {
+    if (!valid_BN(B, N) || !valid_dtype(dtype)) return 0;
+    const bool f32 = dtype == AGNVAR_F32;
+    switch (op) {
+        case AGNVAR_OP_E13_ITERATE: return f32 ? ws_e13<float>(B, N) : ws_e13<double>(B, N);
+        case AGNVAR_OP_TK_GENERATE:
+            if (!valid_oversample(oversample) || N * (int64_t)oversample > ((int64_t)1 << 28)) return 0;
+            return f32 ? ws_tk<float>(B, N, oversample) : ws_tk<double>(B, N, oversample);
+        case AGNVAR_OP_ERDF_SAMPLE_SORTED:
+            if (aux < 2 || aux > 65536) return 0;
+            // + a scratch permutation for callers that pass d_perm0 = NULL
+            return (f32 ? ws_erdf<float>(B, N, aux) : ws_erdf<double>(B, N, aux)) + align_up((size_t)B * N * 4, 256);
+        case AGNVAR_OP_PERIODOGRAM:
+            if (aux < 0 || aux > 4096) return 0;
+            return f32 ? ws_pgram<float>(B, N, aux) : ws_pgram<double>(B, N, aux);
+        default: return 0;
+    }
+}
+
+int agnvar_philox_u32(uint64_t seed, uint64_t i0, int64_t n, uint32_t curve, uint32_t tag, uint32_t* d_out,
+                      void* stream) {
+    if (n < 0) return AGNVAR_EINVAL;
+    if (n == 0) return AGNVAR_OK;
+    if (!d_out) return AGNVAR_EINVAL;
+    philox_words_kernel<<<cdiv(n, 256), 256, 0, (cudaStream_t)stream>>>(seed, i0, n, curve, tag, (uint4*)d_out);
+    return cuda_status(cudaGetLastError());
+}
+
+int agnvar_psd_bpl(const double* d_f, int64_t n, const agnvar_psd* h_p, double* d_out, void* stream) {
+    if (n < 0 || !h_p) return AGNVAR_EINVAL;
+    if (!std::isfinite(h_p->A) || !std::isfinite(h_p->f_b) || !std::isfinite(h_p->alpha_low) ||
+        !std::isfinite(h_p->alpha_high) || !(h_p->f_b > 0.0))
+        return AGNVAR_EINVAL;
+    if (n == 0) return AGNVAR_OK;
+    if (!d_f || !d_out) return AGNVAR_EINVAL;
+    PsdDev p{h_p->A, h_p->f_b, h_p->alpha_low, h_p->alpha_high};
+    psd_bpl_kernel<<<cdiv(n, 256), 256, 0, (cudaStream_t)stream>>>(d_f, n, p, d_out);
+    return cuda_status(cudaGetLastError());
+}
+
+int agnvar_erdf_sample_sorted(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t B, int64_t N, int dtype,
+                              uint64_t seed, uint32_t curve0, int grid_points, void* d_sorted, uint32_t* d_perm0,
+                              void* d_draw, void* d_ws, size_t ws_bytes, void* stream) {
+    if (!valid_BN(B, N) || !valid_dtype(dtype) || !h_erdf || !d_sorted) return AGNVAR_EINVAL;
+    if (!(n_erdf == 1 || n_erdf == B) || grid_points < 2 || grid_points > 65536) return AGNVAR_EINVAL;
+    for (int64_t i = 0; i < n_erdf; ++i) {
+        const agnvar_erdf& e = h_erdf[i];
+        if (e.kind != AGNVAR_ERDF_BPL && e.kind != AGNVAR_ERDF_LOGNORMAL) return AGNVAR_EINVAL;
+        if (!std::isfinite(e.lam_min) || !std::isfinite(e.lam_max) || !(e.lam_min > 0.0) || !(e.lam_min < e.lam_max))
+            return AGNVAR_EINVAL;
+        if (e.kind == AGNVAR_ERDF_BPL) {
+            if (!std::isfinite(e.lam_star) || !(e.lam_star > 0.0) || !std::isfinite(e.delta1) || !std::isfinite(e.delta2))
+                return AGNVAR_EINVAL;
+        } else {
+            if (!std::isfinite(e.mu_log10) || !std::isfinite(e.sigma_log10) || !(e.sigma_log10 > 0.0)) return AGNVAR_EINVAL;
+        }
+    }
+    size_t need = agnvar_workspace_bytes(AGNVAR_OP_ERDF_SAMPLE_SORTED, B, N, dtype, 1, grid_points);
+    if (!d_ws || ws_bytes < need || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
+    const size_t tail = align_up((size_t)B * N * 4, 256);
+    uint32_t* perm = d_perm0 ? d_perm0 : (uint32_t*)((unsigned char*)d_ws + (need - tail));
+    if (dtype == AGNVAR_F32)
+        return erdf_impl<float>(h_erdf, n_erdf, B, N, seed, curve0, grid_points, d_sorted, perm, d_draw, d_ws,
+                                need - tail, (cudaStream_t)stream);
+    return erdf_impl<double>(h_erdf, n_erdf, B, N, seed, curve0, grid_points, d_sorted, perm, d_draw, d_ws, need - tail,
+                             (cudaStream_t)stream);
+}
+
+int agnvar_tk_generate(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_t N, double dt, int oversample,
+                       int dtype, uint64_t seed, uint32_t curve0, void* d_xnorm, void* d_anorm, void* d_ws,
+                       size_t ws_bytes, void* stream) {
+    if (!valid_BN(B, N) || !valid_dtype(dtype) || !h_psd || !valid_oversample(oversample)) return AGNVAR_EINVAL;
+    if (!(n_psd == 1 || n_psd == B) || !(dt > 0.0) || !std::isfinite(dt)) return AGNVAR_EINVAL;
+    if (!d_xnorm && !d_anorm) return AGNVAR_EINVAL;
+    for (int64_t i = 0; i < n_psd; ++i) {
+        const agnvar_psd& p = h_psd[i];
+        if (!std::isfinite(p.A) || !std::isfinite(p.f_b) || !(p.f_b > 0.0) || !std::isfinite(p.alpha_low) ||
+            !std::isfinite(p.alpha_high))
+            return AGNVAR_EINVAL;
+    }
+    if (N * (int64_t)oversample > ((int64_t)1 << 28)) return AGNVAR_EUNSUPPORTED;
+    if (dtype == AGNVAR_F32)
+        return tk_impl<float>(h_psd, n_psd, B, N, dt, oversample, seed, curve0, d_xnorm, d_anorm, d_ws, ws_bytes,
+                              (cudaStream_t)stream);
+    return tk_impl<double>(h_psd, n_psd, B, N, dt, oversample, seed, curve0, d_xnorm, d_anorm, d_ws, ws_bytes,
+                           (cudaStream_t)stream);
+}
+
+int agnvar_e13_iterate(int64_t B, int64_t N, int dtype, const void* d_anorm, const void* d_sorted, uint32_t* d_perm,
+                       void* d_x, int max_iter, int32_t* d_iters_used, int64_t* d_changed_hist, void* d_xadj_dbg,
+                       void* d_ws, size_t ws_bytes, void* stream) {
+    if (!valid_BN(B, N) || !valid_dtype(dtype) || max_iter < 1) return AGNVAR_EINVAL;
+    if (!d_anorm || !d_sorted || !d_perm || !d_x) return AGNVAR_EINVAL;
+    if (!aligned(d_perm, 16) || !aligned(d_x, 16) || !aligned(d_sorted, 16)) return AGNVAR_EINVAL;
+    if (dtype == AGNVAR_F32)
+        return e13_impl<float>(B, N, d_anorm, d_sorted, d_perm, d_x, max_iter, d_iters_used, d_changed_hist,
+                               d_xadj_dbg, d_ws, ws_bytes, (cudaStream_t)stream);
+    return e13_impl<double>(B, N, d_anorm, d_sorted, d_perm, d_x, max_iter, d_iters_used, d_changed_hist, d_xadj_dbg,
+                            d_ws, ws_bytes, (cudaStream_t)stream);
+}
+
+int agnvar_periodogram(int64_t B, int64_t N, int dtype, const void* d_x, double dt, int norm, int nbins,
+                       const int64_t* h_bin_edges_j, double* d_out, int64_t* d_counts, void* d_ws, size_t ws_bytes,
+                       void* stream) {
+    if (!valid_BN(B, N) || !valid_dtype(dtype) || !d_x || !d_out) return AGNVAR_EINVAL;
+    if (!(norm == 0 || norm == 1) || !(dt > 0.0) || !std::isfinite(dt) || nbins < 0 || nbins > 4096) return AGNVAR_EINVAL;
+    if (!aligned(d_x, 16)) return AGNVAR_EINVAL;
+    if (nbins > 0) {
+        if (!h_bin_edges_j) return AGNVAR_EINVAL;
+        if (h_bin_edges_j[0] < 1 || h_bin_edges_j[nbins] > N / 2 + 1) return AGNVAR_EINVAL;
+        for (int e = 0; e < nbins; ++e)
+            if (!(h_bin_edges_j[e] < h_bin_edges_j[e + 1])) return AGNVAR_EINVAL;
+    }
+    if (dtype == AGNVAR_F32)
+        return pgram_impl<float>(B, N, d_x, dt, norm, nbins, h_bin_edges_j, d_out, d_counts, d_ws, ws_bytes,
+                                 (cudaStream_t)stream);
+    return pgram_impl<double>(B, N, d_x, dt, norm, nbins, h_bin_edges_j, d_out, d_counts, d_ws, ws_bytes,
+                              (cudaStream_t)stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,119 @@
+// common.cuh -- shared device helpers of the agnvar CUDA library (sm_100a).
+// Nothing here is shared with oracle/ (the CPU oracle is independent test infrastructure).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+namespace agn {
+
+// ------------------------------------------------------------------------------------------------
+// complex numbers on float2 / double2
+// ------------------------------------------------------------------------------------------------
+template <typename T> struct Cx;
+template <> struct Cx<float> { typedef float2 type; };
+template <> struct Cx<double> { typedef double2 type; };
+
+template <typename T> __host__ __device__ __forceinline__ typename Cx<T>::type mk(T a, T b) {
+    typename Cx<T>::type r; r.x = a; r.y = b; return r;
+}
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { a.x += b.x; a.y += b.y; return a; }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { a.x -= b.x; a.y -= b.y; return a; }
+template <typename C> __device__ __forceinline__ C cmul(C a, C b) {
+    C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
+}
+// a * conj(b)
+template <typename C> __device__ __forceinline__ C cmulc(C a, C b) {
+    C r; r.x = a.x * b.x + a.y * b.y; r.y = a.y * b.x - a.x * b.y; return r;
+}
+template <typename C> __device__ __forceinline__ C cconj(C a) { a.y = -a.y; return a; }
+template <typename C> __device__ __forceinline__ C cswap(C a) { C r; r.x = a.y; r.y = a.x; return r; }
+// multiply by -i (forward radix-4 rotation) : (x, y) -> (y, -x)
+template <typename C> __device__ __forceinline__ C cmul_mi(C a) { C r; r.x = a.y; r.y = -a.x; return r; }
+
+__host__ __device__ __forceinline__ int ilog2_u64(uint64_t v) {
+    int l = 0;
+    while (v > 1) { v >>= 1; ++l; }
+    return l;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Philox4x32-10 (O1).  Round: p0 = 0xD2511F53*c0, p1 = 0xCD9E8D57*c2;
+// c <- (hi(p1)^c1^k0, lo(p1), hi(p0)^c3^k1, lo(p0)); key += (0x9E3779B9, 0xBB67AE85).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+        uint4 n;
+        n.x = hi1 ^ c.y ^ k.x;
+        n.y = lo1;
+        n.z = hi0 ^ c.w ^ k.y;
+        n.w = lo0;
+        c = n;
+        k.x += 0x9E3779B9u;
+        k.y += 0xBB67AE85u;
+    }
+    return c;
+}
+
+// counter = (i lo, i hi, curve b, tag), key = (seed lo, seed hi)
+__device__ __forceinline__ uint4 philox_stream(uint64_t seed, uint64_t i, uint32_t b, uint32_t tag) {
+    uint4 c = make_uint4((uint32_t)i, (uint32_t)(i >> 32), b, tag);
+    uint2 k = make_uint2((uint32_t)seed, (uint32_t)(seed >> 32));
+    return philox4x32_10(c, k);
+}
+
+// u = (2*(wa*2^20 + (wb>>12)) + 1) * 2^-53, exact in fp64, in (0,1)
+__device__ __forceinline__ double u53(uint32_t wa, uint32_t wb) {
+    uint64_t m = ((uint64_t)wa << 20) + (uint64_t)(wb >> 12);
+    return (double)(2 * m + 1) * (1.0 / 9007199254740992.0);
+}
+
+// ------------------------------------------------------------------------------------------------
+// order-preserving radix keys; -0 is canonicalised to +0 (Q13) so that bitwise order == '<' order
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t key_of(float v) {
+    uint32_t u = __float_as_uint(v);
+    if (u == 0x80000000u) u = 0u;
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ uint64_t key_of(double v) {
+    uint64_t u = (uint64_t)__double_as_longlong(v);
+    if (u == 0x8000000000000000ull) u = 0ull;
+    return (u & 0x8000000000000000ull) ? ~u : (u | 0x8000000000000000ull);
+}
+__device__ __forceinline__ float val_of(uint32_t k) {
+    uint32_t u = (k & 0x80000000u) ? (k & 0x7FFFFFFFu) : ~k;
+    return __uint_as_float(u);
+}
+__device__ __forceinline__ double val_of(uint64_t k) {
+    uint64_t u = (k & 0x8000000000000000ull) ? (k & 0x7FFFFFFFFFFFFFFFull) : ~k;
+    return __longlong_as_double((long long)u);
+}
+
+template <typename T> struct KeyT;
+template <> struct KeyT<float> { typedef uint32_t type; static constexpr int bits = 32; };
+template <> struct KeyT<double> { typedef uint64_t type; static constexpr int bits = 64; };
+
+// ------------------------------------------------------------------------------------------------
+// accurate sin/cos of 2*pi*num/den for integer num in [0, den), den a power of two (exact argument)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void sincos_2pi_frac(uint64_t num, int log_den, double* s, double* c) {
+    // 2*num/den is exact in fp64 (num < 2^53)
+    double a = ldexp((double)num, 1 - log_den);
+    sincospi(a, s, c);
+}
+
+// batch index spread over grid y and z (gridDim.y is limited to 65535)
+__device__ __forceinline__ long long bidx() { return (long long)blockIdx.z * gridDim.y + blockIdx.y; }
+static inline dim3 bgrid(unsigned x, long long nb) {
+    unsigned gy = nb > 32768 ? 32768u : (unsigned)nb;
+    unsigned gz = (unsigned)((nb + gy - 1) / gy);
+    return dim3(x, gy, gz);
+}
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace agn

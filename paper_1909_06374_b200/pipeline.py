@@ -1,0 +1,33 @@
+"""One pass of the whole hot path (S1, S2, L1-L6, P) for one batch of curves.
+
+Pure sequencing of the C-ABI calls; no arithmetic of the method happens here.
+"""
+import torch
+
+from . import binding as _b
+from . import workloads as _w
+
+
+def generate_light_curves(cfg, device="cuda", host_out=None, want_hist=False, curve0=0):
+    """Run erdf_sample_sorted -> tk_generate -> e13_iterate (-> periodogram if cfg['nbins']) for cfg
+    (a dict from workloads.config).  Returns dict(x, perm, iters_used, changed_hist, pbin, counts).
+
+    host_out: optional pinned host tensor [B][N]; when given, the final light curves are copied into it
+    (device -> host) on the current stream and the call synchronises, so that the result is usable on
+    return -- this is the end-to-end entry point timed by bench.py's e2e leg.
+    """
+    B, N = cfg["B"], cfg["N"]
+    srt, perm, _ = _b.agnvar_erdf_sample_sorted(cfg["erdf"], B, N, cfg["dtype"], cfg["seed"], curve0,
+                                                cfg["grid_points"], device=device)
+    _, anorm = _b.agnvar_tk_generate(cfg["psd"], B, N, cfg["dt"], cfg["oversample"], cfg["dtype"], cfg["seed"],
+                                     curve0, want_xnorm=False, device=device)
+    out = _b.agnvar_e13_iterate(anorm, srt, perm, cfg["max_iter"], want_hist=want_hist)
+    out["pbin"] = out["counts"] = None
+    if cfg.get("nbins", 0):
+        out["pbin"], out["counts"] = _b.agnvar_periodogram(out["x"], cfg["dt"], 0,
+                                                           _w.log_bin_edges(N, cfg["nbins"]))
+    if host_out is not None:
+        host_out.copy_(out["x"], non_blocking=True)
+        out["iters_host"] = out["iters_used"].cpu()  # synchronises the stream
+        out["x_host"] = host_out
+    return out

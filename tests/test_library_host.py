@@ -1,0 +1,74 @@
+"""CPU-side checks of the product library: it builds for sm_100a, loads, exports every symbol that
+include/agnvar.h declares, and its argument validation (which runs before any launch) returns the
+documented status codes.  No compute call is made (no GPU here)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    from paper_1909_06374_b200 import binding
+    return binding.lib()
+
+
+def test_exports_match_header(L):
+    hdr = open(os.path.join(ROOT, "include", "agnvar.h")).read()
+    declared = set(re.findall(r"\b(agnvar_[a-z0-9_]+)\s*\(", hdr))
+    from paper_1909_06374_b200 import binding
+    assert declared == set(binding.EXPORTS)
+    for name in declared:
+        assert getattr(L, name) is not None
+
+
+def test_built_for_sm_100a():
+    from paper_1909_06374_b200 import _build
+    import subprocess
+    out = subprocess.run(["cuobjdump", "-lelf", _build.LIB], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+
+
+def test_workspace_query_and_validation(L):
+    from paper_1909_06374_b200 import binding as b
+    assert b.workspace_bytes(b.OP_E13_ITERATE, 4, 2 ** 26, "f32") > 4 * 2 ** 26 * 4
+    assert b.workspace_bytes(b.OP_E13_ITERATE, 4, 2 ** 26 + 2, "f32") == 0
+    assert b.workspace_bytes(b.OP_E13_ITERATE, 4, 2, "f32") == 0
+    assert b.workspace_bytes(b.OP_E13_ITERATE, 4, 2 ** 28, "f32") == 0
+    assert b.workspace_bytes(b.OP_TK_GENERATE, 4, 4096, "f64", 3) == 0
+    assert b.workspace_bytes(b.OP_TK_GENERATE, 4, 4096, "f64", 10) > 0
+    assert b.workspace_bytes(b.OP_ERDF_SAMPLE_SORTED, 4, 4096, "f64", 1, 1) == 0
+    assert b.workspace_bytes(99, 4, 4096, "f64") == 0
+    # EINVAL is returned before any launch, so these are safe without a device
+    psd = b.agnvar_psd(0.0, -1.0, 1.0, 2.0)
+    one = C.c_void_p(256)
+    assert L.agnvar_tk_generate(C.byref(psd), 1, 1, 1024, 1.0, 1, 0, 0, 0, one, one, one, 1 << 40, None) == 1
+    good = b.agnvar_psd(0.0, 0.01, 1.0, 2.0)
+    assert L.agnvar_tk_generate(C.byref(good), 1, 1, 1000, 1.0, 1, 0, 0, 0, one, one, one, 1 << 40, None) == 1
+    assert L.agnvar_tk_generate(C.byref(good), 1, 1, 1024, 1.0, 1, 0, 0, 0, None, None, one, 1 << 40, None) == 1
+    assert L.agnvar_tk_generate(C.byref(good), 1, 1, 2 ** 27, 1.0, 4, 0, 0, 0, one, one, one, 1 << 40, None) == 4
+    assert L.agnvar_e13_iterate(1, 1024, 0, one, one, one, one, 0, None, None, None, one, 1 << 40, None) == 1
+    assert L.agnvar_e13_iterate(1, 1024, 7, one, one, one, one, 1, None, None, None, one, 1 << 40, None) == 1
+    assert L.agnvar_e13_iterate(1, 1024, 0, one, one, one, one, 1, None, None, None, one, 16, None) == 2
+    e = b.agnvar_erdf(0, 0, 0.1, 0.4, 2.4, 0.0, 1.0, 1e-4, 1e-5)
+    assert L.agnvar_erdf_sample_sorted(C.byref(e), 1, 1, 1024, 0, 0, 0, 4096, one, one, None, one, 1 << 40, None) == 1
+    edges = (C.c_int64 * 3)(1, 5, 4)
+    assert L.agnvar_periodogram(1, 1024, 0, one, 1.0, 0, 2, edges, one, None, one, 1 << 40, None) == 1
+    assert L.agnvar_psd_bpl(None, -1, C.byref(good), None, None) == 1
+    assert L.agnvar_philox_u32(0, 0, -1, 0, 0, None, None) == 1
+    assert L.agnvar_strerror(1).decode() == "invalid argument"
+    assert b"sm_100a" in L.agnvar_version()
+
+
+def test_workloads_are_seeded_and_shaped():
+    from paper_1909_06374_b200 import workloads as w
+    c2a, c2b = w.config("C2", B=8), w.config("C2", B=8)
+    assert c2a["psd"] == c2b["psd"] and len(c2a["psd"]) == 8
+    assert all(1e-3 <= p["f_b"] <= 2e-2 for p in c2a["psd"])
+    c4 = w.config("C4")
+    assert (c4["B"], c4["N"], c4["max_iter"], c4["dtype"]) == (4, 2 ** 26, 50, "f32")
+    e = w.log_bin_edges(2 ** 20, 64)
+    assert e[0] == 1 and e[-1] == 2 ** 19 + 1 and all(a < b for a, b in zip(e, e[1:]))
