@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
+#include <stdlib.h>
 
 namespace agn {
 
@@ -115,5 +116,53 @@ static inline dim3 bgrid(unsigned x, long long nb) {
 }
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ------------------------------------------------------------------------------------------------
+// launch trace (agnvar_trace_start / agnvar_trace_stop): when enabled, every kernel launch of the
+// library is bracketed by two CUDA events on its stream, so that a caller can read per-kernel device
+// time and launch counts of exactly the launches it timed.  Off by default (zero cost).
+// ------------------------------------------------------------------------------------------------
+enum KernelId {
+    K_FFT_STRIDED = 0, K_FFT_CONTIG, K_REPLACE, K_SORT_CTA, K_SORT_HIST, K_SORT_SWEEP, K_SCATTER, K_ITER_POST,
+    K_PERM_ANORM, K_TK_FILL, K_TK_COMBINE, K_UNTANGLE_OUT, K_PSD, K_ERDF_TABLE, K_ERDF_SAMPLE, K_PGRAM, K_TABLES,
+    K_COPY, K_PHILOX, K_NIDS
+};
+static const char* const kKernelNames[K_NIDS] = {
+    "fft_pass_strided", "fft_pass_contiguous", "amplitude_replace", "cta_argsort", "sort_digit_hist",
+    "sort_onesweep", "rank_scatter_count", "iter_bookkeeping", "perm_anorm", "tk_fill", "tk_combine5_crop",
+    "untangle_out", "psd", "erdf_table", "erdf_sample", "periodogram_scale_bin", "twiddle_tables", "copy", "philox"};
+
+struct TraceRec { int id; cudaEvent_t e0, e1; };
+struct TraceState {
+    bool on = false;
+    TraceRec* recs = nullptr;
+    size_t n = 0, cap = 0;
+    cudaEvent_t* pool = nullptr;
+    size_t pool_n = 0, pool_used = 0;
+};
+inline TraceState& trace_state() { static TraceState s; return s; }
+inline cudaEvent_t trace_event() {
+    TraceState& t = trace_state();
+    if (t.pool_used == t.pool_n) {
+        size_t nn = t.pool_n ? t.pool_n * 2 : 1024;
+        t.pool = (cudaEvent_t*)realloc(t.pool, nn * sizeof(cudaEvent_t));
+        for (size_t i = t.pool_n; i < nn; ++i) cudaEventCreate(&t.pool[i]);
+        t.pool_n = nn;
+    }
+    return t.pool[t.pool_used++];
+}
+struct TraceScope {
+    cudaStream_t st; bool on;
+    TraceScope(int id, cudaStream_t s) : st(s), on(trace_state().on) {
+        if (!on) return;
+        TraceState& t = trace_state();
+        if (t.n == t.cap) { t.cap = t.cap ? t.cap * 2 : 1024; t.recs = (TraceRec*)realloc(t.recs, t.cap * sizeof(TraceRec)); }
+        TraceRec& r = t.recs[t.n++];
+        r.id = id; r.e0 = trace_event(); r.e1 = trace_event();
+        cudaEventRecord(r.e0, st);
+    }
+    ~TraceScope() { if (on) cudaEventRecord(trace_state().recs[trace_state().n - 1].e1, st); }
+};
+#define AGN_TRACE(id, st) ::agn::TraceScope _agn_trace_scope_((id), (st))
 
 }  // namespace agn
