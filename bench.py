@@ -1,0 +1,332 @@
+#!/usr/bin/env python
+"""bench.py -- the headline benchmark: E13 light-curve samples x iterations per second on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl agnvar|reference] [--workload C4]
+
+One "step" = one pass of the whole hot path (S1 ERDF draw + sort, S2 TK generate,
+max_iter x [L1 FFT, L2 replace, L3 IFFT, L4 argsort, L5 scatter+count, L6 bookkeeping], P periodogram
+where the configuration asks for it) over one batch of synthetic curves of BASELINE.json's configuration
+(default C4: B=4, N=2^26, fp32, 50 iterations -- the configuration the metric is quoted on).
+Prints ONE JSON line (rank 0).  N > 1: launched by torchrun, one rank per GPU, every rank runs its own
+batch of curves (curve numbers rank*B ...; no data-path collective; weak scaling).
+
+--impl reference times the CPU oracle (oracle/, fp64, plain) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "E13 samples x iterations / s"
+UNIT = "samples*iterations/s"
+
+# Algorithmic (compulsory) bytes per light-curve sample and launch, fp32, by kernel family: every input
+# read once, every output written once.  w = 4 bytes per value.
+ALGO_BYTES_PER_SAMPLE = {
+    "fft_pass_strided": 8.0,        # read + write one complex half-length array = 4 + 4 B per real sample
+    "fft_pass_contiguous": 8.0,
+    "fft_mid_fused": 10.0,          # read Z 4 + A_norm 2 + write Z' 4
+    "amplitude_replace": 10.0,      # read Z 4 + A_norm 2 + write Z' 4
+    "sort_digit_hist": 4.0,         # read keys
+    "sort_onesweep": 16.0,          # read (key, idx) 8 + write (key, idx) 8 (first/last pass move less)
+    "sort_msd_partition": 12.0,     # read key 4 + write (key, idx) 8
+    "sort_bucket_finish": 12.0,     # read (key, idx) 8 + write idx 4
+    "cta_argsort": 8.0,             # read key 4 + write idx 4
+    "rank_scatter_count": 16.0,     # idx_new 4 + idx_old 4 + sorted 4 + write x 4
+    "scatter_bin": 20.0,            # read 12 + write (val, dst) 8
+    "scatter_place": 12.0,          # read 8 + write 4
+}
+# SURVEY.md 8(d) two-level model, bytes per sample per iteration, per stage (fp32)
+STAGE_MODEL_BYTES = {"fft": 26.0, "argsort": 28.0, "scatter": 32.0}
+STAGE_OF = {
+    "fft_pass_strided": "fft", "fft_pass_contiguous": "fft", "amplitude_replace": "fft", "fft_mid_fused": "fft",
+    "sort_digit_hist": "argsort", "sort_onesweep": "argsort", "cta_argsort": "argsort",
+    "sort_msd_partition": "argsort", "sort_bucket_finish": "argsort",
+    "rank_scatter_count": "scatter", "scatter_bin": "scatter", "scatter_place": "scatter",
+}
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload_label(cfg):
+    return (f"{cfg['name']}: B={cfg['B']} curves x N=2^{cfg['N'].bit_length() - 1} samples, {cfg['dtype']}, "
+            f"max_iter={cfg['max_iter']}, oversample={cfg['oversample']}")
+
+
+# ------------------------------------------------------------------------------------------------------
+# the CPU oracle, timed as it stands on a bounded sample (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------------------
+def oracle_sample_inputs(cfg, logn):
+    import numpy as np
+    import oracle
+    N = 1 << logn
+    e, p = cfg["erdf"][0], cfg["psd"][0]
+    srt, perm0, _ = oracle.erdf_sample_sorted(e, cfg["grid_points"], N, cfg["seed"], 0, 0 if cfg["dtype"] == "f32" else 1)
+    tk = oracle.tk_generate(0.0, p["f_b"], p["alpha_low"], p["alpha_high"], N, cfg["dt"], 1, cfg["seed"], 0)
+    return np.ascontiguousarray(tk["A_norm"]), srt, perm0
+
+
+def oracle_time(cfg, logn, iters, inputs=None):
+    import oracle
+    an, srt, perm0 = inputs if inputs is not None else oracle_sample_inputs(cfg, logn)
+    t0 = time.perf_counter()
+    oracle.e13_iterate(an, srt, perm0, iters)
+    dt = time.perf_counter() - t0
+    return (1 << logn) * iters / dt, dt
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    logn = min(22, cfg["N"].bit_length() - 1)
+    iters = 1
+    inputs = oracle_sample_inputs(cfg, logn)
+    for _ in range(args.warmup):
+        oracle_time(cfg, logn, iters, inputs)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_time(cfg, logn, iters, inputs)
+    dt = time.perf_counter() - t0
+    value = args.steps * (1 << logn) * iters / dt
+    sample = (f"1 curve of {cfg['name']}'s PSD/ERDF parameters at N=2^{logn}, {iters} E13 iteration per step "
+              f"(fp64 CPU oracle, 1 thread)")
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": workload_label(cfg), "sample": sample},
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="agnvar", choices=["agnvar", "reference"])
+    ap.add_argument("--workload", default="C4")
+    ap.add_argument("--batch", type=int, default=None, help="override B (subset of the configuration)")
+    ap.add_argument("--max-iter", type=int, default=None, help="override max_iter (NOT the headline configuration)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    from paper_1909_06374_b200 import workloads
+    cfg = workloads.config(args.workload, B=args.batch)
+    if args.max_iter is not None:
+        cfg["max_iter"] = args.max_iter
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    import torch
+    import paper_1909_06374_b200 as ag
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    ag.lib()
+
+    B, N, iters = cfg["B"], cfg["N"], cfg["max_iter"]
+    curve0 = rank * B          # Philox curve numbers of this rank's rows: results do not depend on the partition
+    units_per_step = B * N * iters
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step(host_out=None):
+        return ag.generate_light_curves(cfg, device=dev, host_out=host_out, curve0=curve0)
+
+    # ---- device-resident timing ----------------------------------------------------------------------
+    for _ in range(args.warmup):
+        out = step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    l0 = ag.launch_count()
+    ag.trace_begin()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        out = step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    trace = ag.trace_end()
+    launches = ag.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    iters_used = out["iters_used"].cpu().tolist()
+    del out
+    tmax = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms = float(tmax.item())
+    value = world * units_per_step * args.steps / (ms * 1e-3)
+
+    # ---- per-kernel accounting (CUDA events around every launch of the timed steps) --------------------
+    fam = {}
+    for name, t in trace:
+        f = fam.setdefault(name, [0, 0.0])
+        f[0] += 1
+        f[1] += t
+    peak, peak_src = measured_peaks()
+    kernels = {k: {"launches": v[0], "ms_total": round(v[1], 4), "ms_avg": v[1] / v[0]} for k, v in fam.items()}
+    loop = {k: v for k, v in fam.items() if k in ALGO_BYTES_PER_SAMPLE}
+    roofline = None
+    stages = {}
+    if loop:
+        top = max(loop, key=lambda k: loop[k][1])
+        n_l, t_l = loop[top]
+        bytes_per_launch = ALGO_BYTES_PER_SAMPLE[top] * B * N       # every loop kernel covers the whole batch
+        achieved = bytes_per_launch / (t_l / n_l * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_ms": t_l / n_l,
+                    "share_of_step": t_l / ms}
+        prof = os.path.join(ROOT, "profiles", "traffic.json")     # dram bytes per launch from the committed ncu capture
+        try:
+            with open(prof) as f:
+                roofline["traffic"] = json.load(f).get(top)
+        except Exception:
+            pass
+        # stage view (the north_star target: each stage >= 60% of the HBM roofline on the 2-level byte model)
+        n_iter_total = args.steps * iters
+        for k, v in loop.items():
+            s = stages.setdefault(STAGE_OF[k], 0.0)
+            stages[STAGE_OF[k]] = s + v[1]
+        stages = {s: {"ms_per_iteration": t / n_iter_total,
+                      "model_bytes_per_sample": STAGE_MODEL_BYTES[s],
+                      "achieved_GBps": STAGE_MODEL_BYTES[s] * B * N / (t / n_iter_total * 1e-3) / 1e9,
+                      "frac_of_peak": STAGE_MODEL_BYTES[s] * B * N / (t / n_iter_total * 1e-3) / 1e9 / peak}
+                  for s, t in stages.items()}
+
+    # ---- end to end: host parameters in, light curves out to pinned host memory -------------------------
+    e2e = None
+    if not args.no_e2e:
+        host = torch.empty((B, N), dtype=torch.float32 if cfg["dtype"] == "f32" else torch.float64).pin_memory()
+        step(host_out=host)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            step(host_out=host)     # synchronises: the result is on the host when it returns
+        barrier()
+        dt = time.perf_counter() - t0
+        tm = torch.tensor([dt], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+        h2d = 32 * len(cfg["psd"]) + 64 * len(cfg["erdf"]) + (8 * (cfg["nbins"] + 1) if cfg.get("nbins") else 0)
+        d2h = host.numel() * host.element_size() + 4 * B
+        e2e = {"value": world * units_per_step * args.steps / float(tm.item()), "unit": UNIT,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
+        del host
+
+    # ---- the oracle on this box's host cores (rank 0, N = 1 only) ---------------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        logn = min(23, N.bit_length() - 1)
+        v, dt = oracle_time(cfg, logn, 1)
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"1 curve of {cfg['name']}'s parameters at N=2^{logn}, 1 E13 iteration, fp64, {dt:.1f} s",
+               "host_cores_available": os.cpu_count()}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": cfg["dtype"], "data": "synthetic",
+                "config": {"workload": workload_label(cfg), "curves_per_gpu": B, "iterations_executed": iters,
+                           "iters_used": iters_used[:8], "l2": "inputs larger than L2 (every array >= 1 GiB)"
+                           if B * N * 4 > 2 ** 28 else "arrays smaller than L2: not flushed between steps",
+                           "step": "S1 + S2 + max_iter x (L1..L6) + P"},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "stages": stages,
+                "cpu_baseline": cpu, "kernels": kernels}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

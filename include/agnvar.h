@@ -152,6 +152,20 @@ int agnvar_periodogram(int64_t B, int64_t N, int dtype, const void* d_x, double 
 int agnvar_philox_u32(uint64_t seed, uint64_t i0, int64_t n, uint32_t curve, uint32_t tag, uint32_t* d_out,
                       void* stream);
 
+/* Measurement aids (bench.py's roofline and gpu_launches figures).  Not thread-safe: one host thread
+ * drives the library while a trace is open.
+ *   agnvar_launch_count   kernels launched by the library in this process so far (memsets/copies excluded)
+ *   agnvar_trace_begin    from now on every kernel launch is bracketed by two CUDA events on its stream
+ *   agnvar_trace_end      stops tracing, waits for the recorded events and returns the launches in issue
+ *                         order: h_ids[i] = kernel family (see agnvar_kernel_name), h_ms[i] = device time of
+ *                         launch i in ms.  *h_n receives the number of launches recorded; at most `cap`
+ *                         entries are written.  ECUDA if an event query fails; EINVAL if no trace is open.
+ *   agnvar_kernel_name    name of kernel family `id`, NULL if id is out of range */
+uint64_t agnvar_launch_count(void);
+int agnvar_trace_begin(void);
+int agnvar_trace_end(int64_t cap, int32_t* h_ids, float* h_ms, int64_t* h_n);
+const char* agnvar_kernel_name(int id);
+
 /* Static, never NULL. */
 const char* agnvar_strerror(int status);
 

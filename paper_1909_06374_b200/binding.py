@@ -19,6 +19,7 @@ OP_ERDF_SAMPLE_SORTED, OP_TK_GENERATE, OP_E13_ITERATE, OP_PERIODOGRAM = 1, 2, 3,
 EXPORTS = (
     "agnvar_workspace_bytes", "agnvar_psd_bpl", "agnvar_erdf_sample_sorted", "agnvar_tk_generate",
     "agnvar_e13_iterate", "agnvar_periodogram", "agnvar_philox_u32", "agnvar_strerror", "agnvar_version",
+    "agnvar_launch_count", "agnvar_trace_begin", "agnvar_trace_end", "agnvar_kernel_name",
 )
 
 
@@ -74,6 +75,14 @@ def lib():
     L.agnvar_strerror.argtypes = [i32]
     L.agnvar_version.restype = C.c_char_p
     L.agnvar_version.argtypes = []
+    L.agnvar_launch_count.restype = u64
+    L.agnvar_launch_count.argtypes = []
+    L.agnvar_trace_begin.restype = i32
+    L.agnvar_trace_begin.argtypes = []
+    L.agnvar_trace_end.restype = i32
+    L.agnvar_trace_end.argtypes = [i64, vp, vp, C.POINTER(i64)]
+    L.agnvar_kernel_name.restype = C.c_char_p
+    L.agnvar_kernel_name.argtypes = [i32]
     _lib = L
     return L
 
@@ -84,6 +93,25 @@ def strerror(status):
 
 def version():
     return lib().agnvar_version().decode()
+
+
+def launch_count():
+    """Kernels launched by the library in this process so far."""
+    return int(lib().agnvar_launch_count())
+
+
+def trace_begin():
+    _check(lib().agnvar_trace_begin(), "agnvar_trace_begin")
+
+
+def trace_end(cap=1 << 20):
+    """Returns a list of (kernel family name, device ms) in issue order for every launch since trace_begin()."""
+    ids = (C.c_int32 * cap)()
+    ms = (C.c_float * cap)()
+    n = C.c_int64(0)
+    _check(lib().agnvar_trace_end(cap, ids, ms, C.byref(n)), "agnvar_trace_end")
+    m = min(int(n.value), cap)
+    return [(lib().agnvar_kernel_name(ids[i]).decode(), float(ms[i])) for i in range(m)]
 
 
 # ---- marshalling helpers --------------------------------------------------------------------------

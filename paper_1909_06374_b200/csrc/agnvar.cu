@@ -131,32 +131,32 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
     TwLevel<T> rlv = real_level<T>(plan);
     cudaMemsetAsync(changed, 0, (size_t)B * sizeof(unsigned long long), st);
     cudaMemsetAsync(first_zero, 0, (size_t)B * sizeof(int), st);
-    perm_anorm_kernel<T><<<bgrid(cdiv(L + 1, 256), B), 256, 0, st>>>((const T*)d_anorm, Ap, plan.dg, (int)B);
+    AGN_LAUNCH(K_PERM_ANORM, st, (perm_anorm_kernel<T><<<bgrid(cdiv(L + 1, 256), B), 256, 0, st>>>((const T*)d_anorm, Ap, plan.dg, (int)B)));
     const unsigned sg = (unsigned)std::min<long long>((N + 1023) / 1024, 148 * 16);
     // first x_sim: the draw in draw order (Q15)
-    scatter_count_kernel<T, false><<<bgrid(sg, B), 256, 0, st>>>(d_perm, nullptr, sorted, x, N, nullptr, (int)B);
+    AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, false><<<bgrid(sg, B), 256, 0, st>>>(d_perm, nullptr, sorted, x, N, nullptr, (int)B)));
     uint32_t* cur = d_perm;
     uint32_t* nxt = P1;
     for (int k = 1; k <= max_iter; ++k) {
         // L1 forward FFT (x_sim -> Z, position order)
         fft_forward<T>(plan, (const C*)x, (C*)Z, L, L, (int)B, st);
         // L2 amplitude replace
-        replace_kernel<T><<<bgrid(cdiv(L, 256), B), 256, 0, st>>>((C*)Z, Ap, plan.dg, rlv, (int)B);
+        AGN_LAUNCH(K_REPLACE, st, (replace_kernel<T><<<bgrid(cdiv(L, 256), B), 256, 0, st>>>((C*)Z, Ap, plan.dg, rlv, (int)B)));
         // L3 inverse FFT (Z -> x_adj, natural order, 1/L)
         fft_inverse<T>(plan, (const C*)Z, (C*)Z, L, L, (int)B, (T)(1.0 / (double)L), st);
         // L4 segmented stable argsort
         cudaError_t e = seg_argsort<T>(Z, nxt, nullptr, B, N, sort_ws, st);
         if (e != cudaSuccess) return AGNVAR_ECUDA;
         // L5 rank scatter + change count
-        scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(nxt, cur, sorted, x, N, changed, (int)B);
+        AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(nxt, cur, sorted, x, N, changed, (int)B)));
         // L6 bookkeeping
-        post_iter_kernel<<<cdiv(B, 256), 256, 0, st>>>(changed, first_zero, k, (long long*)d_changed_hist, max_iter, (int)B);
+        AGN_LAUNCH(K_ITER_POST, st, (post_iter_kernel<<<cdiv(B, 256), 256, 0, st>>>(changed, first_zero, k, (long long*)d_changed_hist, max_iter, (int)B)));
         std::swap(cur, nxt);
     }
     if (cur != d_perm) cudaMemcpyAsync(d_perm, cur, (size_t)B * N * 4, cudaMemcpyDeviceToDevice, st);
     if (d_xadj_dbg)
-        copy_canon_kernel<T><<<cdiv(B * N, 256), 256, 0, st>>>(Z, (T*)d_xadj_dbg, (long long)B * N);
-    if (d_iters_used) finalize_iters_kernel<<<cdiv(B, 256), 256, 0, st>>>(first_zero, d_iters_used, max_iter, (int)B);
+        AGN_LAUNCH(K_COPY, st, (copy_canon_kernel<T><<<cdiv(B * N, 256), 256, 0, st>>>(Z, (T*)d_xadj_dbg, (long long)B * N)));
+    if (d_iters_used) AGN_LAUNCH(K_ITER_POST, st, (finalize_iters_kernel<<<cdiv(B, 256), 256, 0, st>>>(first_zero, d_iters_used, max_iter, (int)B)));
     return cuda_status(cudaGetLastError());
 }
 
@@ -192,27 +192,27 @@ int tk_impl(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_t N, double
         long long half = M / 2;
         int nchunks = (int)std::min<long long>(1024, (half + 4095) / 4096);
         int chunk = (int)((half + nchunks - 1) / nchunks);
-        psd_norm_partial_kernel<<<bgrid(nchunks, B), 256, 0, st>>>(psd, M, dt, chunk, partial, nchunks, (int)B);
-        psd_norm_final_kernel<<<(unsigned)B, 256, 0, st>>>(psd, partial, nchunks, M);
+        AGN_LAUNCH(K_PSD, st, (psd_norm_partial_kernel<<<bgrid(nchunks, B), 256, 0, st>>>(psd, M, dt, chunk, partial, nchunks, (int)B)));
+        AGN_LAUNCH(K_PSD, st, (psd_norm_final_kernel<<<(unsigned)B, 256, 0, st>>>(psd, partial, nchunks, M)));
     }
     T* xsrc;   // where x_norm ends up
     if (five) {
         const int64_t Mp = M / 5;
         const int logMp = ilog2_u64((uint64_t)Mp);
         FftPlan<T> pm = fft_plan_init<T>(logMp, tabM, st);
-        tk_fill5_kernel<T><<<bgrid(cdiv(Mp, 256), 3 * B), 256, 0, st>>>((C*)ZM, psd, pm.dg, dt, seed, curve0, (int)B);
+        AGN_LAUNCH(K_TK_FILL, st, (tk_fill5_kernel<T><<<bgrid(cdiv(Mp, 256), 3 * B), 256, 0, st>>>((C*)ZM, psd, pm.dg, dt, seed, curve0, (int)B)));
         fft_inverse<T>(pm, (const C*)ZM, (C*)ZM, Mp, Mp, (int)(3 * B), (T)1, st);
-        tk_combine5_kernel<T><<<bgrid(cdiv(N, 256), B), 256, 0, st>>>((const C*)ZM, xn, Mp, N, (M - N) / 2, (int)B);
+        AGN_LAUNCH(K_TK_COMBINE, st, (tk_combine5_kernel<T><<<bgrid(cdiv(N, 256), B), 256, 0, st>>>((const C*)ZM, xn, Mp, N, (M - N) / 2, (int)B)));
         xsrc = xn;
     } else {
         const int logLM = ilog2_u64((uint64_t)M) - 1;
         const long long LM = M / 2;
         FftPlan<T> pm = fft_plan_init<T>(logLM, tabM, st);
-        tk_fill_kernel<T><<<bgrid(cdiv(LM, 256), B), 256, 0, st>>>((C*)ZM, psd, pm.dg, dt, seed, curve0, (int)B);
+        AGN_LAUNCH(K_TK_FILL, st, (tk_fill_kernel<T><<<bgrid(cdiv(LM, 256), B), 256, 0, st>>>((C*)ZM, psd, pm.dg, dt, seed, curve0, (int)B)));
         fft_inverse<T>(pm, (const C*)ZM, (C*)ZM, LM, LM, (int)B, (T)(1.0 / (double)LM), st);
         if (os == 1) xsrc = ZM;
         else {
-            crop_kernel<T><<<bgrid(cdiv(N, 256), B), 256, 0, st>>>(ZM, M, (M - N) / 2, xn, N, (int)B);
+            AGN_LAUNCH(K_TK_COMBINE, st, (crop_kernel<T><<<bgrid(cdiv(N, 256), B), 256, 0, st>>>(ZM, M, (M - N) / 2, xn, N, (int)B)));
             xsrc = xn;
         }
     }
@@ -222,8 +222,8 @@ int tk_impl(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_t N, double
         const long long L = N / 2;
         FftPlan<T> pn = fft_plan_init<T>(logL, tabN, st);
         fft_forward<T>(pn, (const C*)xsrc, (C*)ZN, L, L, (int)B, st);
-        untangle_out_kernel<T, 0><<<bgrid(cdiv(L, 256), B), 256, 0, st>>>((const C*)ZN, pn.dg, real_level<T>(pn),
-                                                                          (T*)d_anorm, nullptr, nullptr, (int)B);
+        AGN_LAUNCH(K_UNTANGLE_OUT, st, (untangle_out_kernel<T, 0><<<bgrid(cdiv(L, 256), B), 256, 0, st>>>((const C*)ZN, pn.dg, real_level<T>(pn),
+                                                                          (T*)d_anorm, nullptr, nullptr, (int)B)));
     }
     return cuda_status(cudaGetLastError());
 }
@@ -248,9 +248,9 @@ int erdf_impl(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t B, int64_t N, u
     }
     if (cudaMemcpyAsync(erdf, he.data(), (size_t)n_erdf * sizeof(ErdfDev), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return AGNVAR_ECUDA;
-    erdf_table_kernel<<<(unsigned)n_erdf, 256, 0, st>>>(erdf, G, Ctab);
-    erdf_sample_kernel<T><<<bgrid(cdiv(N / 2, 256), B), 256, 0, st>>>(erdf, n_erdf == 1 ? 0 : 1, Ctab, G, N, seed,
-                                                                      curve0, draw, (int)B);
+    AGN_LAUNCH(K_ERDF_TABLE, st, (erdf_table_kernel<<<(unsigned)n_erdf, 256, 0, st>>>(erdf, G, Ctab)));
+    AGN_LAUNCH(K_ERDF_SAMPLE, st, (erdf_sample_kernel<T><<<bgrid(cdiv(N / 2, 256), B), 256, 0, st>>>(erdf, n_erdf == 1 ? 0 : 1, Ctab, G, N, seed,
+                                                                      curve0, draw, (int)B)));
     // stable ascending sort carrying the draw index; perm0 is needed internally even if the caller
     // does not want it -> use the tail of the sort workspace? no: sort straight into d_perm0 or a scratch
     uint32_t* perm = d_perm0;
@@ -276,15 +276,15 @@ int pgram_impl(int64_t B, int64_t N, const void* d_x, double dt, int norm, int n
     const int logL = ilog2_u64((uint64_t)N) - 1;
     const long long L = N / 2;
     FftPlan<T> plan = fft_plan_init<T>(logL, tables, st);
-    pgram_scale_kernel<T><<<(unsigned)B, 256, 0, st>>>((const T*)d_x, N, dt, norm, scale);
+    AGN_LAUNCH(K_PGRAM, st, (pgram_scale_kernel<T><<<(unsigned)B, 256, 0, st>>>((const T*)d_x, N, dt, norm, scale)));
     fft_forward<T>(plan, (const C*)d_x, (C*)Z, L, L, (int)B, st);
     double* Pout = nbins > 0 ? P : d_out;
-    untangle_out_kernel<T, 1><<<bgrid(cdiv(L, 256), B), 256, 0, st>>>((const C*)Z, plan.dg, real_level<T>(plan), nullptr,
-                                                                      Pout, scale, (int)B);
+    AGN_LAUNCH(K_UNTANGLE_OUT, st, (untangle_out_kernel<T, 1><<<bgrid(cdiv(L, 256), B), 256, 0, st>>>((const C*)Z, plan.dg, real_level<T>(plan), nullptr,
+                                                                      Pout, scale, (int)B)));
     if (nbins > 0) {
         if (cudaMemcpyAsync(edges, h_edges, (size_t)(nbins + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st) != cudaSuccess)
             return AGNVAR_ECUDA;
-        pgram_bin_kernel<<<bgrid((unsigned)nbins, B), 256, 0, st>>>(P, L, edges, nbins, d_out, (long long*)d_counts, (int)B);
+        AGN_LAUNCH(K_PGRAM, st, (pgram_bin_kernel<<<bgrid((unsigned)nbins, B), 256, 0, st>>>(P, L, edges, nbins, d_out, (long long*)d_counts, (int)B)));
     }
     return cuda_status(cudaGetLastError());
 }
@@ -308,6 +308,38 @@ const char* agnvar_strerror(int status) {
 }
 
 const char* agnvar_version(void) { return "agnvar 0.1 (sm_100a)"; }
+
+uint64_t agnvar_launch_count(void) { return trace_state().launches; }
+
+int agnvar_trace_begin(void) {
+    TraceState& t = trace_state();
+    t.n = 0;
+    t.pool_used = 0;
+    t.on = true;
+    return AGNVAR_OK;
+}
+
+int agnvar_trace_end(int64_t cap, int32_t* h_ids, float* h_ms, int64_t* h_n) {
+    TraceState& t = trace_state();
+    if (!t.on) return AGNVAR_EINVAL;
+    t.on = false;
+    if (h_n) *h_n = (int64_t)t.n;
+    int rc = AGNVAR_OK;
+    for (size_t i = 0; i < t.n; ++i) {
+        if (cudaEventSynchronize(t.recs[i].e1) != cudaSuccess) { rc = AGNVAR_ECUDA; break; }
+        if ((int64_t)i < cap && h_ids && h_ms) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, t.recs[i].e0, t.recs[i].e1) != cudaSuccess) { rc = AGNVAR_ECUDA; break; }
+            h_ids[i] = t.recs[i].id;
+            h_ms[i] = ms;
+        }
+    }
+    t.n = 0;
+    t.pool_used = 0;
+    return rc;
+}
+
+const char* agnvar_kernel_name(int id) { return (id >= 0 && id < K_NIDS) ? kKernelNames[id] : nullptr; }
 
 size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int oversample, int64_t aux) {
     if (!valid_BN(B, N) || !valid_dtype(dtype)) return 0;
@@ -333,7 +365,7 @@ int agnvar_philox_u32(uint64_t seed, uint64_t i0, int64_t n, uint32_t curve, uin
     if (n < 0) return AGNVAR_EINVAL;
     if (n == 0) return AGNVAR_OK;
     if (!d_out) return AGNVAR_EINVAL;
-    philox_words_kernel<<<cdiv(n, 256), 256, 0, (cudaStream_t)stream>>>(seed, i0, n, curve, tag, (uint4*)d_out);
+    AGN_LAUNCH(K_PHILOX, (cudaStream_t)stream, (philox_words_kernel<<<cdiv(n, 256), 256, 0, (cudaStream_t)stream>>>(seed, i0, n, curve, tag, (uint4*)d_out)));
     return cuda_status(cudaGetLastError());
 }
 
@@ -345,7 +377,7 @@ int agnvar_psd_bpl(const double* d_f, int64_t n, const agnvar_psd* h_p, double* 
     if (n == 0) return AGNVAR_OK;
     if (!d_f || !d_out) return AGNVAR_EINVAL;
     PsdDev p{h_p->A, h_p->f_b, h_p->alpha_low, h_p->alpha_high};
-    psd_bpl_kernel<<<cdiv(n, 256), 256, 0, (cudaStream_t)stream>>>(d_f, n, p, d_out);
+    AGN_LAUNCH(K_PSD, (cudaStream_t)stream, (psd_bpl_kernel<<<cdiv(n, 256), 256, 0, (cudaStream_t)stream>>>(d_f, n, p, d_out)));
     return cuda_status(cudaGetLastError());
 }
 

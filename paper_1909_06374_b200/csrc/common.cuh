@@ -135,6 +135,7 @@ static const char* const kKernelNames[K_NIDS] = {
 struct TraceRec { int id; cudaEvent_t e0, e1; };
 struct TraceState {
     bool on = false;
+    unsigned long long launches = 0;   // every kernel launch of the library, traced or not
     TraceRec* recs = nullptr;
     size_t n = 0, cap = 0;
     cudaEvent_t* pool = nullptr;
@@ -154,8 +155,9 @@ inline cudaEvent_t trace_event() {
 struct TraceScope {
     cudaStream_t st; bool on;
     TraceScope(int id, cudaStream_t s) : st(s), on(trace_state().on) {
-        if (!on) return;
         TraceState& t = trace_state();
+        ++t.launches;
+        if (!on) return;
         if (t.n == t.cap) { t.cap = t.cap ? t.cap * 2 : 1024; t.recs = (TraceRec*)realloc(t.recs, t.cap * sizeof(TraceRec)); }
         TraceRec& r = t.recs[t.n++];
         r.id = id; r.e0 = trace_event(); r.e1 = trace_event();
@@ -164,5 +166,7 @@ struct TraceScope {
     ~TraceScope() { if (on) cudaEventRecord(trace_state().recs[trace_state().n - 1].e1, st); }
 };
 #define AGN_TRACE(id, st) ::agn::TraceScope _agn_trace_scope_((id), (st))
+// one kernel launch, counted and (when tracing) timed
+#define AGN_LAUNCH(id, st, ...) do { ::agn::TraceScope _agn_ts_((id), (st)); __VA_ARGS__; } while (0)
 
 }  // namespace agn

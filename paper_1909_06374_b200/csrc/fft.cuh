@@ -320,14 +320,14 @@ inline FftPlan<T> fft_plan_init(int logL, typename Cx<T>::type* tables, cudaStre
     FftPlan<T> p;
     p.dg = make_digits<T>(logL);
     C* t = tables;
-    tw_init_kernel<T><<<(1 << kLogTw) / 256, 256, 0, st>>>(t, 1 << kLogTw, kLogTw);
+    AGN_LAUNCH(K_TABLES, st, (tw_init_kernel<T><<<(1 << kLogTw) / 256, 256, 0, st>>>(t, 1 << kLogTw, kLogTw)));
     p.tw14 = t; t += (size_t)1 << kLogTw;
     int logLi = logL;
     for (int i = 0; i < kMaxPass; ++i) {
         p.lo[i] = nullptr;
         if (i < p.dg.n) {
             if (logLi > kLogTw && i < p.dg.n - 1) {
-                tw_init_kernel<T><<<(1 << kLogLo) / 256, 256, 0, st>>>(t, 1 << kLogLo, logLi);
+                AGN_LAUNCH(K_TABLES, st, (tw_init_kernel<T><<<(1 << kLogLo) / 256, 256, 0, st>>>(t, 1 << kLogLo, logLi)));
                 p.lo[i] = t;
             }
             logLi -= p.dg.lg[i];
@@ -336,7 +336,7 @@ inline FftPlan<T> fft_plan_init(int logL, typename Cx<T>::type* tables, cudaStre
     }
     p.lo_real = nullptr;
     if (logL + 1 > kLogTw) {
-        tw_init_kernel<T><<<(1 << kLogLo) / 256, 256, 0, st>>>(t, 1 << kLogLo, logL + 1);
+        AGN_LAUNCH(K_TABLES, st, (tw_init_kernel<T><<<(1 << kLogLo) / 256, 256, 0, st>>>(t, 1 << kLogLo, logL + 1)));
         p.lo_real = t;
     }
     return p;
@@ -379,8 +379,8 @@ inline void fft_launch_pass(const FftPlan<T>& p, int i, bool inverse, const type
     long long tiles = (a.total + (1ll << FftCfg<T>::logE) - 1) >> FftCfg<T>::logE;
     a.nbatch = gy;
     dim3 grid = bgrid((unsigned)tiles, gy);
-    fft_pass_kernel<T, kFftThreads, FftCfg<T>::EPT>
-        <<<grid, kFftThreads, fft_smem_bytes<T>(contiguous), st>>>(a);
+    AGN_LAUNCH((contiguous ? K_FFT_CONTIG : K_FFT_STRIDED), st, (fft_pass_kernel<T, kFftThreads, FftCfg<T>::EPT>
+        <<<grid, kFftThreads, fft_smem_bytes<T>(contiguous), st>>>(a)));
 }
 
 // forward complex FFT: in (natural) -> out (position order).  in may equal out.

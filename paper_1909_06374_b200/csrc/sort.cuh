@@ -324,13 +324,13 @@ inline cudaError_t seg_argsort(const T* vals, uint32_t* idx_out, T* sorted_out, 
     constexpr int NP = SortCfg<T>::NP;
     if (N <= SortCfg<T>::ctaMax) {
         if (N <= 1024)
-            cta_argsort_kernel<T, 256, 4><<<(unsigned)B, 256, cta_sort_smem<T, 256, 4>(), st>>>(vals, idx_out, sorted_out, (int)N, N);
+            AGN_LAUNCH(K_SORT_CTA, st, (cta_argsort_kernel<T, 256, 4><<<(unsigned)B, 256, cta_sort_smem<T, 256, 4>(), st>>>(vals, idx_out, sorted_out, (int)N, N)));
         else if (N <= 4096)
-            cta_argsort_kernel<T, 512, 8><<<(unsigned)B, 512, cta_sort_smem<T, 512, 8>(), st>>>(vals, idx_out, sorted_out, (int)N, N);
+            AGN_LAUNCH(K_SORT_CTA, st, (cta_argsort_kernel<T, 512, 8><<<(unsigned)B, 512, cta_sort_smem<T, 512, 8>(), st>>>(vals, idx_out, sorted_out, (int)N, N)));
         else if (N <= 8192)
-            cta_argsort_kernel<T, 1024, 8><<<(unsigned)B, 1024, cta_sort_smem<T, 1024, 8>(), st>>>(vals, idx_out, sorted_out, (int)N, N);
+            AGN_LAUNCH(K_SORT_CTA, st, (cta_argsort_kernel<T, 1024, 8><<<(unsigned)B, 1024, cta_sort_smem<T, 1024, 8>(), st>>>(vals, idx_out, sorted_out, (int)N, N)));
         else
-            cta_argsort_kernel<T, 1024, 16><<<(unsigned)B, 1024, cta_sort_smem<T, 1024, 16>(), st>>>(vals, idx_out, sorted_out, (int)N, N);
+            AGN_LAUNCH(K_SORT_CTA, st, (cta_argsort_kernel<T, 1024, 16><<<(unsigned)B, 1024, cta_sort_smem<T, 1024, 16>(), st>>>(vals, idx_out, sorted_out, (int)N, N)));
         return cudaGetLastError();
     }
     constexpr int TH = SortCfg<T>::SW_THREADS, K = SortCfg<T>::SW_KPT, TILE = SortCfg<T>::SW_TILE;
@@ -348,7 +348,7 @@ inline cudaError_t seg_argsort(const T* vals, uint32_t* idx_out, T* sorted_out, 
     if (e != cudaSuccess) return e;
     const int chunk = 1 << 16;
     dim3 hg = bgrid((unsigned)((N + chunk - 1) / chunk), B);
-    digit_hist_kernel<T, 512><<<hg, 512, 0, st>>>(vals, hist, N, N, chunk, B);
+    AGN_LAUNCH(K_SORT_HIST, st, (digit_hist_kernel<T, 512><<<hg, 512, 0, st>>>(vals, hist, N, N, chunk, B)));
     const size_t sm = cta_sort_smem<T, TH, K>();
     dim3 grid = bgrid((unsigned)ntiles, B);
     for (int p = 0; p < NP; ++p) {
@@ -365,9 +365,9 @@ inline cudaError_t seg_argsort(const T* vals, uint32_t* idx_out, T* sorted_out, 
         a.status = status + (size_t)p * B * ntiles * kRadix;
         a.ticket = ticket + (size_t)p * B;
         a.ntiles = (int)ntiles; a.B = B;
-        if (p == 0) onesweep_kernel<T, TH, K, true, false><<<grid, TH, sm, st>>>(a);
-        else if (p == NP - 1) onesweep_kernel<T, TH, K, false, true><<<grid, TH, sm, st>>>(a);
-        else onesweep_kernel<T, TH, K, false, false><<<grid, TH, sm, st>>>(a);
+        if (p == 0) AGN_LAUNCH(K_SORT_SWEEP, st, (onesweep_kernel<T, TH, K, true, false><<<grid, TH, sm, st>>>(a)));
+        else if (p == NP - 1) AGN_LAUNCH(K_SORT_SWEEP, st, (onesweep_kernel<T, TH, K, false, true><<<grid, TH, sm, st>>>(a)));
+        else AGN_LAUNCH(K_SORT_SWEEP, st, (onesweep_kernel<T, TH, K, false, false><<<grid, TH, sm, st>>>(a)));
     }
     (void)TILE;
     return cudaGetLastError();
