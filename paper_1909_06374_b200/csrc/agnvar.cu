@@ -62,6 +62,7 @@ template <typename T> size_t ws_e13(int64_t B, int64_t N) {
     c.take<uint32_t>((size_t)B * N);          // permutation ping-pong
     c.take<unsigned long long>((size_t)B);    // changed counters
     c.take<int>((size_t)B);                   // first_zero
+    c.take<uint32_t>((size_t)B * kRadix);     // bin cursors of the two-level scatter
     return c.off + sort_ws_bytes<T>(B, N);
 }
 template <typename T> size_t ws_tk(int64_t B, int64_t N, int os) {
@@ -123,7 +124,12 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
     uint32_t* P1 = c.take<uint32_t>((size_t)B * N);
     unsigned long long* changed = c.take<unsigned long long>((size_t)B);
     int* first_zero = c.take<int>((size_t)B);
+    uint32_t* cursor = c.take<uint32_t>((size_t)B * kRadix);
     void* sort_ws = (unsigned char*)d_ws + c.off;
+    const bool two_level = N >= (1ll << kTwoLevelScatterLog);
+    // the binned (value, dst) pairs live in the sort's ping-pong buffers, which are idle after the sort
+    T* pv = (T*)sort_ws;
+    uint32_t* pd = (uint32_t*)((unsigned char*)sort_ws + 2 * align_up((size_t)B * N * sizeof(T), 256));
     T* x = (T*)d_x;
     const T* sorted = (const T*)d_sorted;
 
@@ -131,6 +137,7 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
     TwLevel<T> rlv = real_level<T>(plan);
     cudaMemsetAsync(changed, 0, (size_t)B * sizeof(unsigned long long), st);
     cudaMemsetAsync(first_zero, 0, (size_t)B * sizeof(int), st);
+    cudaMemsetAsync(cursor, 0, (size_t)B * kRadix * sizeof(uint32_t), st);
     AGN_LAUNCH(K_PERM_ANORM, st, (perm_anorm_kernel<T><<<bgrid(cdiv(L + 1, 256), B), 256, 0, st>>>((const T*)d_anorm, Ap, plan.dg, (int)B)));
     const unsigned sg = (unsigned)std::min<long long>((N + 1023) / 1024, 148 * 16);
     // first x_sim: the draw in draw order (Q15)
@@ -148,7 +155,12 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
         cudaError_t e = seg_argsort<T>(Z, nxt, nullptr, B, N, sort_ws, st);
         if (e != cudaSuccess) return AGNVAR_ECUDA;
         // L5 rank scatter + change count
-        AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(nxt, cur, sorted, x, N, changed, (int)B)));
+        if (two_level) {
+            if (rank_scatter_two_level<T>(nxt, cur, sorted, x, B, N, pv, pd, cursor, changed, st) != cudaSuccess)
+                return AGNVAR_ECUDA;
+        } else {
+            AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(nxt, cur, sorted, x, N, changed, (int)B)));
+        }
         // L6 bookkeeping
         AGN_LAUNCH(K_ITER_POST, st, (post_iter_kernel<<<cdiv(B, 256), 256, 0, st>>>(changed, first_zero, k, (long long*)d_changed_hist, max_iter, (int)B)));
         std::swap(cur, nxt);

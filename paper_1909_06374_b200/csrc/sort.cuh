@@ -264,6 +264,90 @@ __global__ void __launch_bounds__(THREADS) onesweep_kernel(SweepArgs<T> a) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// L5 for segments much larger than L2: two-level rank scatter.
+//   bin pass   reads idx_new[r], idx_old[r], sorted[r]; counts idx_new != idx_old; appends (value, dst)
+//              to the bin dst >> shift (256 bins per segment).  idx_new is a permutation, so bin d
+//              receives exactly 2^shift pairs: its region is [d << shift, (d+1) << shift) and only a
+//              cursor per bin is needed (order inside a bin is irrelevant: every pair carries its dst).
+//   place pass streams the pairs of one bin and stores x[dst]; all stores of a bin fall into a window of
+//              2^shift values, which stays in L2 until every sector of it is complete.
+// A direct x[idx_new[r]] = sorted[r] over a 256 MB segment costs a 32-byte sector read-modify-write
+// in HBM per 4-byte value; the two passes move 20 + 12 bytes per value instead.
+// ------------------------------------------------------------------------------------------------
+template <typename T, int THREADS, int KPT>
+__global__ void __launch_bounds__(THREADS) scatter_bin_kernel(const uint32_t* __restrict__ idx_new,
+                                                              const uint32_t* __restrict__ idx_old,
+                                                              const T* __restrict__ sorted, T* __restrict__ pv,
+                                                              uint32_t* __restrict__ pd, long long N, int shift,
+                                                              uint32_t* __restrict__ cursor,
+                                                              unsigned long long* __restrict__ changed, long long B) {
+    constexpr int TILE = THREADS * KPT;
+    constexpr int W = THREADS / 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* sv = reinterpret_cast<T*>(smem_raw);
+    uint32_t* sd = reinterpret_cast<uint32_t*>(sv + TILE);
+    uint32_t* scratch = sd + TILE;
+    uint32_t* tile_off = scratch + W * kRadix;
+    uint32_t* tile_cnt = tile_off + kRadix;
+    __shared__ long long goff[kRadix];
+    __shared__ unsigned int s_diff[W];
+    const long long b = bidx();
+    if (b >= B) return;
+    const long long base = (long long)blockIdx.x * TILE;
+    const long long segoff = b * N;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint32_t dst[KPT], pos[KPT];
+    T val[KPT];
+    unsigned int diff = 0;
+    // N is a multiple of TILE here (N >= 2^22), so every tile is full
+#pragma unroll
+    for (int j = 0; j < KPT; ++j) {
+        long long g = segoff + base + warp * 32 * KPT + j * 32 + lane;
+        dst[j] = idx_new[g];
+        diff += (dst[j] != idx_old[g]);
+        val[j] = sorted[g];
+    }
+    rank_keys<uint32_t, THREADS, KPT>(dst, shift, pos, scratch);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) diff += __shfl_xor_sync(0xffffffffu, diff, o);
+    if (lane == 0) s_diff[warp] = diff;
+    if (threadIdx.x < kRadix) {
+        const int d = threadIdx.x;
+        uint32_t c = tile_cnt[d];
+        uint32_t start = c ? atomicAdd(&cursor[b * kRadix + d], c) : 0u;
+        goff[d] = ((long long)d << shift) + (long long)start - (long long)tile_off[d];
+    }
+#pragma unroll
+    for (int j = 0; j < KPT; ++j) { sv[pos[j]] = val[j]; sd[pos[j]] = dst[j]; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned int t = 0;
+        for (int i = 0; i < W; ++i) t += s_diff[i];
+        if (t) atomicAdd(&changed[b], (unsigned long long)t);
+    }
+    for (int s = threadIdx.x; s < TILE; s += THREADS) {
+        uint32_t d = sd[s];
+        long long g = segoff + goff[(d >> shift) & (kRadix - 1)] + s;
+        pv[g] = sv[s];
+        pd[g] = d;
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) scatter_place_kernel(const T* __restrict__ pv, const uint32_t* __restrict__ pd,
+                                                            T* __restrict__ x, long long N,
+                                                            uint32_t* __restrict__ cursor, long long B) {
+    const long long b = bidx();
+    if (b >= B) return;
+    if (blockIdx.x == 0) cursor[b * kRadix + threadIdx.x] = 0u;     // ready for the next iteration's bin pass
+    const long long off = b * N;
+    const long long g = off + ((long long)blockIdx.x * 256 + threadIdx.x) * 4;     // N is a multiple of 1024
+    uint4 d = *reinterpret_cast<const uint4*>(pd + g);
+    T v0 = pv[g], v1 = pv[g + 1], v2 = pv[g + 2], v3 = pv[g + 3];
+    x[off + d.x] = v0; x[off + d.y] = v1; x[off + d.z] = v2; x[off + d.w] = v3;
+}
+
+// ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
 template <typename T> struct SortCfg {
@@ -277,6 +361,11 @@ template <typename T> struct SortCfg {
 template <typename T, int THREADS, int KPT> inline size_t cta_sort_smem() {
     return (size_t)THREADS * KPT * (sizeof(typename KeyT<T>::type) + 4) + RankScratch<THREADS>::words * 4;
 }
+
+template <typename T, int THREADS, int KPT> inline size_t scatter_bin_smem() {
+    return (size_t)THREADS * KPT * (sizeof(T) + 4) + RankScratch<THREADS>::words * 4;
+}
+constexpr int kTwoLevelScatterLog = 22;     // segments of >= 2^22 values use the two-level rank scatter
 
 template <typename T> inline long long sort_ntiles(long long N) { return (N + SortCfg<T>::SW_TILE - 1) / SortCfg<T>::SW_TILE; }
 
@@ -307,7 +396,10 @@ template <typename T> inline cudaError_t sort_set_attrs() {
     cudaError_t e4 = cudaFuncSetAttribute(onesweep_kernel<T, TH, K, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
     cudaError_t e5 = cudaFuncSetAttribute(onesweep_kernel<T, TH, K, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
     cudaError_t e6 = cudaFuncSetAttribute(onesweep_kernel<T, TH, K, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
+    cudaError_t e7 = cudaFuncSetAttribute(scatter_bin_kernel<T, TH, K>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)scatter_bin_smem<T, TH, K>());
     (void)cudaGetLastError();
+    if (e7 != cudaSuccess) return e7;
     if (e != cudaSuccess) return e;
     if (e2 != cudaSuccess) return e2;
     if (e3 != cudaSuccess) return e3;
@@ -370,6 +462,20 @@ inline cudaError_t seg_argsort(const T* vals, uint32_t* idx_out, T* sorted_out, 
         else AGN_LAUNCH(K_SORT_SWEEP, st, (onesweep_kernel<T, TH, K, false, false><<<grid, TH, sm, st>>>(a)));
     }
     (void)TILE;
+    return cudaGetLastError();
+}
+
+// L5 two-level (N >= 2^kTwoLevelScatterLog).  pv/pd: [B][N] scratch for the binned pairs; cursor: [B][256] u32,
+// zero on entry (the place pass leaves it zero again).
+template <typename T>
+inline cudaError_t rank_scatter_two_level(const uint32_t* idx_new, const uint32_t* idx_old, const T* sorted, T* x,
+                                          long long B, long long N, T* pv, uint32_t* pd, uint32_t* cursor,
+                                          unsigned long long* changed, cudaStream_t st) {
+    constexpr int TH = SortCfg<T>::SW_THREADS, K = SortCfg<T>::SW_KPT, TILE = SortCfg<T>::SW_TILE;
+    const int shift = ilog2_u64((uint64_t)N) - kRadixBits;
+    AGN_LAUNCH(K_SCATTER_BIN, st, (scatter_bin_kernel<T, TH, K><<<bgrid((unsigned)(N / TILE), B), TH, scatter_bin_smem<T, TH, K>(), st>>>(
+        idx_new, idx_old, sorted, pv, pd, N, shift, cursor, changed, B)));
+    AGN_LAUNCH(K_SCATTER_PLACE, st, (scatter_place_kernel<T><<<bgrid((unsigned)(N / 1024), B), 256, 0, st>>>(pv, pd, x, N, cursor, B)));
     return cudaGetLastError();
 }
 
