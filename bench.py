@@ -208,7 +208,8 @@ def main():
     ag.lib()
 
     B, N, iters = cfg["B"], cfg["N"], cfg["max_iter"]
-    curve0 = rank * B          # Philox curve numbers of this rank's rows: results do not depend on the partition
+    from paper_1909_06374_b200 import multirank
+    curve0 = multirank.weak_curve0(B, rank)   # Philox curve numbers of this rank's rows: results do not depend on the partition
     units_per_step = B * N * iters
 
     def barrier():
@@ -241,10 +242,7 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     iters_used = out["iters_used"].cpu().tolist()
     del out
-    tmax = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms = float(tmax.item())
+    ms = multirank.max_over_ranks(ms, dev, dist)
     value = world * units_per_step * args.steps / (ms * 1e-3)
 
     # ---- per-kernel accounting (CUDA events around every launch of the timed steps) --------------------
@@ -295,12 +293,10 @@ def main():
             step(host_out=host)     # synchronises: the result is on the host when it returns
         barrier()
         dt = time.perf_counter() - t0
-        tm = torch.tensor([dt], dtype=torch.float64, device=dev)
-        if dist is not None:
-            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+        dt = multirank.max_over_ranks(dt, dev, dist)
         h2d = 32 * len(cfg["psd"]) + 64 * len(cfg["erdf"]) + (8 * (cfg["nbins"] + 1) if cfg.get("nbins") else 0)
         d2h = host.numel() * host.element_size() + 4 * B
-        e2e = {"value": world * units_per_step * args.steps / float(tm.item()), "unit": UNIT,
+        e2e = {"value": world * units_per_step * args.steps / dt, "unit": UNIT,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
         del host
 
