@@ -7,6 +7,7 @@
 #include "fft.cuh"
 #include "sort.cuh"
 #include "kernels.cuh"
+#include "fft2.cuh"
 
 #include <cmath>
 #include <cstring>
@@ -46,6 +47,10 @@ template <typename T> cudaError_t ensure_attrs() {
     if (e != cudaSuccess) return e;
     e = sort_set_attrs<T>();
     if (e != cudaSuccess) return e;
+    if (sizeof(T) == 4) {
+        e = fft2_set_attrs<float>();
+        if (e != cudaSuccess) return e;
+    }
     g_attrs_done[slot] = true;
     return cudaSuccess;
 }
@@ -56,7 +61,8 @@ inline unsigned cdiv(long long a, long long b) { return (unsigned)((a + b - 1) /
 template <typename T> size_t ws_e13(int64_t B, int64_t N) {
     typedef typename Cx<T>::type C;
     Carver c(nullptr);
-    c.take<C>(FftPlan<T>::table_elems());
+    c.take<C>(std::max(FftPlan<T>::table_elems(), Fft2Plan<T>::table_elems()));
+    c.take<unsigned int>(Fft2Plan<T>::counter_words(B));
     c.take<T>((size_t)B * N);                 // Z / x_adj
     c.take<T>((size_t)B * (N / 2 + 1));       // A_norm in position order
     c.take<uint32_t>((size_t)B * N);          // permutation ping-pong
@@ -118,7 +124,8 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
     const int logL = ilog2_u64((uint64_t)N) - 1;
     const long long L = N / 2;
     Carver c(d_ws);
-    C* tables = c.take<C>(FftPlan<T>::table_elems());
+    C* tables = c.take<C>(std::max(FftPlan<T>::table_elems(), Fft2Plan<T>::table_elems()));
+    unsigned int* counters = c.take<unsigned int>(Fft2Plan<T>::counter_words(B));
     T* Z = c.take<T>((size_t)B * N);
     T* Ap = c.take<T>((size_t)B * (N / 2 + 1));
     uint32_t* P1 = c.take<uint32_t>((size_t)B * N);
@@ -133,8 +140,20 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
     T* x = (T*)d_x;
     const T* sorted = (const T*)d_sorted;
 
-    FftPlan<T> plan = fft_plan_init<T>(logL, tables, st);
-    TwLevel<T> rlv = real_level<T>(plan);
+    // long fp32 curves: column sub-passes in registers + fused mid kernel (fft2.cuh); otherwise the generic passes
+    const bool use2 = fft2_applicable(sizeof(T), logL);
+    FftPlan<T> plan;
+    Fft2Plan<T> plan2;
+    TwLevel<T> rlv;
+    if (use2) {
+        if constexpr (sizeof(T) == 4) {
+            plan2 = fft2_plan_init<T>(logL, tables, counters, st);
+            plan.dg = plan2.dfull;
+        }
+    } else {
+        plan = fft_plan_init<T>(logL, tables, st);
+        rlv = real_level<T>(plan);
+    }
     cudaMemsetAsync(changed, 0, (size_t)B * sizeof(unsigned long long), st);
     cudaMemsetAsync(first_zero, 0, (size_t)B * sizeof(int), st);
     cudaMemsetAsync(cursor, 0, (size_t)B * kRadix * sizeof(uint32_t), st);
@@ -145,12 +164,22 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
     uint32_t* cur = d_perm;
     uint32_t* nxt = P1;
     for (int k = 1; k <= max_iter; ++k) {
-        // L1 forward FFT (x_sim -> Z, position order)
-        fft_forward<T>(plan, (const C*)x, (C*)Z, L, L, (int)B, st);
-        // L2 amplitude replace
-        AGN_LAUNCH(K_REPLACE, st, (replace_kernel<T><<<bgrid(cdiv(L, 256), B), 256, 0, st>>>((C*)Z, Ap, plan.dg, rlv, (int)B)));
-        // L3 inverse FFT (Z -> x_adj, natural order, 1/L)
-        fft_inverse<T>(plan, (const C*)Z, (C*)Z, L, L, (int)B, (T)(1.0 / (double)L), st);
+        if constexpr (sizeof(T) == 4) if (use2) {
+            // L1 column sub-passes (x_sim -> Z), then rows: forward FFT + L2 amplitude replace + inverse FFT
+            // in one kernel, then L3 inverse column sub-passes (Z -> x_adj, natural order, 1/L)
+            if (fft2_columns<T>(plan2, false, (const C*)x, (C*)Z, (int)B, (T)1, st) != cudaSuccess) return AGNVAR_ECUDA;
+            if (fft2_mid<T>(plan2, (C*)Z, Ap, (int)B, st) != cudaSuccess) return AGNVAR_ECUDA;
+            if (fft2_columns<T>(plan2, true, (const C*)Z, (C*)Z, (int)B, (T)(1.0 / (double)L), st) != cudaSuccess)
+                return AGNVAR_ECUDA;
+        }
+        if (!use2) {
+            // L1 forward FFT (x_sim -> Z, position order)
+            fft_forward<T>(plan, (const C*)x, (C*)Z, L, L, (int)B, st);
+            // L2 amplitude replace
+            AGN_LAUNCH(K_REPLACE, st, (replace_kernel<T><<<bgrid(cdiv(L, 256), B), 256, 0, st>>>((C*)Z, Ap, plan.dg, rlv, (int)B)));
+            // L3 inverse FFT (Z -> x_adj, natural order, 1/L)
+            fft_inverse<T>(plan, (const C*)Z, (C*)Z, L, L, (int)B, (T)(1.0 / (double)L), st);
+        }
         // L4 segmented stable argsort
         cudaError_t e = seg_argsort<T>(Z, nxt, nullptr, B, N, sort_ws, st);
         if (e != cudaSuccess) return AGNVAR_ECUDA;

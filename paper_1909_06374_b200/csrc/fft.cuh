@@ -21,9 +21,10 @@ constexpr int kLogLo = 13;        // per-level low table: exp(-2 pi i l / D), l 
 constexpr int kMaxPass = 3;
 constexpr int kFftThreads = 512;
 
-struct Digits {           // pass radices (log2), forward order
+constexpr int kMaxDigits = 6;
+struct Digits {           // pass / stage radices (log2), forward order
     int n;
-    int lg[kMaxPass];
+    int lg[kMaxDigits];
     int logL;
 };
 
