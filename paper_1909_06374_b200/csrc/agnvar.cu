@@ -8,6 +8,7 @@
 #include "sort.cuh"
 #include "kernels.cuh"
 #include "fft2.cuh"
+#include "sort32.cuh"
 
 #include <cmath>
 #include <cstring>
@@ -50,6 +51,8 @@ template <typename T> cudaError_t ensure_attrs() {
     if (sizeof(T) == 4) {
         e = fft2_set_attrs<float>();
         if (e != cudaSuccess) return e;
+        e = sort32_set_attrs();
+        if (e != cudaSuccess) return e;
     }
     g_attrs_done[slot] = true;
     return cudaSuccess;
@@ -58,6 +61,11 @@ template <typename T> cudaError_t ensure_attrs() {
 inline unsigned cdiv(long long a, long long b) { return (unsigned)((a + b - 1) / b); }
 
 // ---- workspace sizes -----------------------------------------------------------------------------
+template <typename T> size_t sort_ws_any(int64_t B, int64_t N) {
+    size_t s = sort_ws_bytes<T>(B, N);
+    if (sort32_applicable(sizeof(T), N)) s = std::max(s, sort32_ws_bytes(B, N));
+    return s;
+}
 template <typename T> size_t ws_e13(int64_t B, int64_t N) {
     typedef typename Cx<T>::type C;
     Carver c(nullptr);
@@ -69,7 +77,7 @@ template <typename T> size_t ws_e13(int64_t B, int64_t N) {
     c.take<unsigned long long>((size_t)B);    // changed counters
     c.take<int>((size_t)B);                   // first_zero
     c.take<uint32_t>((size_t)B * kRadix);     // bin cursors of the two-level scatter
-    return c.off + sort_ws_bytes<T>(B, N);
+    return c.off + sort_ws_any<T>(B, N);
 }
 template <typename T> size_t ws_tk(int64_t B, int64_t N, int os) {
     typedef typename Cx<T>::type C;
@@ -90,7 +98,7 @@ template <typename T> size_t ws_erdf(int64_t B, int64_t N, int64_t G) {
     c.take<ErdfDev>((size_t)B);
     c.take<double>((size_t)B * G);
     c.take<T>((size_t)B * N);                 // the draw in draw order
-    return c.off + sort_ws_bytes<T>(B, N);
+    return c.off + sort_ws_any<T>(B, N);
 }
 template <typename T> size_t ws_pgram(int64_t B, int64_t N, int64_t nbins) {
     typedef typename Cx<T>::type C;
@@ -180,15 +188,30 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
             // L3 inverse FFT (Z -> x_adj, natural order, 1/L)
             fft_inverse<T>(plan, (const C*)Z, (C*)Z, L, L, (int)B, (T)(1.0 / (double)L), st);
         }
-        // L4 segmented stable argsort
+        // L4 segmented stable argsort, L5 rank scatter + change count
+        bool done45 = false;
+        if constexpr (sizeof(T) == 4) {
+            if (sort32_applicable(sizeof(T), N)) {
+                uint2* spare = nullptr;
+                if (seg_argsort32(Z, nxt, nullptr, B, N, sort_ws, &spare, st) != cudaSuccess) return AGNVAR_ECUDA;
+                if (two_level) {
+                    if (rank_scatter_two_level32(nxt, cur, sorted, x, B, N, spare, cursor, changed, st) != cudaSuccess)
+                        return AGNVAR_ECUDA;
+                } else {
+                    AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(nxt, cur, sorted, x, N, changed, (int)B)));
+                }
+                done45 = true;
+            }
+        }
+        if (!done45) {
         cudaError_t e = seg_argsort<T>(Z, nxt, nullptr, B, N, sort_ws, st);
         if (e != cudaSuccess) return AGNVAR_ECUDA;
-        // L5 rank scatter + change count
         if (two_level) {
             if (rank_scatter_two_level<T>(nxt, cur, sorted, x, B, N, pv, pd, cursor, changed, st) != cudaSuccess)
                 return AGNVAR_ECUDA;
         } else {
             AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(nxt, cur, sorted, x, N, changed, (int)B)));
+        }
         }
         // L6 bookkeeping
         AGN_LAUNCH(K_ITER_POST, st, (post_iter_kernel<<<cdiv(B, 256), 256, 0, st>>>(changed, first_zero, k, (long long*)d_changed_hist, max_iter, (int)B)));
@@ -296,6 +319,12 @@ int erdf_impl(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t B, int64_t N, u
     // does not want it -> use the tail of the sort workspace? no: sort straight into d_perm0 or a scratch
     uint32_t* perm = d_perm0;
     if (!perm) return AGNVAR_EINVAL;   // guarded by the caller (scratch provided there)
+    if constexpr (sizeof(T) == 4) {
+        if (sort32_applicable(sizeof(T), N)) {
+            if (seg_argsort32(draw, perm, (T*)d_sorted, B, N, sort_ws, nullptr, st) != cudaSuccess) return AGNVAR_ECUDA;
+            return cuda_status(cudaGetLastError());
+        }
+    }
     cudaError_t e = seg_argsort<T>(draw, perm, (T*)d_sorted, B, N, sort_ws, st);
     if (e != cudaSuccess) return AGNVAR_ECUDA;
     return cuda_status(cudaGetLastError());

@@ -354,6 +354,7 @@ template <typename T> inline size_t fft_smem_bytes(bool contiguous) {
 }
 
 template <typename T> inline cudaError_t fft_set_attrs() {
+    cudaFuncSetAttribute(fft_pass_kernel<T, kFftThreads, FftCfg<T>::EPT>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     return cudaFuncSetAttribute(fft_pass_kernel<T, kFftThreads, FftCfg<T>::EPT>,
                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes<T>(true));
 }

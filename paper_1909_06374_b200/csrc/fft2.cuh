@@ -433,6 +433,7 @@ inline Fft2Plan<T> fft2_plan_init(int logL, typename Cx<T>::type* tables, unsign
 }
 
 template <typename T> inline cudaError_t fft2_set_attrs() {
+    cudaFuncSetAttribute(fft_mid_kernel<T>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     return cudaFuncSetAttribute(fft_mid_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMidSmemBytes);
 }
 
