@@ -17,47 +17,60 @@ constexpr int kS32Threads = 256;
 constexpr int kS32Kpt = 16;
 constexpr int kS32Tile = kS32Threads * kS32Kpt;      // 4096
 constexpr int kS32Warps = kS32Threads / 32;
+constexpr int kS32Chunk = 4;                         // tiles per look-back unit of the sweep kernel
 
 struct S32Smem {
     uint2 stage[kS32Tile];
-    uint2 cm[kS32Warps * kRadix];       // {lane mask of the current round, running count} per (warp, digit)
+    uint32_t cm[2 * kS32Warps * kRadix]; // per (half-warp, digit): running count << 16 | lane mask of the current round;
+                                         // after the scan: start of the (half-warp, digit) run inside the tile
     uint32_t tile_off[kRadix];
     uint32_t goff[kRadix];
     uint32_t wsum[kS32Warps];
+    uint32_t hist[kRadix];              // sweep: digit counts of the whole chunk
+    uint32_t gbase[kRadix];             // sweep: running global start of every digit inside the chunk
     uint32_t tile;
     uint32_t diff;
 };
 
-// ranks the 16 warp-striped keys of every thread by `digit`; returns local positions and leaves
-// sm.tile_off[d] (exclusive digit offsets in the tile); returns this thread's digit count (thread == digit)
+// Element arrangement inside a tile: half-warp v = 2*warp + (lane >> 4) owns the 256 consecutive elements
+// v*256 .. v*256+255; item j of sub-lane sl = lane & 15 is element v*256 + j*16 + sl (a half-warp reads 16
+// consecutive elements per item: full 128-byte lines for pairs).  Ranking is per half-warp so that the mask of a
+// round and the running count share ONE 32-bit shared-memory word (a random 32-bit access costs ~3.4 wavefronts,
+// a random 64-bit one ~6): per key one ATOMS.OR, one LDS and one predicated STS.
+// Returns local positions; leaves sm.tile_off[d]; returns this thread's digit count (thread == digit).
+__device__ __forceinline__ uint32_t s32_elem0() {
+    const int v = threadIdx.x >> 4, sl = threadIdx.x & 15;
+    return (uint32_t)(v * 256 + sl);
+}
+constexpr int kS32ItemStride = 16;
+
 __device__ __forceinline__ uint32_t s32_rank(const uint32_t (&dig)[kS32Kpt], uint32_t (&pos)[kS32Kpt], S32Smem& sm) {
+    constexpr int V = 2 * kS32Warps;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int v = threadIdx.x >> 4, sl = threadIdx.x & 15;
 #pragma unroll
-    for (int i = 0; i < kS32Warps; ++i) sm.cm[i * kRadix + threadIdx.x] = make_uint2(0u, 0u);
+    for (int i = 0; i < V; ++i) sm.cm[i * kRadix + threadIdx.x] = 0u;
     __syncthreads();
-    const uint32_t lt = lanemask_lt(), bit = 1u << lane;
-    uint2* cw = sm.cm + warp * kRadix;
+    const uint32_t lt = (1u << sl) - 1u, bit = 1u << sl;
+    uint32_t* cw = sm.cm + v * kRadix;
     uint32_t r[kS32Kpt];
 #pragma unroll
     for (int j = 0; j < kS32Kpt; ++j) {
         const uint32_t d = dig[j];
-        atomicOr(&cw[d].x, bit);
+        atomicOr(&cw[d], bit);
         __syncwarp();
-        const uint2 mc = cw[d];
-        r[j] = mc.y + __popc(mc.x & lt);
+        const uint32_t mc = cw[d];
+        const uint32_t mask = mc & 0xffffu;
+        r[j] = (mc >> 16) + __popc(mask & lt);
         __syncwarp();
-        if ((mc.x & lt) == 0u) cw[d] = make_uint2(0u, mc.y + __popc(mc.x));
+        if ((mask & lt) == 0u) cw[d] = (mc & 0xffff0000u) + ((uint32_t)__popc(mask) << 16);
         __syncwarp();
     }
     __syncthreads();
-    // thread == digit: exclusive scan over the warps, then over the digits
+    // thread == digit: totals over the half-warps, exclusive scan over the digits, then the run starts
     uint32_t run = 0;
 #pragma unroll
-    for (int w = 0; w < kS32Warps; ++w) {
-        const uint32_t t = sm.cm[w * kRadix + threadIdx.x].y;
-        sm.cm[w * kRadix + threadIdx.x].y = run;
-        run += t;
-    }
+    for (int i = 0; i < V; ++i) run += sm.cm[i * kRadix + threadIdx.x] >> 16;
     uint32_t inc = run;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -69,10 +82,18 @@ __device__ __forceinline__ uint32_t s32_rank(const uint32_t (&dig)[kS32Kpt], uin
     uint32_t add = 0;
 #pragma unroll
     for (int w = 0; w < kS32Warps; ++w) add += (w < warp) ? sm.wsum[w] : 0u;
-    sm.tile_off[threadIdx.x] = inc - run + add;
+    const uint32_t toff = inc - run + add;
+    sm.tile_off[threadIdx.x] = toff;
+    uint32_t acc = toff;
+#pragma unroll
+    for (int i = 0; i < V; ++i) {
+        const uint32_t c = sm.cm[i * kRadix + threadIdx.x] >> 16;
+        sm.cm[i * kRadix + threadIdx.x] = acc;
+        acc += c;
+    }
     __syncthreads();
 #pragma unroll
-    for (int j = 0; j < kS32Kpt; ++j) pos[j] = sm.tile_off[dig[j]] + cw[dig[j]].y + r[j];
+    for (int j = 0; j < kS32Kpt; ++j) pos[j] = cw[dig[j]] + r[j];
     return run;
 }
 
@@ -86,9 +107,9 @@ struct Sweep32Args {
     int shift;
     const uint32_t* dstart;     // [B][NP][256] exclusive digit starts (scanned histogram)
     int pass, npass;
-    uint32_t* status;           // [B][ntiles][256] zero-initialised
+    uint32_t* status;           // [B][nchunks][256] zero-initialised
     uint32_t* ticket;           // [B] zero-initialised
-    uint32_t ntiles;
+    uint32_t ntiles, nchunks;
     long long B;
 };
 
@@ -112,6 +133,24 @@ __global__ void __launch_bounds__(kRadix) digit_scan_kernel(uint32_t* __restrict
 }
 
 // KIND 0: first pass (raw values in, pairs out); 1: middle (pairs in, pairs out); 2: last (pairs in, indices out)
+// One CTA handles a CHUNK of kS32Chunk consecutive tiles.  Phase A counts the chunk's digits (one streaming read),
+// publishes the chunk aggregate and looks back over earlier chunks; phase B re-reads the tiles (they are still in
+// L2), ranks each one and writes it out with a running per-digit offset.  The decoupled look-back window is
+// (chunks started per microsecond) x (look-back latency): per-tile look-back at ~90 tiles/us made every tile sum
+// ~50 predecessor aggregates; per-chunk it is a handful.
+template <int KIND>
+__device__ __forceinline__ void s32_load_tile(const Sweep32Args& a, size_t seg, uint32_t e0, uint2 (&kv)[kS32Kpt]) {
+    if (KIND == 0) {
+        const float* v = a.vals + seg + e0;
+#pragma unroll
+        for (int j = 0; j < kS32Kpt; ++j) kv[j] = make_uint2(key_of(v[j * kS32ItemStride]), e0 + j * kS32ItemStride);
+    } else {
+        const uint2* v = a.in + seg + e0;
+#pragma unroll
+        for (int j = 0; j < kS32Kpt; ++j) kv[j] = v[j * kS32ItemStride];
+    }
+}
+
 template <int KIND>
 __global__ void __launch_bounds__(kS32Threads, 4) sweep32_kernel(Sweep32Args a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -119,36 +158,32 @@ __global__ void __launch_bounds__(kS32Threads, 4) sweep32_kernel(Sweep32Args a) 
     const long long b = bidx();
     if (b >= a.B) return;
     if (threadIdx.x == 0) sm.tile = atomicAdd(&a.ticket[b], 1u);
+    sm.hist[threadIdx.x] = 0u;
     __syncthreads();
-    const uint32_t tile = sm.tile;
-    const uint32_t base = tile * kS32Tile;
+    const uint32_t chunk = sm.tile;
+    const uint32_t tiles_here = min((uint32_t)kS32Chunk, a.ntiles - chunk * kS32Chunk);
     const size_t seg = (size_t)b * a.N;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t e00 = chunk * (kS32Chunk * kS32Tile) + s32_elem0();
     uint2 kv[kS32Kpt];
     uint32_t dig[kS32Kpt], pos[kS32Kpt];
-    const uint32_t e0 = base + warp * (32 * kS32Kpt) + lane;
-    if (KIND == 0) {
-        const float* v = a.vals + seg + e0;
+    // ---- phase A: digit counts of the chunk
+    for (uint32_t c = 0; c < tiles_here; ++c) {
+        s32_load_tile<KIND>(a, seg, e00 + c * kS32Tile, kv);
 #pragma unroll
-        for (int j = 0; j < kS32Kpt; ++j) kv[j] = make_uint2(key_of(__ldcs(v + j * 32)), e0 + j * 32);
-    } else {
-        const uint2* v = a.in + seg + e0;
-#pragma unroll
-        for (int j = 0; j < kS32Kpt; ++j) kv[j] = __ldcs(v + j * 32);
+        for (int j = 0; j < kS32Kpt; ++j) atomicAdd(&sm.hist[(kv[j].x >> a.shift) & (kRadix - 1)], 1u);
     }
-#pragma unroll
-    for (int j = 0; j < kS32Kpt; ++j) dig[j] = (kv[j].x >> a.shift) & (kRadix - 1);
-    const uint32_t agg = s32_rank(dig, pos, sm);
-    // thread == digit: publish the tile aggregate, look back over earlier tiles of the segment
+    __syncthreads();
+    // ---- thread == digit: publish the chunk aggregate, look back over earlier chunks of the segment
     {
         const int d = threadIdx.x;
-        volatile uint32_t* st = a.status + (size_t)b * a.ntiles * kRadix + d;
+        const uint32_t agg = sm.hist[d];
+        volatile uint32_t* st = a.status + (size_t)b * a.nchunks * kRadix + d;
         uint32_t excl = 0;
-        if (tile == 0) {
+        if (chunk == 0) {
             st[0] = kFlagInc | agg;
         } else {
-            st[(size_t)tile * kRadix] = kFlagAgg | agg;
-            int t = (int)tile - 1;
+            st[(size_t)chunk * kRadix] = kFlagAgg | agg;
+            int t = (int)chunk - 1;
             bool done = false;
             while (!done) {
                 uint32_t sv[kLookBatch];
@@ -168,23 +203,36 @@ __global__ void __launch_bounds__(kS32Threads, 4) sweep32_kernel(Sweep32Args a) 
                 }
                 t -= used;
             }
-            st[(size_t)tile * kRadix] = kFlagInc | (excl + agg);
+            st[(size_t)chunk * kRadix] = kFlagInc | (excl + agg);
         }
-        sm.goff[d] = a.dstart[((size_t)b * a.npass + a.pass) * kRadix + d] + excl - sm.tile_off[d];
+        sm.gbase[d] = a.dstart[((size_t)b * a.npass + a.pass) * kRadix + d] + excl;
     }
+    // ---- phase B: rank and write every tile of the chunk (re-read through L2)
+    for (uint32_t c = 0; c < tiles_here; ++c) {
+        s32_load_tile<KIND>(a, seg, e00 + c * kS32Tile, kv);
 #pragma unroll
-    for (int j = 0; j < kS32Kpt; ++j) sm.stage[pos[j]] = kv[j];
-    __syncthreads();
-#pragma unroll 4
-    for (int s = threadIdx.x; s < kS32Tile; s += kS32Threads) {
-        const uint2 p = sm.stage[s];
-        const uint32_t g = sm.goff[(p.x >> a.shift) & (kRadix - 1)] + (uint32_t)s;
-        if (KIND == 2) {
-            a.idx_out[seg + g] = p.y;
-            if (a.sorted_out) a.sorted_out[seg + g] = val_of(p.x);
-        } else {
-            a.out[seg + g] = p;
+        for (int j = 0; j < kS32Kpt; ++j) dig[j] = (kv[j].x >> a.shift) & (kRadix - 1);
+        const uint32_t cnt = s32_rank(dig, pos, sm);          // has barriers: the previous tile's stage reads are done
+        {
+            const uint32_t g = sm.gbase[threadIdx.x];
+            sm.goff[threadIdx.x] = g - sm.tile_off[threadIdx.x];
+            sm.gbase[threadIdx.x] = g + cnt;
         }
+#pragma unroll
+        for (int j = 0; j < kS32Kpt; ++j) sm.stage[pos[j]] = kv[j];
+        __syncthreads();
+#pragma unroll 4
+        for (int s = threadIdx.x; s < kS32Tile; s += kS32Threads) {
+            const uint2 p = sm.stage[s];
+            const uint32_t g = sm.goff[(p.x >> a.shift) & (kRadix - 1)] + (uint32_t)s;
+            if (KIND == 2) {
+                a.idx_out[seg + g] = p.y;
+                if (a.sorted_out) a.sorted_out[seg + g] = val_of(p.x);
+            } else {
+                a.out[seg + g] = p;
+            }
+        }
+        __syncthreads();      // stage and goff are rewritten by the next tile
     }
 }
 
@@ -207,14 +255,14 @@ __global__ void __launch_bounds__(kS32Threads, 4) scatter_bin32_kernel(const uin
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint2 kv[kS32Kpt];                  // x = value bits, y = dst
     uint32_t dig[kS32Kpt], pos[kS32Kpt];
-    const size_t e0 = seg + base + warp * (32 * kS32Kpt) + lane;
+    const size_t e0 = seg + base + s32_elem0();
     unsigned int diff = 0;
     if (threadIdx.x == 0) sm.diff = 0u;
 #pragma unroll
     for (int j = 0; j < kS32Kpt; ++j) {
-        const uint32_t dst = __ldcs(idx_new + e0 + j * 32);
-        diff += (dst != __ldcs(idx_old + e0 + j * 32));
-        kv[j] = make_uint2(__float_as_uint(__ldcs(sorted + e0 + j * 32)), dst);
+        const uint32_t dst = __ldcs(idx_new + e0 + j * kS32ItemStride);
+        diff += (dst != __ldcs(idx_old + e0 + j * kS32ItemStride));
+        kv[j] = make_uint2(__float_as_uint(__ldcs(sorted + e0 + j * kS32ItemStride)), dst);
         dig[j] = (dst >> shift) & (kRadix - 1);
     }
     const uint32_t cnt = s32_rank(dig, pos, sm);
@@ -298,7 +346,8 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
     const int chunk = 1 << 16;
     AGN_LAUNCH(K_SORT_HIST, st, (digit_hist_kernel<float, 512><<<bgrid((unsigned)((N + chunk - 1) / chunk), B), 512, 0, st>>>(vals, hist, N, N, chunk, B)));
     AGN_LAUNCH(K_SORT_HIST, st, (digit_scan_kernel<<<(unsigned)(B * NP), kRadix, 0, st>>>(hist)));
-    const dim3 grid = bgrid((unsigned)ntiles, B);
+    const size_t nchunks = (ntiles + kS32Chunk - 1) / kS32Chunk;
+    const dim3 grid = bgrid((unsigned)nchunks, B);
     for (int p = 0; p < NP; ++p) {
         Sweep32Args a;
         a.vals = vals;
@@ -309,7 +358,7 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
         a.dstart = hist; a.pass = p; a.npass = NP;
         a.status = status + (size_t)p * B * ntiles * kRadix;
         a.ticket = ticket + (size_t)p * B;
-        a.ntiles = (uint32_t)ntiles; a.B = B;
+        a.ntiles = (uint32_t)ntiles; a.nchunks = (uint32_t)nchunks; a.B = B;
         if (p == 0) AGN_LAUNCH(K_SORT_SWEEP, st, (sweep32_kernel<0><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
         else if (p == NP - 1) AGN_LAUNCH(K_SORT_SWEEP, st, (sweep32_kernel<2><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
         else AGN_LAUNCH(K_SORT_SWEEP, st, (sweep32_kernel<1><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
