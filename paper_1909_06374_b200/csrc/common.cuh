@@ -125,13 +125,14 @@ static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; 
 enum KernelId {
     K_FFT_STRIDED = 0, K_FFT_CONTIG, K_REPLACE, K_SORT_CTA, K_SORT_HIST, K_SORT_SWEEP, K_SCATTER, K_ITER_POST,
     K_PERM_ANORM, K_TK_FILL, K_TK_COMBINE, K_UNTANGLE_OUT, K_PSD, K_ERDF_TABLE, K_ERDF_SAMPLE, K_PGRAM, K_TABLES,
-    K_COPY, K_PHILOX, K_SCATTER_BIN, K_SCATTER_PLACE, K_FFT_COL, K_FFT_MID, K_NIDS
+    K_COPY, K_PHILOX, K_SCATTER_BIN, K_SCATTER_PLACE, K_FFT_COL, K_FFT_MID, K_SORT_CDF, K_SORT_PART, K_SORT_BUCKET, K_NIDS
 };
 static const char* const kKernelNames[K_NIDS] = {
     "fft_pass_strided", "fft_pass_contiguous", "amplitude_replace", "cta_argsort", "sort_digit_hist",
     "sort_onesweep", "rank_scatter_count", "iter_bookkeeping", "perm_anorm", "tk_fill", "tk_combine5_crop",
     "untangle_out", "psd", "erdf_table", "erdf_sample", "periodogram_scale_bin", "twiddle_tables", "copy", "philox",
-    "scatter_bin", "scatter_place", "fft_columns", "fft_mid_fused"};
+    "scatter_bin", "scatter_place", "fft_columns", "fft_mid_fused", "sort_cdf_tables", "sort_msd_partition",
+    "sort_bucket_finish"};
 
 struct TraceRec { int id; cudaEvent_t e0, e1; };
 struct TraceState {

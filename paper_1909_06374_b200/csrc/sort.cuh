@@ -143,10 +143,12 @@ __global__ void __launch_bounds__(THREADS) cta_argsort_kernel(const T* __restric
 // ------------------------------------------------------------------------------------------------
 template <typename T, int THREADS>
 __global__ void __launch_bounds__(THREADS) digit_hist_kernel(const T* __restrict__ vals, uint32_t* __restrict__ hist,
-                                                             long long N, long long seg_stride, int chunk, long long B) {
+                                                             long long N, long long seg_stride, int chunk, long long B,
+                                                             const uint32_t* __restrict__ gate) {
     typedef typename KeyT<T>::type KeyU;
     constexpr int NP = KeyT<T>::bits / kRadixBits;
     __shared__ uint32_t h[NP * kRadix];
+    if (gate && bidx() < B && gate[bidx()] == 0u) return;      // curve already sorted by the bucket path
     for (int i = threadIdx.x; i < NP * kRadix; i += THREADS) h[i] = 0;
     __syncthreads();
     const long long b = bidx();
@@ -463,7 +465,7 @@ inline cudaError_t seg_argsort(const T* vals, uint32_t* idx_out, T* sorted_out, 
     if (e != cudaSuccess) return e;
     const int chunk = 1 << 16;
     dim3 hg = bgrid((unsigned)((N + chunk - 1) / chunk), B);
-    AGN_LAUNCH(K_SORT_HIST, st, (digit_hist_kernel<T, 512><<<hg, 512, 0, st>>>(vals, hist, N, N, chunk, B)));
+    AGN_LAUNCH(K_SORT_HIST, st, (digit_hist_kernel<T, 512><<<hg, 512, 0, st>>>(vals, hist, N, N, chunk, B, nullptr)));
     const size_t sm = cta_sort_smem<T, TH, K>();
     dim3 grid = bgrid((unsigned)ntiles, B);
     for (int p = 0; p < NP; ++p) {

@@ -10,6 +10,7 @@
 #pragma once
 #include "common.cuh"
 #include "sort.cuh"
+#include "bucket32.cuh"
 
 namespace agn {
 
@@ -111,11 +112,14 @@ struct Sweep32Args {
     uint32_t* ticket;           // [B] zero-initialised
     uint32_t ntiles, nchunks;
     long long B;
+    const uint32_t* gate;       // NULL, or [B]: the curve is sorted here only if its word is non-zero
 };
 
 // exclusive scan of every 256-bin histogram, in place (one warp-scan CTA per histogram)
-__global__ void __launch_bounds__(kRadix) digit_scan_kernel(uint32_t* __restrict__ hist) {
+__global__ void __launch_bounds__(kRadix) digit_scan_kernel(uint32_t* __restrict__ hist, const uint32_t* __restrict__ gate,
+                                                            int per_curve) {
     __shared__ uint32_t ws[8];
+    if (gate && gate[blockIdx.x / per_curve] == 0u) return;
     uint32_t* h = hist + (size_t)blockIdx.x * kRadix;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t c = h[threadIdx.x];
@@ -157,6 +161,7 @@ __global__ void __launch_bounds__(kS32Threads, 4) sweep32_kernel(Sweep32Args a) 
     S32Smem& sm = *reinterpret_cast<S32Smem*>(smem_raw);
     const long long b = bidx();
     if (b >= a.B) return;
+    if (a.gate && a.gate[b] == 0u) return;
     if (threadIdx.x == 0) sm.tile = atomicAdd(&a.ticket[b], 1u);
     sm.hist[threadIdx.x] = 0u;
     __syncthreads();
@@ -314,6 +319,7 @@ inline cudaError_t sort32_set_attrs() {
     cudaFuncSetAttribute(sweep32_kernel<1>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     cudaFuncSetAttribute(sweep32_kernel<2>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     cudaFuncSetAttribute(scatter_bin32_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    if (e == cudaSuccess) e = bucket32_set_attrs();
     return e;
 }
 
@@ -326,6 +332,7 @@ inline size_t sort32_ws_bytes(long long B, long long N) {
     const size_t ntiles = (size_t)(N / kS32Tile);
     size_t s = 2 * align_up((size_t)B * N * sizeof(uint2), 256);
     s += align_up((size_t)B * 4 * kRadix * 4 + (size_t)B * 4 * 4 + (size_t)B * 4 * ntiles * kRadix * 4, 256);
+    if (bucket32_applicable(4, N)) s += bucket32_ctl_bytes(B, N);
     return s;
 }
 
@@ -341,11 +348,18 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
     uint32_t* ticket = hist + (size_t)B * NP * kRadix;
     uint32_t* status = ticket + (size_t)B * NP;
     const size_t ctl = (size_t)B * NP * kRadix * 4 + (size_t)B * NP * 4 + (size_t)B * NP * ntiles * kRadix * 4;
-    cudaError_t e = cudaMemsetAsync(hist, 0, ctl, st);
+    cudaError_t e;
+    // long curves: two-level bucket sort (bucket32.cuh); the LSD passes below then only run for curves it gave up on
+    const uint32_t* gate = nullptr;
+    if (bucket32_applicable(4, N)) {
+        e = bucket32_sort(vals, idx_out, sorted_out, B, N, pa, w + align_up(ctl, 256), &gate, st);
+        if (e != cudaSuccess) return e;
+    }
+    e = cudaMemsetAsync(hist, 0, ctl, st);
     if (e != cudaSuccess) return e;
     const int chunk = 1 << 16;
-    AGN_LAUNCH(K_SORT_HIST, st, (digit_hist_kernel<float, 512><<<bgrid((unsigned)((N + chunk - 1) / chunk), B), 512, 0, st>>>(vals, hist, N, N, chunk, B)));
-    AGN_LAUNCH(K_SORT_HIST, st, (digit_scan_kernel<<<(unsigned)(B * NP), kRadix, 0, st>>>(hist)));
+    AGN_LAUNCH(K_SORT_HIST, st, (digit_hist_kernel<float, 512><<<bgrid((unsigned)((N + chunk - 1) / chunk), B), 512, 0, st>>>(vals, hist, N, N, chunk, B, gate)));
+    AGN_LAUNCH(K_SORT_HIST, st, (digit_scan_kernel<<<(unsigned)(B * NP), kRadix, 0, st>>>(hist, gate, NP)));
     const size_t nchunks = (ntiles + kS32Chunk - 1) / kS32Chunk;
     const dim3 grid = bgrid((unsigned)nchunks, B);
     for (int p = 0; p < NP; ++p) {
@@ -358,7 +372,7 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
         a.dstart = hist; a.pass = p; a.npass = NP;
         a.status = status + (size_t)p * B * ntiles * kRadix;
         a.ticket = ticket + (size_t)p * B;
-        a.ntiles = (uint32_t)ntiles; a.nchunks = (uint32_t)nchunks; a.B = B;
+        a.ntiles = (uint32_t)ntiles; a.nchunks = (uint32_t)nchunks; a.B = B; a.gate = gate;
         if (p == 0) AGN_LAUNCH(K_SORT_SWEEP, st, (sweep32_kernel<0><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
         else if (p == NP - 1) AGN_LAUNCH(K_SORT_SWEEP, st, (sweep32_kernel<2><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
         else AGN_LAUNCH(K_SORT_SWEEP, st, (sweep32_kernel<1><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
