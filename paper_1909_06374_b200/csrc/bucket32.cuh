@@ -29,16 +29,25 @@ constexpr int kBkCap = 8192;                      // slab slots per bucket
 constexpr int kBkSampleLog = 6;                   // one sample per 64 keys
 constexpr int kBkBinLog = 16;                     // CDF bins = top 16 key bits
 constexpr int kBkBins = 1 << kBkBinLog;
-constexpr int kBkShift = kBkBinLog + kBkMeanLog - kBkSampleLog;     // 22
-constexpr int kBkSortThreads = 512;
-constexpr int kBkSlots = 8192;                    // interpolation slots of the in-CTA sort
+constexpr int kBkSortThreads = 1024;
+constexpr int kBkSlotLog = 12;
+constexpr int kBkSlots = 1 << kBkSlotLog;         // interpolation slots of the in-CTA sort
 constexpr int kBkEpt = kBkCap / kBkSortThreads;   // 16 elements per thread
 
-// keys above the largest sampled bin have cum = all samples: clamp them into the last bucket (still monotone)
-__device__ __forceinline__ uint32_t bucket_of(uint32_t key, const uint2* __restrict__ tab, uint32_t nb) {
+// Position of a key on the smoothed CDF: bin weights w = cnt * K + 1 (K = 2^24 / samples, so that the sampled mass is
+// 2^24 and the add-one mass 2^16 whatever N is: keys of an unsampled bin still spread linearly over their own
+// stretch instead of collapsing onto one point), pos = cumw * 2^16 + low16(key) * w < (2^24 + 2^16) * 2^16.
+// The table holds (cumw << 7, w), so that pos >> 9 = tab.x + ((low16 * w) >> 9) fits 32 bits, and
+// bs = bucket << 12 | slot = floor((pos >> 9) * M / 2^32) with M = floor(2^32 * nb * 4096 * 512 / (total * 2^16)):
+// one multiply-high.  Every step is monotone in the key, and equal keys get equal bs.
+constexpr unsigned long long kBkTotalW = (1ull << 24) + (1ull << 16);
+__device__ __forceinline__ uint32_t bs_of(uint32_t key, const uint2* __restrict__ tab, uint32_t M) {
     const uint2 e = __ldg(tab + (key >> (32 - kBkBinLog)));
-    const unsigned long long pos = ((unsigned long long)e.x << kBkBinLog) + (unsigned long long)(key & (kBkBins - 1)) * e.y;
-    return min((uint32_t)(pos >> kBkShift), nb - 1u);
+    const uint32_t pos = e.x + (uint32_t)(((unsigned long long)(key & (kBkBins - 1)) * e.y) >> 9);
+    return __umulhi(pos, M);
+}
+inline uint32_t bucket32_magic(uint32_t nb) {
+    return (uint32_t)((((unsigned __int128)nb) << (32 + 12 + 9)) / (kBkTotalW << 16));
 }
 
 __global__ void __launch_bounds__(256) cdf_sample_kernel(const float* __restrict__ vals, uint32_t* __restrict__ hist,
@@ -53,8 +62,8 @@ __global__ void __launch_bounds__(256) cdf_sample_kernel(const float* __restrict
     atomicAdd(&hist[(size_t)b * kBkBins + (k >> (32 - kBkBinLog))], 1u);
 }
 
-// one CTA (1024 threads) per curve: tab[bin] = (exclusive cum, cnt)
-__global__ void __launch_bounds__(1024) cdf_table_kernel(const uint32_t* __restrict__ hist, uint2* __restrict__ tab) {
+// one CTA (1024 threads) per curve: tab[bin] = (exclusive cumulative weight << 7, weight), weight = (cnt << logK) + 1
+__global__ void __launch_bounds__(1024) cdf_table_kernel(const uint32_t* __restrict__ hist, uint2* __restrict__ tab, int logK) {
     __shared__ uint32_t ws[32];
     const uint32_t* h = hist + (size_t)blockIdx.x * kBkBins;
     uint2* t = tab + (size_t)blockIdx.x * kBkBins;
@@ -62,7 +71,7 @@ __global__ void __launch_bounds__(1024) cdf_table_kernel(const uint32_t* __restr
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint32_t c[PER], sum = 0;
 #pragma unroll
-    for (int i = 0; i < PER; ++i) { c[i] = h[threadIdx.x * PER + i]; sum += c[i]; }
+    for (int i = 0; i < PER; ++i) { c[i] = (h[threadIdx.x * PER + i] << logK) + 1u; sum += c[i]; }
     uint32_t inc = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -83,37 +92,141 @@ __global__ void __launch_bounds__(1024) cdf_table_kernel(const uint32_t* __restr
     __syncthreads();
     uint32_t run = inc - sum + ws[warp];
 #pragma unroll
-    for (int i = 0; i < PER; ++i) { t[threadIdx.x * PER + i] = make_uint2(run, c[i]); run += c[i]; }
+    for (int i = 0; i < PER; ++i) { t[threadIdx.x * PER + i] = make_uint2(run << 7, c[i]); run += c[i]; }
 }
 
+// ------------------------------------------------------------------------------------------------
+// partition: two levels (coarse = high bits of the bucket number, fine = low bits), each a tile kernel that counts
+// its keys per digit in shared memory, reserves one range per digit in the digit's slab (one global atomic per
+// non-empty digit and tile), orders the tile by digit in shared memory and writes the runs out coalesced.
+// The order inside a slab is arbitrary (see the header), so ranking inside the tile is a plain counter per digit.
+// ------------------------------------------------------------------------------------------------
 constexpr int kBkPartThreads = 256;
 constexpr int kBkPartEpt = 16;
+constexpr int kBkPartTile = kBkPartThreads * kBkPartEpt;      // 4096
+constexpr int kBkMaxDigits = 256;
 
-__global__ void __launch_bounds__(kBkPartThreads) bucket_part_kernel(const float* __restrict__ vals,
-                                                                     const uint2* __restrict__ tab,
-                                                                     uint32_t* __restrict__ cursor,
-                                                                     uint2* __restrict__ slabs, uint32_t* __restrict__ overflow,
-                                                                     uint32_t N, uint32_t nb, long long B) {
+struct PartSmem {
+    uint2 stage[kBkPartTile];
+    unsigned char sdig[kBkPartTile];
+    uint32_t cnt[kBkMaxDigits];         // digit populations of the tile
+    uint32_t lstart[kBkMaxDigits];      // first stage position of the digit
+    uint32_t gdst[kBkMaxDigits];        // slab position of stage position 0 of the digit (may wrap: used modulo 2^32)
+    uint32_t wsum[kBkPartThreads / 32];
+};
+
+struct PartArgs {
+    const float* vals;          // LEVEL 0 input [B][N]
+    const uint2* in;            // LEVEL 1 input: coarse slabs [B][nc][cap_in]
+    const uint32_t* in_count;   // LEVEL 1: populations of the coarse slabs [B][nc]
+    uint2* out;                 // slabs [B][n_out][cap_out]
+    uint32_t* cursor;           // [B][n_out] zero on entry
+    uint32_t* overflow;         // [B]
+    const uint2* tab;           // [B][65536]
+    uint32_t N, nb;             // keys per curve, fine buckets per curve
+    uint32_t M;                 // bucket32_magic(nb)
+    uint32_t lb;                // low (fine) bits of the bucket number
+    uint32_t nc;                // coarse slabs per curve
+    uint32_t cap_in, cap_out;
+    uint32_t tiles_in;          // LEVEL 1: tiles per coarse slab
+    long long B;
+};
+
+template <int LEVEL>
+__global__ void __launch_bounds__(kBkPartThreads, 4) bucket_part_kernel(PartArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    PartSmem& sm = *reinterpret_cast<PartSmem*>(smem_raw);
     const long long b = bidx();
-    if (b >= B) return;
-    const float* v = vals + (size_t)b * N;
-    const uint2* t = tab + (size_t)b * kBkBins;
-    uint32_t* cur = cursor + (size_t)b * nb;
-    uint2* sl = slabs + (size_t)b * nb * kBkCap;
-    const uint32_t e0 = blockIdx.x * (kBkPartThreads * kBkPartEpt) + threadIdx.x;
-    uint32_t key[kBkPartEpt], bk[kBkPartEpt];
+    if (b >= a.B) return;
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    const uint2* tab = a.tab + (size_t)b * kBkBins;
+    uint32_t coarse = 0, tile = blockIdx.x, n_in = a.N;
+    if (LEVEL == 1) {
+        coarse = blockIdx.x / a.tiles_in;
+        tile = blockIdx.x - coarse * a.tiles_in;
+        n_in = min(a.in_count[(size_t)b * a.nc + coarse], a.cap_in);
+        if (tile * kBkPartTile >= n_in) return;
+    }
+    sm.cnt[t] = 0u;
+    const uint32_t e0 = tile * kBkPartTile + t;
+    uint2 kv[kBkPartEpt];
+    if (LEVEL == 0) {
+        const float* v = a.vals + (size_t)b * a.N;
 #pragma unroll
-    for (int j = 0; j < kBkPartEpt; ++j) key[j] = key_of(__ldcs(v + e0 + j * kBkPartThreads));
+        for (int j = 0; j < kBkPartEpt; ++j) kv[j] = make_uint2(key_of(__ldcs(v + e0 + j * kBkPartThreads)), e0 + j * kBkPartThreads);
+    } else {
+        const uint2* v = a.in + ((size_t)b * a.nc + coarse) * a.cap_in;
 #pragma unroll
-    for (int j = 0; j < kBkPartEpt; ++j) bk[j] = bucket_of(key[j], t, nb);
-    bool over = false;
+        for (int j = 0; j < kBkPartEpt; ++j)
+            if (e0 + j * kBkPartThreads < n_in) kv[j] = __ldcs(v + e0 + j * kBkPartThreads);
+    }
+    __syncthreads();
+    // digit and arrival number inside the digit: lanes that share lane 0's digit (the common case for a smooth
+    // series) are counted with one atomic, the others with one each
+    uint32_t dr[kBkPartEpt];            // digit << 16 | arrival number
+    const uint32_t dmask = (LEVEL == 0) ? 0xffffffffu : ((1u << a.lb) - 1u);
+    const uint32_t dshift = kBkSlotLog + ((LEVEL == 0) ? a.lb : 0u);
 #pragma unroll
     for (int j = 0; j < kBkPartEpt; ++j) {
-        const uint32_t s = atomicAdd(&cur[bk[j]], 1u);
-        if (s < (uint32_t)kBkCap) sl[(size_t)bk[j] * kBkCap + s] = make_uint2(key[j], e0 + j * kBkPartThreads);
-        else over = true;
+        const bool valid = (LEVEL == 0) || (e0 + j * kBkPartThreads < n_in);
+        const uint32_t d = valid ? ((bs_of(kv[j].x, tab, a.M) >> dshift) & dmask) : 0xffffu;
+        const uint32_t d0 = __shfl_sync(0xffffffffu, d, 0);
+        const uint32_t same = __ballot_sync(0xffffffffu, d == d0);
+        uint32_t r = 0;
+        if (d0 != 0xffffu) {
+            if (lane == 0) r = atomicAdd(&sm.cnt[d0], (uint32_t)__popc(same));
+            r = __shfl_sync(0xffffffffu, r, 0) + __popc(same & ((1u << lane) - 1u));
+        }
+        if (valid && d != d0) r = atomicAdd(&sm.cnt[d], 1u);
+        dr[j] = (d << 16) | r;
     }
-    if (over) overflow[b] = 1u;
+    __syncthreads();
+    // thread == digit: reserve the digit's range in its slab, exclusive scan of the populations
+    {
+        const uint32_t c = sm.cnt[t];
+        const uint32_t slab = (LEVEL == 0) ? (uint32_t)t : ((coarse << a.lb) | (uint32_t)t);
+        const uint32_t n_out = (LEVEL == 0) ? a.nc : a.nb;
+        uint32_t g = 0;
+        if (c) {
+            g = atomicAdd(&a.cursor[(size_t)b * n_out + slab], c);
+            if (g + c > a.cap_out) a.overflow[b] = 1u;
+        }
+        uint32_t inc = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t m = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += m;
+        }
+        if (lane == 31) sm.wsum[warp] = inc;
+        __syncthreads();
+        uint32_t add = 0;
+#pragma unroll
+        for (int w = 0; w < kBkPartThreads / 32; ++w) add += (w < warp) ? sm.wsum[w] : 0u;
+        const uint32_t ls = inc - c + add;
+        sm.lstart[t] = ls;
+        sm.gdst[t] = g - ls;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < kBkPartEpt; ++j) {
+        const bool valid = (LEVEL == 0) || (e0 + j * kBkPartThreads < n_in);
+        if (valid) {
+            const uint32_t d = dr[j] >> 16, s = sm.lstart[d] + (dr[j] & 0xffffu);
+            sm.stage[s] = kv[j];
+            sm.sdig[s] = (unsigned char)d;
+        }
+    }
+    __syncthreads();
+    const uint32_t n_tile = min((uint32_t)kBkPartTile, n_in - tile * kBkPartTile);
+    const uint32_t n_out = (LEVEL == 0) ? a.nc : a.nb;
+    uint2* out = a.out + (size_t)b * n_out * a.cap_out;
+    const uint32_t slab0 = (LEVEL == 0) ? 0u : (coarse << a.lb);
+#pragma unroll 4
+    for (uint32_t s = t; s < n_tile; s += kBkPartThreads) {
+        const uint32_t d = sm.sdig[s];
+        const uint32_t off = sm.gdst[d] + s;
+        if (off < a.cap_out) out[(size_t)(slab0 + d) * a.cap_out + off] = sm.stage[s];
+    }
 }
 
 // one CTA (1024 threads) per curve: base[k] = sum of the populations of buckets < k (populations clamped to the slab)
@@ -147,19 +260,20 @@ __global__ void __launch_bounds__(1024) bucket_base_kernel(const uint32_t* __res
 }
 
 struct BkSmem {
-    unsigned long long pair[kBkCap];      // (key << 32) | index
-    uint32_t cnt[kBkSlots];               // slot populations, then slot starts
+    unsigned long long pair[kBkCap];      // (key << 32) | index, grouped by slot
+    uint32_t cnt[kBkSlots];               // slot populations, then slot starts, then slot ends
+    unsigned short slot[kBkCap];          // slot of slab element e
     uint32_t wsum[kBkSortThreads / 32];
-    uint32_t kmin, kmax;
 };
 
 __global__ void __launch_bounds__(kBkSortThreads, 2) bucket_sort_kernel(const uint2* __restrict__ slabs,
                                                                         const uint32_t* __restrict__ cursor,
                                                                         const uint32_t* __restrict__ base,
                                                                         const uint32_t* __restrict__ overflow,
+                                                                        const uint2* __restrict__ tabs,
                                                                         uint32_t* __restrict__ idx_out,
                                                                         float* __restrict__ sorted_out, uint32_t N,
-                                                                        uint32_t nb, long long B) {
+                                                                        uint32_t nb, uint32_t M, long long B) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     BkSmem& sm = *reinterpret_cast<BkSmem*>(smem_raw);
     const long long b = bidx();
@@ -170,46 +284,22 @@ __global__ void __launch_bounds__(kBkSortThreads, 2) bucket_sort_kernel(const ui
     if (n == 0) return;
     const uint32_t r0 = base[(size_t)b * nb + bk];
     const uint2* sl = slabs + ((size_t)b * nb + bk) * kBkCap;
+    const uint2* tab = tabs + (size_t)b * kBkBins;
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-    if (t == 0) { sm.kmin = 0xffffffffu; sm.kmax = 0u; }
+    constexpr int PER = kBkSlots / kBkSortThreads;
 #pragma unroll
-    for (int i = 0; i < kBkSlots / kBkSortThreads; ++i) sm.cnt[i * kBkSortThreads + t] = 0u;
-    uint2 kv[kBkEpt];
-    uint32_t lo = 0xffffffffu, hi = 0u;
-#pragma unroll
-    for (int j = 0; j < kBkEpt; ++j) {
-        const uint32_t e = j * kBkSortThreads + t;
-        if (e < n) {
-            kv[j] = __ldcs(sl + e);
-            lo = min(lo, kv[j].x); hi = max(hi, kv[j].x);
-        }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
-        hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    for (int i = 0; i < PER; ++i) sm.cnt[i * kBkSortThreads + t] = 0u;
+    __syncthreads();
+    // 1. slot populations (the slab stays in L2 for step 3)
+#pragma unroll 4
+    for (uint32_t e = t; e < n; e += kBkSortThreads) {
+        const uint32_t s = bs_of(__ldcg(&sl[e].x), tab, M) & (uint32_t)(kBkSlots - 1);
+        atomicAdd(&sm.cnt[s], 1u);
+        sm.slot[e] = (unsigned short)s;
     }
     __syncthreads();
-    if (lane == 0) { atomicMin(&sm.kmin, lo); atomicMax(&sm.kmax, hi); }
-    __syncthreads();
-    const uint32_t kmin = sm.kmin;
-    // monotone map of (key - kmin) onto the slots: int -> float conversion, multiplication by a positive constant and
-    // truncation are all monotone, so equal keys share a slot and a larger key never lands in an earlier slot
-    const float scale = (float)kBkSlots / ((float)(sm.kmax - kmin) + 1.0f) * 0.999f;
-    uint32_t sc[kBkEpt];            // slot << 16 | arrival number inside the slot
-#pragma unroll
-    for (int j = 0; j < kBkEpt; ++j) {
-        const uint32_t e = j * kBkSortThreads + t;
-        if (e < n) {
-            const uint32_t s = min((uint32_t)(__uint2float_rz(kv[j].x - kmin) * scale), (uint32_t)(kBkSlots - 1));
-            const uint32_t c = atomicAdd(&sm.cnt[s], 1u);
-            sc[j] = (s << 16) | c;            // c < 8192 < 2^16
-        }
-    }
-    __syncthreads();
-    // exclusive scan of the slot populations (16 consecutive slots per thread)
+    // 2. exclusive scan of the slot populations (PER consecutive slots per thread)
     {
-        constexpr int PER = kBkSlots / kBkSortThreads;
         uint32_t c[PER], sum = 0;
 #pragma unroll
         for (int i = 0; i < PER; ++i) { c[i] = sm.cnt[t * PER + i]; sum += c[i]; }
@@ -229,24 +319,32 @@ __global__ void __launch_bounds__(kBkSortThreads, 2) bucket_sort_kernel(const ui
         for (int i = 0; i < PER; ++i) { sm.cnt[t * PER + i] = run; run += c[i]; }
     }
     __syncthreads();
-#pragma unroll
-    for (int j = 0; j < kBkEpt; ++j) {
-        const uint32_t e = j * kBkSortThreads + t;
-        if (e < n) sm.pair[sm.cnt[sc[j] >> 16] + (sc[j] & 0xffffu)] = ((unsigned long long)kv[j].x << 32) | kv[j].y;
+    // 3. every pair into its slot's range (any order); cnt[s] ends as the END of slot s
+#pragma unroll 4
+    for (uint32_t e = t; e < n; e += kBkSortThreads) {
+        const uint2 kv = __ldcs(sl + e);
+        const uint32_t q = atomicAdd(&sm.cnt[sm.slot[e]], 1u);
+        sm.pair[q] = ((unsigned long long)kv.x << 32) | kv.y;
     }
     __syncthreads();
-    // exact rank among the slot mates (they are contiguous); (key, index) words are all distinct
-    for (uint32_t p = t; p < n; p += kBkSortThreads) {
-        const unsigned long long me = sm.pair[p];
-        const uint32_t key = (uint32_t)(me >> 32);
-        const uint32_t s = min((uint32_t)(__uint2float_rz(key - kmin) * scale), (uint32_t)(kBkSlots - 1));
-        const uint32_t a = sm.cnt[s];
-        const uint32_t z = (s + 1 < (uint32_t)kBkSlots) ? sm.cnt[s + 1] : n;
-        uint32_t r = a;
-        for (uint32_t q = a; q < z; ++q) r += (sm.pair[q] < me);
-        const size_t g = (size_t)b * N + r0 + r;
-        idx_out[g] = (uint32_t)me;
-        if (sorted_out) sorted_out[g] = val_of(key);
+    // 4. exact rank of every pair among its slot mates (they are contiguous; the 64-bit (key, index) words are all
+    //    distinct), one pair per thread at a time, and the index goes to that rank
+    uint32_t* io = idx_out + (size_t)b * N + r0;
+    float* so = sorted_out ? sorted_out + (size_t)b * N + r0 : nullptr;
+#pragma unroll 2
+    for (uint32_t q = t; q < n; q += kBkSortThreads) {
+        const unsigned long long v = sm.pair[q];
+        const uint32_t key = (uint32_t)(v >> 32);
+        const uint32_t s = bs_of(key, tab, M) & (uint32_t)(kBkSlots - 1);
+        const uint32_t z = sm.cnt[s];
+        const uint32_t a = s ? sm.cnt[s - 1] : 0u;
+        uint32_t r = q;
+        if (z - a > 1u) {
+            r = a;
+            for (uint32_t h = a; h < z; ++h) r += (sm.pair[h] < v);
+        }
+        io[r] = (uint32_t)v;
+        if (so) so[r] = val_of(key);
     }
 }
 
@@ -259,39 +357,78 @@ inline bool bucket32_applicable(size_t elem_size, long long N) {
 
 inline cudaError_t bucket32_set_attrs() {
     cudaFuncSetAttribute(bucket_sort_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    return cudaFuncSetAttribute(bucket_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BkSmem));
+    cudaFuncSetAttribute(bucket_part_kernel<0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaFuncSetAttribute(bucket_part_kernel<1>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaError_t e = cudaFuncSetAttribute(bucket_part_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PartSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket_part_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PartSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BkSmem));
+    return e;
 }
 
-// control words: hist [B][65536] u32 | cursor [B][nb] | overflow [B] (zeroed per call) | tab [B][65536] uint2 | base [B][nb]
+// geometry of the two partition levels for N keys per curve
+struct BkGeom {
+    uint32_t nb, lb, nc, cap1, tiles1;
+};
+inline BkGeom bucket32_geom(long long N) {
+    BkGeom g;
+    g.nb = (uint32_t)(N >> kBkMeanLog);
+    const int nbits = ilog2_u64((uint64_t)g.nb);
+    g.lb = (uint32_t)(nbits / 2);
+    g.nc = g.nb >> g.lb;                                        // <= 256
+    const uint32_t mean1 = (uint32_t)(N / g.nc);
+    g.cap1 = mean1 + mean1 / 2;                                 // coarse slabs: 50% head room
+    g.tiles1 = (g.cap1 + kBkPartTile - 1) / kBkPartTile;
+    return g;
+}
+
+// pair scratch (in uint2 units): fine slabs [B][nb][kBkCap] then coarse slabs [B][nc][cap1]
+inline size_t bucket32_pair_elems(long long B, long long N) {
+    const BkGeom g = bucket32_geom(N);
+    return (size_t)B * g.nb * kBkCap + (size_t)B * g.nc * g.cap1;
+}
+
+// control words: hist [B][65536] u32 | cursor2 [B][nb] | cursor1 [B][256] | overflow [B] (zeroed per call) |
+//                tab [B][65536] uint2 | base [B][nb]
+inline size_t bucket32_zero_bytes(long long B, long long N) {
+    const size_t nb = (size_t)(N >> kBkMeanLog);
+    return (size_t)B * kBkBins * 4 + (size_t)B * nb * 4 + (size_t)B * kBkMaxDigits * 4 + (size_t)B * 4;
+}
 inline size_t bucket32_ctl_bytes(long long B, long long N) {
     const size_t nb = (size_t)(N >> kBkMeanLog);
-    return align_up((size_t)B * kBkBins * 4 + (size_t)B * nb * 4 + (size_t)B * 4, 256) +
-           align_up((size_t)B * kBkBins * 8, 256) + align_up((size_t)B * nb * 4, 256);
+    return align_up(bucket32_zero_bytes(B, N), 256) + align_up((size_t)B * kBkBins * 8, 256) + align_up((size_t)B * nb * 4, 256);
 }
 
 // vals [B][N] -> idx_out (and optionally the sorted values) for the curves whose buckets all fit; *overflow_out points
-// at the per-curve flags (1 = not sorted here).  slabs: B*N*2 (key, index) pairs of scratch.
+// at the per-curve flags (1 = not sorted here).  pairs: bucket32_pair_elems(B, N) (key, index) pairs of scratch.
 inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* sorted_out, long long B, long long N,
-                                 uint2* slabs, void* ctl, const uint32_t** overflow_out, cudaStream_t st) {
-    const uint32_t nb = (uint32_t)(N >> kBkMeanLog);
+                                 uint2* pairs, void* ctl, const uint32_t** overflow_out, cudaStream_t st) {
+    const BkGeom g = bucket32_geom(N);
     unsigned char* w = (unsigned char*)ctl;
     uint32_t* hist = (uint32_t*)w;
-    uint32_t* cursor = hist + (size_t)B * kBkBins;
-    uint32_t* overflow = cursor + (size_t)B * nb;
-    const size_t zero_bytes = (size_t)B * kBkBins * 4 + (size_t)B * nb * 4 + (size_t)B * 4;
+    uint32_t* cursor2 = hist + (size_t)B * kBkBins;
+    uint32_t* cursor1 = cursor2 + (size_t)B * g.nb;
+    uint32_t* overflow = cursor1 + (size_t)B * kBkMaxDigits;
+    const size_t zero_bytes = bucket32_zero_bytes(B, N);
     w += align_up(zero_bytes, 256);
     uint2* tab = (uint2*)w; w += align_up((size_t)B * kBkBins * 8, 256);
     uint32_t* base = (uint32_t*)w;
+    uint2* slabs2 = pairs;
+    uint2* slabs1 = pairs + (size_t)B * g.nb * kBkCap;
     cudaError_t e = cudaMemsetAsync(hist, 0, zero_bytes, st);
     if (e != cudaSuccess) return e;
     const uint32_t nsamp = (uint32_t)(N >> kBkSampleLog);
     AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B)));
-    AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)B, 1024, 0, st>>>(hist, tab)));
-    AGN_LAUNCH(K_SORT_PART, st, (bucket_part_kernel<<<bgrid((unsigned)(N / (kBkPartThreads * kBkPartEpt)), B), kBkPartThreads, 0, st>>>(
-        vals, tab, cursor, slabs, overflow, (uint32_t)N, nb, B)));
-    AGN_LAUNCH(K_SORT_CDF, st, (bucket_base_kernel<<<(unsigned)B, 1024, 0, st>>>(cursor, base, nb)));
-    AGN_LAUNCH(K_SORT_BUCKET, st, (bucket_sort_kernel<<<bgrid(nb, B), kBkSortThreads, sizeof(BkSmem), st>>>(
-        slabs, cursor, base, overflow, idx_out, sorted_out, (uint32_t)N, nb, B)));
+    AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)B, 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
+    PartArgs a;
+    a.vals = vals; a.in = slabs1; a.in_count = cursor1; a.overflow = overflow; a.tab = tab;
+    a.N = (uint32_t)N; a.nb = g.nb; a.M = bucket32_magic(g.nb); a.lb = g.lb; a.nc = g.nc; a.cap_in = g.cap1; a.tiles_in = g.tiles1; a.B = B;
+    a.out = slabs1; a.cursor = cursor1; a.cap_out = g.cap1;
+    AGN_LAUNCH(K_SORT_PART, st, (bucket_part_kernel<0><<<bgrid((unsigned)(N / kBkPartTile), B), kBkPartThreads, sizeof(PartSmem), st>>>(a)));
+    a.out = slabs2; a.cursor = cursor2; a.cap_out = kBkCap;
+    AGN_LAUNCH(K_SORT_PART, st, (bucket_part_kernel<1><<<bgrid(g.tiles1 * g.nc, B), kBkPartThreads, sizeof(PartSmem), st>>>(a)));
+    AGN_LAUNCH(K_SORT_CDF, st, (bucket_base_kernel<<<(unsigned)B, 1024, 0, st>>>(cursor2, base, g.nb)));
+    AGN_LAUNCH(K_SORT_BUCKET, st, (bucket_sort_kernel<<<bgrid(g.nb, B), kBkSortThreads, sizeof(BkSmem), st>>>(
+        slabs2, cursor2, base, overflow, tab, idx_out, sorted_out, (uint32_t)N, g.nb, a.M, B)));
     *overflow_out = overflow;
     return cudaGetLastError();
 }

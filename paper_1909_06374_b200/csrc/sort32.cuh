@@ -331,6 +331,7 @@ inline bool sort32_applicable(size_t elem_size, long long N) {
 inline size_t sort32_ws_bytes(long long B, long long N) {
     const size_t ntiles = (size_t)(N / kS32Tile);
     size_t s = 2 * align_up((size_t)B * N * sizeof(uint2), 256);
+    if (bucket32_applicable(4, N)) s = std::max(s, align_up(bucket32_pair_elems(B, N) * sizeof(uint2), 256));
     s += align_up((size_t)B * 4 * kRadix * 4 + (size_t)B * 4 * 4 + (size_t)B * 4 * ntiles * kRadix * 4, 256);
     if (bucket32_applicable(4, N)) s += bucket32_ctl_bytes(B, N);
     return s;
@@ -343,6 +344,7 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
     unsigned char* w = (unsigned char*)ws;
     uint2* pa = (uint2*)w; w += align_up((size_t)B * N * sizeof(uint2), 256);
     uint2* pb = (uint2*)w; w += align_up((size_t)B * N * sizeof(uint2), 256);
+    if (bucket32_applicable(4, N)) w = (unsigned char*)ws + std::max((size_t)(w - (unsigned char*)ws), align_up(bucket32_pair_elems(B, N) * sizeof(uint2), 256));
     const size_t ntiles = (size_t)(N / kS32Tile);
     uint32_t* hist = (uint32_t*)w;
     uint32_t* ticket = hist + (size_t)B * NP * kRadix;
