@@ -24,13 +24,13 @@
 
 namespace agn {
 
-constexpr int kBkMeanLog = 12;                    // mean bucket population 2^12
-constexpr int kBkCap = 8192;                      // slab slots per bucket
+constexpr int kBkMeanLog = 11;                    // mean bucket population 2^11
+constexpr int kBkCap = 4096;                      // slab slots per bucket
 constexpr int kBkSampleLog = 6;                   // one sample per 64 keys
 constexpr int kBkBinLog = 16;                     // CDF bins = top 16 key bits
 constexpr int kBkBins = 1 << kBkBinLog;
-constexpr int kBkSortThreads = 1024;
-constexpr int kBkSlotLog = 12;
+constexpr int kBkSortThreads = 512;
+constexpr int kBkSlotLog = 11;
 constexpr int kBkSlots = 1 << kBkSlotLog;         // interpolation slots of the in-CTA sort
 constexpr int kBkEpt = kBkCap / kBkSortThreads;   // 16 elements per thread
 
@@ -47,7 +47,7 @@ __device__ __forceinline__ uint32_t bs_of(uint32_t key, const uint2* __restrict_
     return __umulhi(pos, M);
 }
 inline uint32_t bucket32_magic(uint32_t nb) {
-    return (uint32_t)((((unsigned __int128)nb) << (32 + 12 + 9)) / (kBkTotalW << 16));
+    return (uint32_t)((((unsigned __int128)nb) << (32 + kBkSlotLog + 9)) / (kBkTotalW << 16));
 }
 
 __global__ void __launch_bounds__(256) cdf_sample_kernel(const float* __restrict__ vals, uint32_t* __restrict__ hist,
@@ -116,7 +116,10 @@ struct PartSmem {
 };
 
 struct PartArgs {
-    const float* vals;          // LEVEL 0 input [B][N]
+    const float* vals;          // LEVEL 0 input [B][N]; LEVEL 2: the sorted ERDF draw [B][N]
+    const uint32_t* idx_new;    // LEVEL 2 (rank scatter, bin step): permutation of this iteration,
+    const uint32_t* idx_old;    //          of the previous one,
+    unsigned long long* changed;//          and the change counters [B]
     const uint2* in;            // LEVEL 1 input: coarse slabs [B][nc][cap_in]
     const uint32_t* in_count;   // LEVEL 1: populations of the coarse slabs [B][nc]
     uint2* out;                 // slabs [B][n_out][cap_out]
@@ -125,7 +128,7 @@ struct PartArgs {
     const uint2* tab;           // [B][65536]
     uint32_t N, nb;             // keys per curve, fine buckets per curve
     uint32_t M;                 // bucket32_magic(nb)
-    uint32_t lb;                // low (fine) bits of the bucket number
+    uint32_t lb;                // low (fine) bits of the bucket number; LEVEL 2: shift of the destination window
     uint32_t nc;                // coarse slabs per curve
     uint32_t cap_in, cap_out;
     uint32_t tiles_in;          // LEVEL 1: tiles per coarse slab
@@ -154,6 +157,19 @@ __global__ void __launch_bounds__(kBkPartThreads, 4) bucket_part_kernel(PartArgs
         const float* v = a.vals + (size_t)b * a.N;
 #pragma unroll
         for (int j = 0; j < kBkPartEpt; ++j) kv[j] = make_uint2(key_of(__ldcs(v + e0 + j * kBkPartThreads)), e0 + j * kBkPartThreads);
+    } else if (LEVEL == 2) {
+        // L5 bin step: (value, destination) pairs by destination window; L5's change count on the way
+        const size_t g0 = (size_t)b * a.N + e0;
+        uint32_t diff = 0;
+#pragma unroll
+        for (int j = 0; j < kBkPartEpt; ++j) {
+            const uint32_t dst = __ldcs(a.idx_new + g0 + j * kBkPartThreads);
+            diff += (dst != __ldcs(a.idx_old + g0 + j * kBkPartThreads));
+            kv[j] = make_uint2(__float_as_uint(__ldcs(a.vals + g0 + j * kBkPartThreads)), dst);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) diff += __shfl_xor_sync(0xffffffffu, diff, o);
+        if (lane == 0 && diff) atomicAdd(&a.changed[b], (unsigned long long)diff);
     } else {
         const uint2* v = a.in + ((size_t)b * a.nc + coarse) * a.cap_in;
 #pragma unroll
@@ -168,8 +184,8 @@ __global__ void __launch_bounds__(kBkPartThreads, 4) bucket_part_kernel(PartArgs
     const uint32_t dshift = kBkSlotLog + ((LEVEL == 0) ? a.lb : 0u);
 #pragma unroll
     for (int j = 0; j < kBkPartEpt; ++j) {
-        const bool valid = (LEVEL == 0) || (e0 + j * kBkPartThreads < n_in);
-        const uint32_t d = valid ? ((bs_of(kv[j].x, tab, a.M) >> dshift) & dmask) : 0xffffu;
+        const bool valid = (LEVEL != 1) || (e0 + j * kBkPartThreads < n_in);
+        const uint32_t d = (LEVEL == 2) ? (kv[j].y >> a.lb) : (valid ? ((bs_of(kv[j].x, tab, a.M) >> dshift) & dmask) : 0xffffu);
         const uint32_t d0 = __shfl_sync(0xffffffffu, d, 0);
         const uint32_t same = __ballot_sync(0xffffffffu, d == d0);
         uint32_t r = 0;
@@ -184,12 +200,12 @@ __global__ void __launch_bounds__(kBkPartThreads, 4) bucket_part_kernel(PartArgs
     // thread == digit: reserve the digit's range in its slab, exclusive scan of the populations
     {
         const uint32_t c = sm.cnt[t];
-        const uint32_t slab = (LEVEL == 0) ? (uint32_t)t : ((coarse << a.lb) | (uint32_t)t);
-        const uint32_t n_out = (LEVEL == 0) ? a.nc : a.nb;
+        const uint32_t slab = (LEVEL != 1) ? (uint32_t)t : ((coarse << a.lb) | (uint32_t)t);
+        const uint32_t n_out = (LEVEL != 1) ? a.nc : a.nb;
         uint32_t g = 0;
         if (c) {
             g = atomicAdd(&a.cursor[(size_t)b * n_out + slab], c);
-            if (g + c > a.cap_out) a.overflow[b] = 1u;
+            if (LEVEL != 2 && g + c > a.cap_out) a.overflow[b] = 1u;
         }
         uint32_t inc = c;
 #pragma unroll
@@ -209,7 +225,7 @@ __global__ void __launch_bounds__(kBkPartThreads, 4) bucket_part_kernel(PartArgs
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < kBkPartEpt; ++j) {
-        const bool valid = (LEVEL == 0) || (e0 + j * kBkPartThreads < n_in);
+        const bool valid = (LEVEL != 1) || (e0 + j * kBkPartThreads < n_in);
         if (valid) {
             const uint32_t d = dr[j] >> 16, s = sm.lstart[d] + (dr[j] & 0xffffu);
             sm.stage[s] = kv[j];
@@ -218,9 +234,9 @@ __global__ void __launch_bounds__(kBkPartThreads, 4) bucket_part_kernel(PartArgs
     }
     __syncthreads();
     const uint32_t n_tile = min((uint32_t)kBkPartTile, n_in - tile * kBkPartTile);
-    const uint32_t n_out = (LEVEL == 0) ? a.nc : a.nb;
+    const uint32_t n_out = (LEVEL != 1) ? a.nc : a.nb;
     uint2* out = a.out + (size_t)b * n_out * a.cap_out;
-    const uint32_t slab0 = (LEVEL == 0) ? 0u : (coarse << a.lb);
+    const uint32_t slab0 = (LEVEL != 1) ? 0u : (coarse << a.lb);
 #pragma unroll 4
     for (uint32_t s = t; s < n_tile; s += kBkPartThreads) {
         const uint32_t d = sm.sdig[s];
@@ -266,7 +282,7 @@ struct BkSmem {
     uint32_t wsum[kBkSortThreads / 32];
 };
 
-__global__ void __launch_bounds__(kBkSortThreads, 2) bucket_sort_kernel(const uint2* __restrict__ slabs,
+__global__ void __launch_bounds__(kBkSortThreads, 4) bucket_sort_kernel(const uint2* __restrict__ slabs,
                                                                         const uint32_t* __restrict__ cursor,
                                                                         const uint32_t* __restrict__ base,
                                                                         const uint32_t* __restrict__ overflow,
@@ -359,8 +375,10 @@ inline cudaError_t bucket32_set_attrs() {
     cudaFuncSetAttribute(bucket_sort_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     cudaFuncSetAttribute(bucket_part_kernel<0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     cudaFuncSetAttribute(bucket_part_kernel<1>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaFuncSetAttribute(bucket_part_kernel<2>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     cudaError_t e = cudaFuncSetAttribute(bucket_part_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PartSmem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket_part_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PartSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket_part_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PartSmem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BkSmem));
     return e;
 }

@@ -8,6 +8,7 @@
 //     round trip, all in-segment indices are 32-bit.
 // Segments are power-of-two lengths >= 2^15, so every tile is full.
 #pragma once
+#include <cstring>
 #include "common.cuh"
 #include "sort.cuh"
 #include "bucket32.cuh"
@@ -388,8 +389,13 @@ inline cudaError_t rank_scatter_two_level32(const uint32_t* idx_new, const uint3
                                             long long B, long long N, uint2* pairs, uint32_t* cursor,
                                             unsigned long long* changed, cudaStream_t st) {
     const int shift = ilog2_u64((uint64_t)N) - kRadixBits;
-    AGN_LAUNCH(K_SCATTER_BIN, st, (scatter_bin32_kernel<<<bgrid((unsigned)(N / kS32Tile), B), kS32Threads, sizeof(S32Smem), st>>>(
-        idx_new, idx_old, sorted, pairs, (uint32_t)N, shift, cursor, changed, B)));
+    // bin step: the tile kernel of bucket32.cuh in its LEVEL 2 form (no order is needed inside a window)
+    PartArgs a;
+    memset(&a, 0, sizeof(a));
+    a.vals = sorted; a.idx_new = idx_new; a.idx_old = idx_old; a.changed = changed;
+    a.out = pairs; a.cursor = cursor; a.N = (uint32_t)N; a.lb = (uint32_t)shift; a.nc = kRadix; a.nb = kRadix;
+    a.cap_out = (uint32_t)(N >> kRadixBits); a.B = B;
+    AGN_LAUNCH(K_SCATTER_BIN, st, (bucket_part_kernel<2><<<bgrid((unsigned)(N / kBkPartTile), B), kBkPartThreads, sizeof(PartSmem), st>>>(a)));
     AGN_LAUNCH(K_SCATTER_PLACE, st, (scatter_place32_kernel<<<bgrid((unsigned)(N / 2048), B), 256, 0, st>>>(
         (const uint4*)pairs, x, (uint32_t)N, cursor, B)));
     return cudaGetLastError();
