@@ -36,7 +36,8 @@ ALGO_BYTES_PER_SAMPLE = {
     "amplitude_replace": 10.0,      # read Z 4 + A_norm 2 + write Z' 4
     "sort_digit_hist": 4.0,         # read keys
     "sort_onesweep": 16.0,          # read (key, idx) 8 + write (key, idx) 8 (first/last pass move less)
-    "sort_msd_partition": 12.0,     # read key 4 + write (key, idx) 8
+    "sort_cdf_tables": 0.5,         # one key in 64, a 32-byte sector each (+ small tables)
+    "sort_msd_partition": 14.0,     # mean of the two levels: (key 4 -> pair 8) and (pair 8 -> pair 8)
     "sort_bucket_finish": 12.0,     # read (key, idx) 8 + write idx 4
     "cta_argsort": 8.0,             # read key 4 + write idx 4
     "rank_scatter_count": 16.0,     # idx_new 4 + idx_old 4 + sorted 4 + write x 4
@@ -48,7 +49,7 @@ STAGE_MODEL_BYTES = {"fft": 26.0, "argsort": 28.0, "scatter": 32.0}
 STAGE_OF = {
     "fft_pass_strided": "fft", "fft_pass_contiguous": "fft", "amplitude_replace": "fft", "fft_mid_fused": "fft",
     "sort_digit_hist": "argsort", "sort_onesweep": "argsort", "cta_argsort": "argsort",
-    "sort_msd_partition": "argsort", "sort_bucket_finish": "argsort",
+    "sort_msd_partition": "argsort", "sort_bucket_finish": "argsort", "sort_cdf_tables": "argsort",
     "rank_scatter_count": "scatter", "scatter_bin": "scatter", "scatter_place": "scatter",
 }
 
