@@ -168,7 +168,17 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
     AGN_LAUNCH(K_PERM_ANORM, st, (perm_anorm_kernel<T><<<bgrid(cdiv(L + 1, 256), B), 256, 0, st>>>((const T*)d_anorm, Ap, plan.dg, (int)B)));
     const unsigned sg = (unsigned)std::min<long long>((N + 1023) / 1024, 148 * 16);
     // first x_sim: the draw in draw order (Q15)
-    AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, false><<<bgrid(sg, B), 256, 0, st>>>(d_perm, nullptr, sorted, x, N, nullptr, (int)B)));
+    bool first_done = false;
+    if constexpr (sizeof(T) == 4) {
+        if (two_level && sort32_applicable(sizeof(T), N)) {
+            // same two-level scatter as in the loop (idx_old = idx_new: the change count stays 0)
+            if (rank_scatter_two_level32(d_perm, d_perm, sorted, x, B, N, (uint2*)sort_ws, cursor, changed, st) != cudaSuccess)
+                return AGNVAR_ECUDA;
+            first_done = true;
+        }
+    }
+    if (!first_done)
+        AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, false><<<bgrid(sg, B), 256, 0, st>>>(d_perm, nullptr, sorted, x, N, nullptr, (int)B)));
     uint32_t* cur = d_perm;
     uint32_t* nxt = P1;
     for (int k = 1; k <= max_iter; ++k) {
