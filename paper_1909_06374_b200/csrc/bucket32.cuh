@@ -1,23 +1,26 @@
-// bucket32.cuh -- L4 for long fp32 curves as a TWO-LEVEL sort (SURVEY 8(d) "2-level" model: every key crosses HBM
-// twice instead of four LSD round trips):
+// bucket32.cuh -- L4 for long fp32 curves (N >= 2^18) as a distribution sort: every key is routed by an estimate of
+// the CDF of the keys to one of N/2048 equal-depth buckets, and each bucket is finished in shared memory.
 //
 //   cdf_sample_kernel    one key in 64 -> a 65536-bin histogram of the key's top 16 bits (per curve)
-//   cdf_table_kernel     exclusive scan -> table (cum, cnt) per bin: a piecewise-linear estimate of the CDF of the
-//                        keys.  bucket(key) = (cum*2^16 + low16(key)*cnt) >> 22 is a MONOTONE map of the key onto
-//                        N/4096 equal-depth buckets (64 samples = 4096 keys per bucket on average).
-//   bucket_part_kernel   one pass over x_adj: (key, time index) pairs appended to their bucket's slab
-//                        (kBkCap = 8192 slots, cursor per bucket).  4 B in + 8 B out per sample.
+//   cdf_table_kernel     exclusive scan of the add-one smoothed bin weights -> table (cumw << 7, w): a piecewise-
+//                        linear, strictly monotone estimate of the CDF.  bs_of(key) = bucket << 11 | slot costs one
+//                        table look-up, one 32x32 multiply and one multiply-high.
+//   bucket_part_kernel   <0> x_adj -> (key, time index) pairs in N^(1/2)-ish coarse slabs (high bits of the bucket),
+//                        <1> coarse slab -> fine slabs (kBkCap = 4096 slots per bucket, mean population 2048),
+//                        <2> the bin step of the two-level rank scatter L5 (same tile logic, digit = window of dst).
+//                        A tile counts its keys per digit in shared memory, reserves one range per (tile, digit) with
+//                        one global atomic, orders the tile by digit in shared memory and writes coalesced runs.
 //   bucket_base_kernel   exclusive scan of the bucket populations -> first rank of every bucket
-//   bucket_sort_kernel   one CTA per bucket: the slab is sorted in shared memory by (key, index) -- an
-//                        interpolation counting sort into 8192 slots followed by an exact rank among the few
-//                        slot mates -- and the indices are written at their ranks.  8 B in + 4 B out per sample.
+//   bucket_sort_kernel   one CTA per bucket: counting sort into 2048 interpolation slots (the next 11 bits of bs_of),
+//                        then the exact rank of every pair among its few slot mates; indices written at their ranks.
 //
+// HBM bytes per sample: 0.5 (sample) + 12 (<0>: 4 in, 8 out) + 16 (<1>) + 12 (finish: 8 in, 4 out).
 // Order inside a slab is arbitrary (atomic cursors), so the final order is defined by the comparison of the 64-bit
 // (key, index) words alone: equal keys come out by ascending time index, which is the stable order the definition
 // asks for (O6 step 4), independently of the run.
-// A bucket that would overflow its slab (inputs with massive ties, or a distribution the sampled CDF misses) raises
-// the curve's `overflow` flag; the LSD passes of sort32.cuh then sort that curve instead (they are always enqueued
-// and exit at once when the flag is clear: the decision is taken on the device, no host synchronisation).
+// A slab that would overflow (inputs with massive ties, or a distribution the sampled CDF misses) raises the curve's
+// `overflow` flag; the LSD passes of sort32.cuh then sort that curve instead (they are always enqueued and exit at
+// once when the flag is clear: the decision is taken on the device, no host synchronisation).
 #pragma once
 #include "common.cuh"
 #include "sort.cuh"
@@ -38,7 +41,7 @@ constexpr int kBkEpt = kBkCap / kBkSortThreads;   // 16 elements per thread
 // 2^24 and the add-one mass 2^16 whatever N is: keys of an unsampled bin still spread linearly over their own
 // stretch instead of collapsing onto one point), pos = cumw * 2^16 + low16(key) * w < (2^24 + 2^16) * 2^16.
 // The table holds (cumw << 7, w), so that pos >> 9 = tab.x + ((low16 * w) >> 9) fits 32 bits, and
-// bs = bucket << 12 | slot = floor((pos >> 9) * M / 2^32) with M = floor(2^32 * nb * 4096 * 512 / (total * 2^16)):
+// bs = bucket << 11 | slot = floor((pos >> 9) * M / 2^32) with M = floor(2^32 * nb * 2048 * 512 / (total * 2^16)):
 // one multiply-high.  Every step is monotone in the key, and equal keys get equal bs.
 constexpr unsigned long long kBkTotalW = (1ull << 24) + (1ull << 16);
 __device__ __forceinline__ uint32_t bs_of(uint32_t key, const uint2* __restrict__ tab, uint32_t M) {
