@@ -33,6 +33,7 @@ ALGO_BYTES_PER_SAMPLE = {
     "fft_pass_strided": 8.0,        # read + write one complex half-length array = 4 + 4 B per real sample
     "fft_pass_contiguous": 8.0,
     "fft_mid_fused": 10.0,          # read Z 4 + A_norm 2 + write Z' 4
+    "fft_columns": 8.0,             # all column sub-passes of one direction: read 4 + write 4 (intermediates stay in L2)
     "amplitude_replace": 10.0,      # read Z 4 + A_norm 2 + write Z' 4
     "sort_digit_hist": 4.0,         # read keys
     "sort_onesweep": 16.0,          # read (key, idx) 8 + write (key, idx) 8 (first/last pass move less)
@@ -47,7 +48,7 @@ ALGO_BYTES_PER_SAMPLE = {
 # SURVEY.md 8(d) two-level model, bytes per sample per iteration, per stage (fp32)
 STAGE_MODEL_BYTES = {"fft": 26.0, "argsort": 28.0, "scatter": 32.0}
 STAGE_OF = {
-    "fft_pass_strided": "fft", "fft_pass_contiguous": "fft", "amplitude_replace": "fft", "fft_mid_fused": "fft",
+    "fft_pass_strided": "fft", "fft_pass_contiguous": "fft", "amplitude_replace": "fft", "fft_mid_fused": "fft", "fft_columns": "fft",
     "sort_digit_hist": "argsort", "sort_onesweep": "argsort", "cta_argsort": "argsort",
     "sort_msd_partition": "argsort", "sort_bucket_finish": "argsort", "sort_cdf_tables": "argsort",
     "rank_scatter_count": "scatter", "scatter_bin": "scatter", "scatter_place": "scatter",

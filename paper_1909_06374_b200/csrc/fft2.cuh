@@ -24,6 +24,7 @@ namespace agn {
 constexpr int kLogR1 = 13;              // row length of the mid kernel
 constexpr int kColThreads = 128;        // columns per column tile
 constexpr int kMaxColPhases = 3;
+constexpr int kColMaxLog = 6;            // largest column radix (log2): radix 64 in registers, 2 sub-passes for N = 2^26 (radix 16 with 3 sub-passes and 3.5x the warps measured 12 % slower)
 
 // ------------------------------------------------------------------------------------------------
 // column sub-passes
@@ -105,8 +106,10 @@ __device__ __forceinline__ void col_tile(const ColArgs<T>& a, int e, int b, int 
     }
 }
 
-template <typename T, int THREADS>
-__global__ void __launch_bounds__(THREADS, 1) fft_col_kernel(ColArgs<T> a) {
+// MAXLOG: largest radix (log2) this instantiation can run; the register budget follows it (radix 64: ~250 registers,
+// 2 CTAs per SM; radix 16: < 96 registers, 5 CTAs per SM, which hides the load latency far better)
+template <typename T, int THREADS, int MAXLOG>
+__global__ void __launch_bounds__(THREADS, (MAXLOG >= 6 ? 1 : (MAXLOG == 5 ? 3 : 5))) fft_col_kernel(ColArgs<T> a) {
     __shared__ unsigned int s_ticket;
     const int slots = a.prefix[a.nph];
     const int nsg = a.B * a.G;
@@ -133,8 +136,8 @@ __global__ void __launch_bounds__(THREADS, 1) fft_col_kernel(ColArgs<T> a) {
             __syncthreads();
         }
         switch (a.logRad[e]) {
-            case 6: col_tile<T, 6, THREADS>(a, e, b, g, q); break;
-            case 5: col_tile<T, 5, THREADS>(a, e, b, g, q); break;
+            case 6: if constexpr (MAXLOG >= 6) col_tile<T, 6, THREADS>(a, e, b, g, q); break;
+            case 5: if constexpr (MAXLOG >= 5) col_tile<T, 5, THREADS>(a, e, b, g, q); break;
             case 4: col_tile<T, 4, THREADS>(a, e, b, g, q); break;
             case 3: col_tile<T, 3, THREADS>(a, e, b, g, q); break;
             case 2: col_tile<T, 2, THREADS>(a, e, b, g, q); break;
@@ -393,7 +396,8 @@ inline Fft2Plan<T> fft2_plan_init(int logL, typename Cx<T>::type* tables, unsign
     Fft2Plan<T> p;
     p.logL = logL;
     p.logR0 = logL - kLogR1;
-    p.nph = (p.logR0 + 5) / 6;
+    p.nph = (p.logR0 + kColMaxLog - 1) / kColMaxLog;
+    if (p.nph > kMaxColPhases) p.nph = kMaxColPhases;
     {
         int base = p.logR0 / p.nph, extra = p.logR0 % p.nph;
         for (int i = 0; i < kMaxColPhases; ++i) p.logRad[i] = (i < p.nph) ? base + (i < extra ? 1 : 0) : 0;
@@ -437,8 +441,9 @@ template <typename T> inline cudaError_t fft2_set_attrs() {
     return cudaFuncSetAttribute(fft_mid_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMidSmemBytes);
 }
 
-inline int fft2_col_grid(const void* func, int threads) {
-    static int cached = 0;
+inline int fft2_col_grid(const void* func, int threads, int slot) {
+    static int cache[4] = {0, 0, 0, 0};
+    int& cached = cache[slot];
     if (cached) return cached;
     int dev = 0, sms = 0, per = 0;
     cudaGetDevice(&dev);
@@ -477,8 +482,18 @@ inline cudaError_t fft2_columns(const Fft2Plan<T>& p, bool inverse, const typena
     if (e != cudaSuccess) return e;
     a.ticket = p.counters; a.done = p.counters + 1;
     a.total = (unsigned)((B * a.G + (p.nph - 1) * a.D) * a.prefix[p.nph]);
-    const int grid = fft2_col_grid((const void*)fft_col_kernel<T, kColThreads>, kColThreads);
-    AGN_LAUNCH(K_FFT_COL, st, (fft_col_kernel<T, kColThreads><<<grid, kColThreads, 0, st>>>(a)));
+    int maxlog = 0;
+    for (int i = 0; i < p.nph; ++i) maxlog = std::max(maxlog, p.logRad[i]);
+    if (maxlog <= 4) {
+        const int grid = fft2_col_grid((const void*)fft_col_kernel<T, kColThreads, 4>, kColThreads, 0);
+        AGN_LAUNCH(K_FFT_COL, st, (fft_col_kernel<T, kColThreads, 4><<<grid, kColThreads, 0, st>>>(a)));
+    } else if (maxlog == 5) {
+        const int grid = fft2_col_grid((const void*)fft_col_kernel<T, kColThreads, 5>, kColThreads, 1);
+        AGN_LAUNCH(K_FFT_COL, st, (fft_col_kernel<T, kColThreads, 5><<<grid, kColThreads, 0, st>>>(a)));
+    } else {
+        const int grid = fft2_col_grid((const void*)fft_col_kernel<T, kColThreads, 6>, kColThreads, 2);
+        AGN_LAUNCH(K_FFT_COL, st, (fft_col_kernel<T, kColThreads, 6><<<grid, kColThreads, 0, st>>>(a)));
+    }
     return cudaGetLastError();
 }
 
