@@ -203,7 +203,10 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
         if constexpr (sizeof(T) == 4) {
             if (sort32_applicable(sizeof(T), N)) {
                 uint2* spare = nullptr;
-                if (seg_argsort32(Z, nxt, nullptr, B, N, sort_ws, &spare, st) != cudaSuccess) return AGNVAR_ECUDA;
+                // the CDF tables are re-estimated in every iteration: reusing them for 3 out of 4 iterations was measured to
+                // overflow slabs (stale table -> LSD fallback) often enough to cost more than the 0.25 ms it saves
+                const bool reuse_cdf = false;
+                if (seg_argsort32(Z, nxt, nullptr, B, N, sort_ws, &spare, st, reuse_cdf) != cudaSuccess) return AGNVAR_ECUDA;
                 if (two_level) {
                     if (rank_scatter_two_level32(nxt, cur, sorted, x, B, N, spare, cursor, changed, st) != cudaSuccess)
                         return AGNVAR_ECUDA;

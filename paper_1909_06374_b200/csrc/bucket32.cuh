@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(kBkPartThreads, 4) bucket_part_kernel(PartArgs
         if (valid) {
             const uint32_t d = dr[j] >> 16, s = sm.lstart[d] + (dr[j] & 0xffffu);
             sm.stage[s] = kv[j];
-            sm.sdig[s] = (unsigned char)d;
+            if (LEVEL != 2) sm.sdig[s] = (unsigned char)d;          // level 2 reads the digit off the pair itself
         }
     }
     __syncthreads();
@@ -242,9 +242,10 @@ __global__ void __launch_bounds__(kBkPartThreads, 4) bucket_part_kernel(PartArgs
     const uint32_t slab0 = (LEVEL != 1) ? 0u : (coarse << a.lb);
 #pragma unroll 4
     for (uint32_t s = t; s < n_tile; s += kBkPartThreads) {
-        const uint32_t d = sm.sdig[s];
+        const uint2 pr = sm.stage[s];
+        const uint32_t d = (LEVEL == 2) ? (pr.y >> a.lb) : (uint32_t)sm.sdig[s];
         const uint32_t off = sm.gdst[d] + s;
-        if (off < a.cap_out) out[(size_t)(slab0 + d) * a.cap_out + off] = sm.stage[s];
+        if (off < a.cap_out) out[(size_t)(slab0 + d) * a.cap_out + off] = pr;
     }
 }
 
@@ -422,8 +423,10 @@ inline size_t bucket32_ctl_bytes(long long B, long long N) {
 
 // vals [B][N] -> idx_out (and optionally the sorted values) for the curves whose buckets all fit; *overflow_out points
 // at the per-curve flags (1 = not sorted here).  pairs: bucket32_pair_elems(B, N) (key, index) pairs of scratch.
+// reuse_cdf: keep the CDF tables of the previous call on the same workspace (the key distribution of x_adj barely
+// moves from one E13 iteration to the next; a stale table can only cost a slab overflow, i.e. the LSD fallback).
 inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* sorted_out, long long B, long long N,
-                                 uint2* pairs, void* ctl, const uint32_t** overflow_out, cudaStream_t st) {
+                                 uint2* pairs, void* ctl, const uint32_t** overflow_out, bool reuse_cdf, cudaStream_t st) {
     const BkGeom g = bucket32_geom(N);
     unsigned char* w = (unsigned char*)ctl;
     uint32_t* hist = (uint32_t*)w;
@@ -436,11 +439,17 @@ inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* so
     uint32_t* base = (uint32_t*)w;
     uint2* slabs2 = pairs;
     uint2* slabs1 = pairs + (size_t)B * g.nb * kBkCap;
-    cudaError_t e = cudaMemsetAsync(hist, 0, zero_bytes, st);
-    if (e != cudaSuccess) return e;
-    const uint32_t nsamp = (uint32_t)(N >> kBkSampleLog);
-    AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B)));
-    AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)B, 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
+    cudaError_t e;
+    if (reuse_cdf) {
+        e = cudaMemsetAsync(cursor2, 0, zero_bytes - (size_t)B * kBkBins * 4, st);      // cursors and flags only
+        if (e != cudaSuccess) return e;
+    } else {
+        e = cudaMemsetAsync(hist, 0, zero_bytes, st);
+        if (e != cudaSuccess) return e;
+        const uint32_t nsamp = (uint32_t)(N >> kBkSampleLog);
+        AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B)));
+        AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)B, 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
+    }
     PartArgs a;
     a.vals = vals; a.in = slabs1; a.in_count = cursor1; a.overflow = overflow; a.tab = tab;
     a.N = (uint32_t)N; a.nb = g.nb; a.M = bucket32_magic(g.nb); a.lb = g.lb; a.nc = g.nc; a.cap_in = g.cap1; a.tiles_in = g.tiles1; a.B = B;

@@ -340,7 +340,7 @@ inline size_t sort32_ws_bytes(long long B, long long N) {
 
 // vals [B][N] -> idx_out [B][N]; optionally the sorted values.  Returns the free pair buffer (for the scatter) in *spare.
 inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* sorted_out, long long B, long long N,
-                                 void* ws, uint2** spare, cudaStream_t st) {
+                                 void* ws, uint2** spare, cudaStream_t st, bool reuse_cdf = false) {
     constexpr int NP = 4;
     unsigned char* w = (unsigned char*)ws;
     uint2* pa = (uint2*)w; w += align_up((size_t)B * N * sizeof(uint2), 256);
@@ -355,7 +355,7 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
     // long curves: two-level bucket sort (bucket32.cuh); the LSD passes below then only run for curves it gave up on
     const uint32_t* gate = nullptr;
     if (bucket32_applicable(4, N)) {
-        e = bucket32_sort(vals, idx_out, sorted_out, B, N, pa, w + align_up(ctl, 256), &gate, st);
+        e = bucket32_sort(vals, idx_out, sorted_out, B, N, pa, w + align_up(ctl, 256), &gate, reuse_cdf, st);
         if (e != cudaSuccess) return e;
     }
     e = cudaMemsetAsync(hist, 0, ctl, st);
