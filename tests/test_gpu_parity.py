@@ -249,6 +249,41 @@ def test_e13_ties_and_zero_amplitude(ag, orc):
         assert out["changed_hist"][b, 0].item() == np.count_nonzero(pnew[b] != perm0[b])
 
 
+@pytest.mark.parametrize("N", [2 ** 18, 2 ** 21])
+@pytest.mark.parametrize("case", ["red_noise", "quantised", "all_equal", "one_outlier"])
+def test_long_curve_argsort_paths(ag, orc, N, case):
+    """fp32 curves of N >= 2^18 go through the distribution sort (bucket32.cuh); inputs it cannot bucket (massive
+    ties -> slab overflow) must fall back to the LSD passes on the device.  Either way the permutation is THE stable
+    argsort of the GPU's own x_adj, the scatter is exact and the change count is exact."""
+    B = 2
+    rng = np.random.default_rng(5)
+    srt = np.sort(rng.standard_normal((B, N)).astype(np.float32), axis=1)
+    perm0 = np.stack([rng.permutation(N) for _ in range(B)]).astype(np.uint32)
+    an = np.zeros((B, N // 2 + 1), dtype=np.float32)
+    if case == "red_noise":
+        j = np.arange(1, N // 2 + 1)
+        an[:, 1:] = (1.0 / j).astype(np.float32)          # x_adj smooth in time, continuous distribution
+    elif case == "quantised":
+        an[:, N // 8] = 1.0                                # period-8 tone: at most 8 distinct values, N/8 copies each
+    elif case == "all_equal":
+        pass                                               # zero amplitudes: x_adj == 0 everywhere
+    else:
+        an[:, 0] = 1e-3                                    # constant + one huge spike bin pair -> extreme key range
+        an[:, 1] = 1e30
+    d = lambda a: torch.tensor(a.view(np.int32) if a.dtype == np.uint32 else a, device="cuda")
+    perm = d(perm0)
+    out = ag.agnvar_e13_iterate(d(an), d(srt), perm, 1, want_hist=True, want_xadj=True)
+    xadj = out["x_adj"].cpu().numpy()
+    pnew, x = u32(out["perm"]), out["x"].cpu().numpy()
+    for b in range(B):
+        assert np.isfinite(xadj[b]).all()
+        assert (pnew[b] == orc.stable_argsort(xadj[b].astype(np.float64))).all()
+        xs = np.empty(N, dtype=np.float32)
+        xs[pnew[b]] = srt[b]
+        assert (x[b] == xs).all()
+        assert out["changed_hist"][b, 0].item() == np.count_nonzero(pnew[b] != perm0[b])
+
+
 # ---- boundary behaviour ---------------------------------------------------------------------------
 def test_error_codes(ag):
     import ctypes as C
