@@ -320,11 +320,14 @@ __global__ void __launch_bounds__(kBkSortThreads, 4) bucket_sort_kernel(const ui
     __syncthreads();
     // 2. exclusive scan of the slot populations (PER consecutive slots per thread)
     {
-        static_assert(PER == 4, "one uint4 of slot counters per thread");
+        static_assert(PER % 4 == 0, "whole uint4s of slot counters per thread");
         uint32_t c[PER], sum = 0;
-        const uint4 c4 = reinterpret_cast<const uint4*>(sm.cnt)[t];
-        c[0] = c4.x; c[1] = c4.y; c[2] = c4.z; c[3] = c4.w;
-        sum = c4.x + c4.y + c4.z + c4.w;
+#pragma unroll
+        for (int i = 0; i < PER / 4; ++i) {
+            const uint4 c4 = reinterpret_cast<const uint4*>(sm.cnt)[t * (PER / 4) + i];
+            c[4 * i] = c4.x; c[4 * i + 1] = c4.y; c[4 * i + 2] = c4.z; c[4 * i + 3] = c4.w;
+            sum += c4.x + c4.y + c4.z + c4.w;
+        }
         uint32_t inc = sum;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -336,8 +339,16 @@ __global__ void __launch_bounds__(kBkSortThreads, 4) bucket_sort_kernel(const ui
         uint32_t add = 0;
 #pragma unroll
         for (int w = 0; w < kBkSortThreads / 32; ++w) add += (w < warp) ? sm.wsum[w] : 0u;
-        const uint32_t run = inc - sum + add;
-        reinterpret_cast<uint4*>(sm.cnt)[t] = make_uint4(run, run + c[0], run + c[0] + c[1], run + c[0] + c[1] + c[2]);
+        uint32_t run = inc - sum + add;
+#pragma unroll
+        for (int i = 0; i < PER / 4; ++i) {
+            uint4 o4;
+            o4.x = run; run += c[4 * i];
+            o4.y = run; run += c[4 * i + 1];
+            o4.z = run; run += c[4 * i + 2];
+            o4.w = run; run += c[4 * i + 3];
+            reinterpret_cast<uint4*>(sm.cnt)[t * (PER / 4) + i] = o4;
+        }
     }
     __syncthreads();
     // 3. every pair into its slot's range (any order); cnt[s] ends as the END of slot s
