@@ -159,7 +159,7 @@ constexpr int kMidL1 = 4, kMidL2 = 4, kMidL3 = 5;        // log2 of the stage ra
 constexpr int kMidPadShift = 5;                           // one pad element per 32
 __host__ __device__ constexpr int mid_pad(int a) { return a + (a >> kMidPadShift); }
 constexpr int kMidRowElems = (1 << kLogR1) + (1 << (kLogR1 - kMidPadShift));
-constexpr size_t kMidSmemBytes = 2 * (size_t)kMidRowElems * sizeof(float2);
+constexpr size_t kMidSmemBytes = 2 * (size_t)kMidRowElems * sizeof(float2) + 2 * ((size_t)1 << kLogR1) * sizeof(float);   // rows + their A_norm
 
 template <typename T> struct MidArgs {
     typedef typename Cx<T>::type C;
@@ -198,6 +198,23 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
     zrow[0] = a.Z + b * a.bstride + ((long long)rp[0] << kLogR1);
     zrow[1] = a.Z + b * a.bstride + ((long long)rp[1] << kLogR1);
     if (t < 2) s_wrow[t] = tw_lookup<T>(a.rlv, (uint32_t)k0[t]);
+    // the target amplitudes of the two rows travel to shared memory while the forward row FFTs run
+    T* sA = reinterpret_cast<T*>(smem_raw + 2 * (size_t)kMidRowElems * sizeof(C));
+    {
+        const T* Ab0 = a.Ap + b * (a.bstride + 1);
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            if (r < nrows) {
+                const T* Ar = Ab0 + ((long long)rp[r] << kLogR1);
+#pragma unroll 4
+                for (int p = t; p < R1; p += kMidThreads) {
+                    const unsigned d = (unsigned)__cvta_generic_to_shared(sA + r * R1 + p);
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(d), "l"(Ar + p) : "memory");
+                }
+            }
+        }
+        asm volatile("cp.async.commit_group;\n" ::: "memory");
+    }
     C pw[16];
 
     // ---- forward stage 1: thread j = t owns (d2, d3) = j, butterfly over d1 (stride J1)
@@ -249,6 +266,7 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
 #pragma unroll
         for (int k = 0; k < RAD3; ++k) sr[k] = v[bitrev<RAD3>(k)];
     }
+    asm volatile("cp.async.wait_group 0;\n" ::: "memory");
     __syncthreads();
     // ---- L2: untangle + amplitude replace on the pairs (K, L - K)
     {
@@ -256,8 +274,8 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
         if (pid != 0) {
             // bin k of row A pairs with bin R1-1-k of row B: position p <-> R1-1-p
             const C wrow = s_wrow[0];
-            const T* A1p = Ab + ((long long)rp[0] << kLogR1);
-            const T* A2p = Ab + ((long long)rp[1] << kLogR1);
+            const T* A1p = sA;
+            const T* A2p = sA + R1;
 #pragma unroll 4
             for (int p = t; p < R1; p += kMidThreads) {
                 const int p2 = R1 - 1 - p;
@@ -268,7 +286,7 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
             }
         } else {
             // row 0: bin k pairs with (R1 - k) mod R1 (table sp); k = 0 holds DC and Nyquist
-            const T* A1p = Ab + ((long long)rp[0] << kLogR1);
+            const T* A1p = sA;
             for (int p = t; p < R1; p += kMidThreads) {
                 const int p2 = a.sp[p];
                 if (p2 < p) continue;
@@ -289,7 +307,7 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
             if (nrows == 2) {
                 // row R0/2 pairs with itself: position p <-> R1-1-p
                 const C wrow = s_wrow[1];
-                const T* A2p = Ab + ((long long)rp[1] << kLogR1);
+                const T* A2p = sA + R1;
                 C* sr = s + kMidRowElems;
                 for (int p = t; p < R1 / 2; p += kMidThreads) {
                     const int p2 = R1 - 1 - p;

@@ -232,6 +232,22 @@ __device__ __forceinline__ typename Cx<T>::type replace_amp(typename Cx<T>::type
     if (m > (T)0) { T s = A / m; return mk<T>(X.x * s, X.y * s); }
     return mk<T>(A, (T)0);
 }
+// fp32: 1/|X| from the hardware reciprocal square root plus one Newton step (<= 1 ulp) whenever |X|^2 is a normal
+// number that cannot overflow; the scaled hypot and the IEEE division above only for the rest (they were 45 % of
+// the fused middle kernel's time).
+template <>
+__device__ __forceinline__ float2 replace_amp<float>(float2 X, float A) {
+    const float m2 = fmaf(X.x, X.x, X.y * X.y);
+    if (m2 > 1e-30f && m2 < 1e30f) {
+        float r = rsqrtf(m2);
+        r = r * fmaf(-0.5f * m2, r * r, 1.5f);
+        const float s = A * r;
+        return make_float2(X.x * s, X.y * s);
+    }
+    const float m = hypotf(X.x, X.y);
+    if (m > 0.f) { const float s = A / m; return make_float2(X.x * s, X.y * s); }
+    return make_float2(A, 0.f);
+}
 
 template <typename T>
 __device__ __forceinline__ void replace_pair(typename Cx<T>::type& z1, typename Cx<T>::type& z2,
