@@ -338,6 +338,22 @@ inline size_t sort32_ws_bytes(long long B, long long N) {
     return s;
 }
 
+// Control words of the LSD passes for the curves that take them (gate[b] != 0): digit histograms [B][4][256], tickets
+// [4][B], look-back status [4][B][nchunks][256] (pass stride B * ntiles * 256).  Exits at once for the other curves,
+// which is every curve of a normal run: the bucket sort has already sorted them.
+__global__ void __launch_bounds__(kRadix) lsd_clear_kernel(uint32_t* __restrict__ hist, uint32_t* __restrict__ ticket,
+                                                           uint32_t* __restrict__ status, const uint32_t* __restrict__ gate,
+                                                           uint32_t nchunks, size_t pass_stride, long long B) {
+    const long long b = bidx();
+    if (b >= B || gate[b] == 0u) return;
+    const uint32_t p = blockIdx.x / nchunks, c = blockIdx.x - p * nchunks;
+    status[(size_t)p * pass_stride + ((size_t)b * nchunks + c) * kRadix + threadIdx.x] = 0u;
+    if (c == 0) {
+        hist[((size_t)b * 4 + p) * kRadix + threadIdx.x] = 0u;
+        if (threadIdx.x == 0) ticket[(size_t)p * B + b] = 0u;
+    }
+}
+
 // vals [B][N] -> idx_out [B][N]; optionally the sorted values.  Returns the free pair buffer (for the scatter) in *spare.
 inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* sorted_out, long long B, long long N,
                                  void* ws, uint2** spare, cudaStream_t st, bool reuse_cdf = false) {
@@ -358,12 +374,17 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
         e = bucket32_sort(vals, idx_out, sorted_out, B, N, pa, w + align_up(ctl, 256), &gate, reuse_cdf, st);
         if (e != cudaSuccess) return e;
     }
-    e = cudaMemsetAsync(hist, 0, ctl, st);
-    if (e != cudaSuccess) return e;
+    const size_t nchunks = (ntiles + kS32Chunk - 1) / kS32Chunk;
+    if (gate) {
+        AGN_LAUNCH(K_SORT_HIST, st, (lsd_clear_kernel<<<bgrid((unsigned)(NP * nchunks), B), kRadix, 0, st>>>(
+            hist, ticket, status, gate, (uint32_t)nchunks, (size_t)B * ntiles * kRadix, B)));
+    } else {
+        e = cudaMemsetAsync(hist, 0, ctl, st);
+        if (e != cudaSuccess) return e;
+    }
     const int chunk = 1 << 16;
     AGN_LAUNCH(K_SORT_HIST, st, (digit_hist_kernel<float, 512><<<bgrid((unsigned)((N + chunk - 1) / chunk), B), 512, 0, st>>>(vals, hist, N, N, chunk, B, gate)));
     AGN_LAUNCH(K_SORT_HIST, st, (digit_scan_kernel<<<(unsigned)(B * NP), kRadix, 0, st>>>(hist, gate, NP)));
-    const size_t nchunks = (ntiles + kS32Chunk - 1) / kS32Chunk;
     const dim3 grid = bgrid((unsigned)nchunks, B);
     for (int p = 0; p < NP; ++p) {
         Sweep32Args a;
