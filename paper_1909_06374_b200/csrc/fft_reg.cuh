@@ -16,6 +16,42 @@ template <int N> __host__ __device__ constexpr int bitrev(int k) {
     return r;
 }
 
+// Packed fp32 pair arithmetic of sm_100 (FADD2 / FMUL2 / FFMA2: one issue slot for both halves of a complex number).
+__device__ __forceinline__ unsigned long long pk(float2 a) {
+    unsigned long long u;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(u) : "f"(a.x), "f"(a.y));
+    return u;
+}
+__device__ __forceinline__ float2 unpk(unsigned long long u) {
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(u));
+    return r;
+}
+__device__ __forceinline__ float2 pk_add(float2 a, float2 b) {
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(b)));
+    return unpk(r);
+}
+__device__ __forceinline__ float2 pk_sub(float2 a, float2 b) {
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(b)));
+    return unpk(r);
+}
+__device__ __forceinline__ float2 pk_mul(float2 a, float2 b) {
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(b)));
+    return unpk(r);
+}
+__device__ __forceinline__ float2 pk_fma(float2 a, float2 b, float2 c) {
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pk(a)), "l"(pk(b)), "l"(pk(c)));
+    return unpk(r);
+}
+// d * (c - i s) for a compile-time twiddle: (d.x c + d.y s, d.y c - d.x s) = d * (c, c) + (d.y, d.x) * (s, -s)
+__device__ __forceinline__ float2 pk_twiddle(float2 d, float c, float s) {
+    return pk_fma(make_float2(d.y, d.x), make_float2(s, -s), pk_mul(d, make_float2(c, c)));
+}
+
 template <typename T, int N, int LEN, typename C> struct RegDifLevel {
     static __device__ __forceinline__ void run(C (&v)[N]) {
         constexpr int HALF = LEN / 2;
@@ -25,9 +61,17 @@ template <typename T, int N, int LEN, typename C> struct RegDifLevel {
 #pragma unroll
             for (int j = 0; j < HALF; ++j) {
                 const C a = v[blk + j], b = v[blk + j + HALF];
+                const int tw = j * STEP;
+                if constexpr (sizeof(T) == 4) {
+                    v[blk + j] = pk_add(a, b);
+                    const C d = pk_sub(a, b);
+                    if (tw == 0) v[blk + j + HALF] = d;
+                    else if (tw == 16) v[blk + j + HALF] = cmul_mi(d);
+                    else v[blk + j + HALF] = pk_twiddle(d, (float)cos64(tw), (float)sin64(tw));
+                    continue;
+                }
                 v[blk + j] = cadd(a, b);
                 const C d = csub(a, b);
-                const int tw = j * STEP;
                 C r;
                 if (tw == 0) r = d;
                 else if (tw == 16) r = cmul_mi(d);
