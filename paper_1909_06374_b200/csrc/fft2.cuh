@@ -197,7 +197,7 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
     C* zrow[2];
     zrow[0] = a.Z + b * a.bstride + ((long long)rp[0] << kLogR1);
     zrow[1] = a.Z + b * a.bstride + ((long long)rp[1] << kLogR1);
-    if (t < 2) s_wrow[t] = tw_lookup<T>(a.rlv, (uint32_t)k0[t]);
+    if (t < 2) s_wrow[t] = tw_lookup<T>(a.rlv, (uint32_t)(t == 0 ? k0[0] : k0[1]));      // no dynamic index: k0 stays in registers
     // the target amplitudes of the two rows travel to shared memory while the forward row FFTs run
     T* sA = reinterpret_cast<T*>(smem_raw + 2 * (size_t)kMidRowElems * sizeof(C));
     {

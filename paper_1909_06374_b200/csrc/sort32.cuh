@@ -346,11 +346,13 @@ __global__ void __launch_bounds__(kRadix) lsd_clear_kernel(uint32_t* __restrict_
                                                            uint32_t nchunks, size_t pass_stride, long long B) {
     const long long b = bidx();
     if (b >= B || gate[b] == 0u) return;
-    const uint32_t p = blockIdx.x / nchunks, c = blockIdx.x - p * nchunks;
-    status[(size_t)p * pass_stride + ((size_t)b * nchunks + c) * kRadix + threadIdx.x] = 0u;
-    if (c == 0) {
-        hist[((size_t)b * 4 + p) * kRadix + threadIdx.x] = 0u;
-        if (threadIdx.x == 0) ticket[(size_t)p * B + b] = 0u;
+    for (uint32_t u = blockIdx.x; u < 4u * nchunks; u += gridDim.x) {
+        const uint32_t p = u / nchunks, c = u - p * nchunks;
+        status[(size_t)p * pass_stride + ((size_t)b * nchunks + c) * kRadix + threadIdx.x] = 0u;
+        if (c == 0) {
+            hist[((size_t)b * 4 + p) * kRadix + threadIdx.x] = 0u;
+            if (threadIdx.x == 0) ticket[(size_t)p * B + b] = 0u;
+        }
     }
 }
 
@@ -376,7 +378,7 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
     }
     const size_t nchunks = (ntiles + kS32Chunk - 1) / kS32Chunk;
     if (gate) {
-        AGN_LAUNCH(K_SORT_HIST, st, (lsd_clear_kernel<<<bgrid((unsigned)(NP * nchunks), B), kRadix, 0, st>>>(
+        AGN_LAUNCH(K_SORT_HIST, st, (lsd_clear_kernel<<<bgrid((unsigned)std::min<size_t>(NP * nchunks, 512), B), kRadix, 0, st>>>(
             hist, ticket, status, gate, (uint32_t)nchunks, (size_t)B * ntiles * kRadix, B)));
     } else {
         e = cudaMemsetAsync(hist, 0, ctl, st);
