@@ -58,11 +58,14 @@ __global__ void __launch_bounds__(256) cdf_sample_kernel(const float* __restrict
     const long long b = bidx();
     if (b >= B) return;
     const uint32_t i = blockIdx.x * 256 + threadIdx.x;          // sample number
-    if (i >= (N >> kBkSampleLog)) return;
+    const bool in = i < (N >> kBkSampleLog);
     // the sample of block i of 64 keys sits at a position that varies with i (no fixed phase)
     const uint32_t e = (i << kBkSampleLog) + ((i * 0x9E3779B1u) >> (32 - kBkSampleLog));
-    const uint32_t k = key_of(vals[(size_t)b * N + e]);
-    atomicAdd(&hist[(size_t)b * kBkBins + (k >> (32 - kBkBinLog))], 1u);
+    const uint32_t bin = in ? (key_of(vals[(size_t)b * N + e]) >> (32 - kBkBinLog)) : 0xffffffffu;
+    // neighbouring samples of a smooth series share their bin: one atomic per distinct bin and warp
+    const uint32_t peers = __match_any_sync(0xffffffffu, bin);
+    if (in && (threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1))
+        atomicAdd(&hist[(size_t)b * kBkBins + bin], (uint32_t)__popc(peers));
 }
 
 // one CTA (1024 threads) per curve: tab[bin] = (exclusive cumulative weight << 7, weight), weight = (cnt << logK) + 1
@@ -72,9 +75,11 @@ __global__ void __launch_bounds__(1024) cdf_table_kernel(const uint32_t* __restr
     uint2* t = tab + (size_t)blockIdx.x * kBkBins;
     constexpr int PER = kBkBins / 1024;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t c[PER], sum = 0;
-#pragma unroll
-    for (int i = 0; i < PER; ++i) { c[i] = (h[threadIdx.x * PER + i] << logK) + 1u; sum += c[i]; }
+    // two sweeps over the thread's PER bins (whole uint4s; the second one hits L1): no per-bin register array
+    const uint4* h4 = reinterpret_cast<const uint4*>(h + threadIdx.x * PER);
+    uint32_t sum = PER;
+#pragma unroll 4
+    for (int i = 0; i < PER / 4; ++i) { const uint4 v = h4[i]; sum += (v.x + v.y + v.z + v.w) << logK; }
     uint32_t inc = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -94,8 +99,16 @@ __global__ void __launch_bounds__(1024) cdf_table_kernel(const uint32_t* __restr
     }
     __syncthreads();
     uint32_t run = inc - sum + ws[warp];
-#pragma unroll
-    for (int i = 0; i < PER; ++i) { t[threadIdx.x * PER + i] = make_uint2(run << 7, c[i]); run += c[i]; }
+    uint4* t4 = reinterpret_cast<uint4*>(t + threadIdx.x * PER);
+#pragma unroll 4
+    for (int i = 0; i < PER / 4; ++i) {
+        const uint4 v = h4[i];
+        const uint32_t w0 = (v.x << logK) + 1u, w1 = (v.y << logK) + 1u, w2 = (v.z << logK) + 1u, w3 = (v.w << logK) + 1u;
+        t4[2 * i] = make_uint4(run << 7, w0, (run + w0) << 7, w1);
+        run += w0 + w1;
+        t4[2 * i + 1] = make_uint4(run << 7, w2, (run + w2) << 7, w3);
+        run += w2 + w3;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
