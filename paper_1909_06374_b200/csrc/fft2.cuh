@@ -185,11 +185,50 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
     C* s = reinterpret_cast<C*>(smem_raw);
     __shared__ C s_wrow[2];
     const int t = threadIdx.x;
-    const long long b = bidx();
-    if (b >= a.B) return;
     const int R0 = 1 << a.logR0;
-    const int pid = blockIdx.x;                   // 0: rows 0 and R0/2 (self-paired); else rows pid, R0 - pid
     const int nrows = (R0 == 1) ? 1 : 2;
+    const int gx = (R0 == 1) ? 1 : (R0 >> 1);
+    const long long total = (long long)a.B * gx;
+    T* sA = reinterpret_cast<T*>(smem_raw + 2 * (size_t)kMidRowElems * sizeof(C));
+    // Persistent CTA (one per SM: 196 KB of shared memory): work item = (curve b, row pair pid).  The rows and the
+    // target amplitudes of the NEXT item are fetched with cp.async while the current one is still being finished:
+    // the amplitudes after the replace step has released sA, each row right after this thread has read its own 16
+    // elements of it in inverse stage 1 (stage 1 touches thread-private positions only, forward and inverse).
+    auto row_pos = [&](int pid, int r) -> int {
+        const int k = (r == 0) ? pid : ((pid == 0) ? (R0 >> 1) : (R0 - pid));
+        return (R0 == 1) ? 0 : (int)k2pos(a.dcol, (uint32_t)k);
+    };
+    auto fetch_row = [&](long long bb, int rp_, int r) {
+        const C* z = a.Z + bb * a.bstride + ((long long)rp_ << kLogR1);
+#pragma unroll
+        for (int i = 0; i < RAD1; ++i) {
+            const unsigned d = (unsigned)__cvta_generic_to_shared(s + r * kMidRowElems + mid_pad(i * J1 + t));
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(z + i * J1 + t) : "memory");
+        }
+    };
+    auto fetch_amp = [&](long long bb, int rp_, int r) {
+        const T* Ar = a.Ap + bb * (a.bstride + 1) + ((long long)rp_ << kLogR1);
+#pragma unroll 4
+        for (int p = t; p < R1; p += kMidThreads) {
+            const unsigned d = (unsigned)__cvta_generic_to_shared(sA + r * R1 + p);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(d), "l"(Ar + p) : "memory");
+        }
+    };
+    long long work = blockIdx.x;
+    if (work >= total) return;
+    {
+        const long long b0 = work / gx;
+        const int pid0 = (int)(work - b0 * gx);
+        for (int r = 0; r < nrows; ++r) { const int q = row_pos(pid0, r); fetch_row(b0, q, r); fetch_amp(b0, q, r); }
+        asm volatile("cp.async.commit_group;\n" ::: "memory");
+    }
+    for (; work < total; work += gridDim.x) {
+    const long long b = work / gx;
+    const int pid = (int)(work - b * gx);         // 0: rows 0 and R0/2 (self-paired); else rows pid, R0 - pid
+    const long long work_n = work + gridDim.x;
+    const bool has_next = work_n < total;
+    const long long b_n = has_next ? work_n / gx : 0;
+    const int pid_n = has_next ? (int)(work_n - b_n * gx) : 0;
     int k0[2], rp[2];
     k0[0] = pid; k0[1] = (pid == 0) ? (R0 >> 1) : (R0 - pid);
     rp[0] = (int)k2pos(a.dcol, (uint32_t)k0[0]);
@@ -198,23 +237,7 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
     zrow[0] = a.Z + b * a.bstride + ((long long)rp[0] << kLogR1);
     zrow[1] = a.Z + b * a.bstride + ((long long)rp[1] << kLogR1);
     if (t < 2) s_wrow[t] = tw_lookup<T>(a.rlv, (uint32_t)(t == 0 ? k0[0] : k0[1]));      // no dynamic index: k0 stays in registers
-    // the target amplitudes of the two rows travel to shared memory while the forward row FFTs run
-    T* sA = reinterpret_cast<T*>(smem_raw + 2 * (size_t)kMidRowElems * sizeof(C));
-    {
-        const T* Ab0 = a.Ap + b * (a.bstride + 1);
-#pragma unroll
-        for (int r = 0; r < 2; ++r) {
-            if (r < nrows) {
-                const T* Ar = Ab0 + ((long long)rp[r] << kLogR1);
-#pragma unroll 4
-                for (int p = t; p < R1; p += kMidThreads) {
-                    const unsigned d = (unsigned)__cvta_generic_to_shared(sA + r * R1 + p);
-                    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(d), "l"(Ar + p) : "memory");
-                }
-            }
-        }
-        asm volatile("cp.async.commit_group;\n" ::: "memory");
-    }
+    asm volatile("cp.async.wait_group 0;\n" ::: "memory");      // this item's rows and amplitudes have landed
     C pw[16];
 
     // ---- forward stage 1: thread j = t owns (d2, d3) = j, butterfly over d1 (stride J1)
@@ -224,7 +247,7 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
         if (r < nrows) {
             C v[RAD1];
 #pragma unroll
-            for (int i = 0; i < RAD1; ++i) v[i] = __ldcs(zrow[r] + i * J1 + t);
+            for (int i = 0; i < RAD1; ++i) v[i] = s[r * kMidRowElems + mid_pad(i * J1 + t)];
             fft_reg_dif<T, RAD1, C>(v);
 #pragma unroll
             for (int k = 0; k < RAD1; ++k) {
@@ -266,7 +289,6 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
 #pragma unroll
         for (int k = 0; k < RAD3; ++k) sr[k] = v[bitrev<RAD3>(k)];
     }
-    asm volatile("cp.async.wait_group 0;\n" ::: "memory");
     __syncthreads();
     // ---- L2: untangle + amplitude replace on the pairs (K, L - K)
     {
@@ -320,6 +342,9 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
         }
     }
     __syncthreads();
+    if (has_next) {
+        for (int r = 0; r < nrows; ++r) fetch_amp(b_n, row_pos(pid_n, r), r);        // sA is free now
+    }
     // ---- inverse stage 3
     if (r3 < nrows) {
         C v[RAD3];
@@ -361,11 +386,14 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
                 if (k > 0) x = cmulc(x, pw[k]);
                 v[k] = cswap(x);
             }
+            if (has_next) fetch_row(b_n, row_pos(pid_n, r), r);     // this thread's 16 positions of row r are free now
             fft_reg_dif<T, RAD1, C>(v);
 #pragma unroll
             for (int n = 0; n < RAD1; ++n) zrow[r][n * J1 + t] = cswap(v[bitrev<RAD1>(n)]);
         }
     }
+    asm volatile("cp.async.commit_group;\n" ::: "memory");
+    }   // work loop
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -522,7 +550,10 @@ inline cudaError_t fft2_mid(const Fft2Plan<T>& p, typename Cx<T>::type* Z, const
     m.twpos = p.twpos; m.sp = p.sp; m.tw14 = p.tw14;
     m.rlv.tw14 = p.tw14; m.rlv.lo = p.lo_real; m.rlv.logD = p.logL + 1;
     const unsigned gx = p.logR0 == 0 ? 1u : (1u << (p.logR0 - 1));
-    AGN_LAUNCH(K_FFT_MID, st, (fft_mid_kernel<T><<<bgrid(gx, B), kMidThreads, kMidSmemBytes, st>>>(m)));
+    static int sms = 0;
+    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+    const unsigned grid = (unsigned)std::min<long long>((long long)gx * B, sms);
+    AGN_LAUNCH(K_FFT_MID, st, (fft_mid_kernel<T><<<grid, kMidThreads, kMidSmemBytes, st>>>(m)));
     return cudaGetLastError();
 }
 
