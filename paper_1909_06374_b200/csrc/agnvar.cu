@@ -72,7 +72,7 @@ template <typename T> size_t ws_e13(int64_t B, int64_t N) {
     c.take<C>(std::max(FftPlan<T>::table_elems(), Fft2Plan<T>::table_elems()));
     c.take<unsigned int>(Fft2Plan<T>::counter_words(B));
     c.take<T>((size_t)B * N);                 // Z / x_adj
-    c.take<T>((size_t)B * (N / 2 + 1));       // A_norm in position order
+    c.take<T>((size_t)B * (N / 2 + kApPad));  // A_norm in position order
     c.take<uint32_t>((size_t)B * N);          // permutation ping-pong
     c.take<unsigned long long>((size_t)B);    // changed counters
     c.take<int>((size_t)B);                   // first_zero
@@ -135,7 +135,7 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
     C* tables = c.take<C>(std::max(FftPlan<T>::table_elems(), Fft2Plan<T>::table_elems()));
     unsigned int* counters = c.take<unsigned int>(Fft2Plan<T>::counter_words(B));
     T* Z = c.take<T>((size_t)B * N);
-    T* Ap = c.take<T>((size_t)B * (N / 2 + 1));
+    T* Ap = c.take<T>((size_t)B * (N / 2 + kApPad));
     uint32_t* P1 = c.take<uint32_t>((size_t)B * N);
     unsigned long long* changed = c.take<unsigned long long>((size_t)B);
     int* first_zero = c.take<int>((size_t)B);

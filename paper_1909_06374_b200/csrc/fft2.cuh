@@ -207,11 +207,12 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
         }
     };
     auto fetch_amp = [&](long long bb, int rp_, int r) {
-        const T* Ar = a.Ap + bb * (a.bstride + 1) + ((long long)rp_ << kLogR1);
-#pragma unroll 4
-        for (int p = t; p < R1; p += kMidThreads) {
+        const T* Ar = a.Ap + bb * (a.bstride + kApPad) + ((long long)rp_ << kLogR1);
+        static_assert(sizeof(T) == 4, "16-byte copies of four fp32 amplitudes");
+#pragma unroll
+        for (int p = 4 * t; p < R1; p += 4 * kMidThreads) {
             const unsigned d = (unsigned)__cvta_generic_to_shared(sA + r * R1 + p);
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(d), "l"(Ar + p) : "memory");
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(Ar + p) : "memory");
         }
     };
     long long work = blockIdx.x;
@@ -292,7 +293,7 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
     __syncthreads();
     // ---- L2: untangle + amplitude replace on the pairs (K, L - K)
     {
-        const T* Ab = a.Ap + b * (a.bstride + 1);
+        const T* Ab = a.Ap + b * (a.bstride + kApPad);
         if (pid != 0) {
             // bin k of row A pairs with bin R1-1-k of row B: position p <-> R1-1-p
             const C wrow = s_wrow[0];

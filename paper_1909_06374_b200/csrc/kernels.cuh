@@ -214,14 +214,16 @@ __global__ void untangle_out_kernel(const typename Cx<T>::type* __restrict__ Z, 
     }
 }
 
-// A_norm natural order [B][L+1] -> position order [B][L+1] (entry L stays at L)
+// A_norm natural order [B][L+1] -> position order [B][L+kApPad] (entry L stays at L); the padded curve stride keeps
+// every row of 2^13 amplitudes 16-byte aligned for the asynchronous copies of the fused middle kernel
+constexpr int kApPad = 4;
 template <typename T>
 __global__ void perm_anorm_kernel(const T* __restrict__ A, T* __restrict__ Ap, Digits dg, int B) {
     const long long L = 1ll << dg.logL;
     long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long b = bidx();
     if (p > L || b >= B) return;
-    Ap[b * (L + 1) + p] = (p == L) ? A[b * (L + 1) + L] : A[b * (L + 1) + pos2k(dg, (uint32_t)p)];
+    Ap[b * (L + kApPad) + p] = (p == L) ? A[b * (L + 1) + L] : A[b * (L + 1) + pos2k(dg, (uint32_t)p)];
 }
 
 // L2 amplitude replace (O6 step 2) in position order, in place:
@@ -274,7 +276,7 @@ __global__ void replace_kernel(typename Cx<T>::type* __restrict__ Z, const T* __
     const uint32_t k = pos2k(dg, (uint32_t)p);
     if (2ll * k > L) return;
     C* z = Z + b * L;
-    const T* A = Ap + b * (L + 1);
+    const T* A = Ap + b * (L + kApPad);
     if (k == 0) {
         C z0 = z[0];
         T x0 = z0.x + z0.y, xl = z0.x - z0.y;
