@@ -418,7 +418,7 @@ inline cudaError_t rank_scatter_two_level32(const uint32_t* idx_new, const uint3
     a.vals = sorted; a.idx_new = idx_new; a.idx_old = idx_old; a.changed = changed;
     a.out = pairs; a.cursor = cursor; a.N = (uint32_t)N; a.lb = (uint32_t)shift; a.nc = kRadix; a.nb = kRadix;
     a.cap_out = (uint32_t)(N >> kRadixBits); a.B = B;
-    AGN_LAUNCH(K_SCATTER_BIN, st, (bucket_part_kernel<2><<<bgrid((unsigned)(N / kBkPartTile), B), kBkPartThreads, sizeof(PartSmem), st>>>(a)));
+    AGN_LAUNCH(K_SCATTER_BIN, st, (bucket_part_kernel<2><<<bgrid((unsigned)(N / bk_part_tile(2)), B), kBkPartThreads, sizeof(PartSmem<2>), st>>>(a)));
     AGN_LAUNCH(K_SCATTER_PLACE, st, (scatter_place32_kernel<<<bgrid((unsigned)(N / 2048), B), 256, 0, st>>>(
         (const uint4*)pairs, x, (uint32_t)N, cursor, B)));
     return cudaGetLastError();
