@@ -68,46 +68,59 @@ __global__ void __launch_bounds__(256) cdf_sample_kernel(const float* __restrict
         atomicAdd(&hist[(size_t)b * kBkBins + bin], (uint32_t)__popc(peers));
 }
 
-// one CTA (1024 threads) per curve: tab[bin] = (exclusive cumulative weight << 7, weight), weight = (cnt << logK) + 1
-__global__ void __launch_bounds__(1024) cdf_table_kernel(const uint32_t* __restrict__ hist, uint2* __restrict__ tab, int logK) {
-    __shared__ uint32_t ws[32];
-    const uint32_t* h = hist + (size_t)blockIdx.x * kBkBins;
-    uint2* t = tab + (size_t)blockIdx.x * kBkBins;
-    constexpr int PER = kBkBins / 1024;
+// tab[bin] = (exclusive cumulative weight << 7, weight), weight = (cnt << logK) + 1.  kCdfChunks CTAs per curve, each
+// owning 65536 / kCdfChunks consecutive bins: a CTA first adds up the weights of all bins before its chunk (the
+// histogram is L2-resident, the reads are coalesced), then scans its own chunk 1024 bins at a time.  No CTA waits for
+// another one.
+constexpr int kCdfChunks = 16;
+__device__ __forceinline__ uint32_t block_sum_1024(uint32_t v, uint32_t* ws) {      // sum over the CTA, returned to all
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // two sweeps over the thread's PER bins (whole uint4s; the second one hits L1): no per-bin register array
-    const uint4* h4 = reinterpret_cast<const uint4*>(h + threadIdx.x * PER);
-    uint32_t sum = PER;
-#pragma unroll 4
-    for (int i = 0; i < PER / 4; ++i) { const uint4 v = h4[i]; sum += (v.x + v.y + v.z + v.w) << logK; }
-    uint32_t inc = sum;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __syncthreads();
+    if (lane == 0) ws[warp] = v;
+    __syncthreads();
+    uint32_t t = ws[lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    return t;
+}
+// exclusive scan over the CTA's 1024 values; *total receives the sum
+__device__ __forceinline__ uint32_t block_excl_scan_1024(uint32_t v, uint32_t* ws, uint32_t* total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t inc = v;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const uint32_t n = __shfl_up_sync(0xffffffffu, inc, o);
         if (lane >= o) inc += n;
     }
+    __syncthreads();
     if (lane == 31) ws[warp] = inc;
     __syncthreads();
-    if (warp == 0) {
-        uint32_t v = ws[lane], w = v;
+    uint32_t w = ws[lane], wi = w;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t n = __shfl_up_sync(0xffffffffu, w, o);
-            if (lane >= o) w += n;
-        }
-        ws[lane] = w - v;
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t n = __shfl_up_sync(0xffffffffu, wi, o);
+        if (lane >= o) wi += n;
     }
-    __syncthreads();
-    uint32_t run = inc - sum + ws[warp];
-    uint4* t4 = reinterpret_cast<uint4*>(t + threadIdx.x * PER);
-#pragma unroll 4
-    for (int i = 0; i < PER / 4; ++i) {
-        const uint4 v = h4[i];
-        const uint32_t w0 = (v.x << logK) + 1u, w1 = (v.y << logK) + 1u, w2 = (v.z << logK) + 1u, w3 = (v.w << logK) + 1u;
-        t4[2 * i] = make_uint4(run << 7, w0, (run + w0) << 7, w1);
-        run += w0 + w1;
-        t4[2 * i + 1] = make_uint4(run << 7, w2, (run + w2) << 7, w3);
-        run += w2 + w3;
+    *total = __shfl_sync(0xffffffffu, wi, 31);
+    return inc - v + __shfl_sync(0xffffffffu, wi - w, warp);
+}
+__global__ void __launch_bounds__(1024) cdf_table_kernel(const uint32_t* __restrict__ hist, uint2* __restrict__ tab, int logK) {
+    __shared__ uint32_t ws[32];
+    const uint32_t curve = blockIdx.x / kCdfChunks, chunk = blockIdx.x % kCdfChunks;
+    const uint32_t* h = hist + (size_t)curve * kBkBins;
+    uint2* t = tab + (size_t)curve * kBkBins;
+    constexpr uint32_t PER = kBkBins / kCdfChunks;          // bins per chunk
+    uint32_t before = 0;
+    for (uint32_t i = threadIdx.x; i < chunk * PER; i += 1024) before += (h[i] << logK) + 1u;
+    uint32_t run = block_sum_1024(before, ws);
+    for (uint32_t i0 = chunk * PER; i0 < (chunk + 1) * PER; i0 += 1024) {
+        const uint32_t w = (h[i0 + threadIdx.x] << logK) + 1u;
+        uint32_t total;
+        const uint32_t ex = block_excl_scan_1024(w, ws, &total);
+        t[i0 + threadIdx.x] = make_uint2((run + ex) << 7, w);
+        run += total;
     }
 }
 
@@ -265,33 +278,25 @@ __global__ void __launch_bounds__(kBkPartThreads, (LEVEL == 2 ? 4 : 6)) bucket_p
     }
 }
 
-// one CTA (1024 threads) per curve: base[k] = sum of the populations of buckets < k (populations clamped to the slab)
+// base[k] = sum of the populations of buckets < k (populations clamped to the slab).  `chunks` CTAs per curve, same
+// scheme as cdf_table_kernel: sum of everything before the chunk, then a scan of the chunk.
 __global__ void __launch_bounds__(1024) bucket_base_kernel(const uint32_t* __restrict__ cursor, uint32_t* __restrict__ base,
-                                                           uint32_t nb) {
+                                                           uint32_t nb, uint32_t chunks) {
     __shared__ uint32_t ws[32];
-    __shared__ uint32_t carry;
-    const uint32_t* c = cursor + (size_t)blockIdx.x * nb;
-    uint32_t* o = base + (size_t)blockIdx.x * nb;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry = 0u;
-    __syncthreads();
-    for (uint32_t k0 = 0; k0 < nb; k0 += 1024) {
+    const uint32_t curve = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
+    const uint32_t* c = cursor + (size_t)curve * nb;
+    uint32_t* o = base + (size_t)curve * nb;
+    const uint32_t per = nb / chunks;
+    uint32_t before = 0;
+    for (uint32_t i = threadIdx.x; i < chunk * per; i += 1024) before += min(c[i], (uint32_t)kBkCap);
+    uint32_t run = block_sum_1024(before, ws);
+    for (uint32_t k0 = chunk * per; k0 < (chunk + 1) * per; k0 += 1024) {
         const uint32_t k = k0 + threadIdx.x;
-        const uint32_t n = (k < nb) ? min(c[k], (uint32_t)kBkCap) : 0u;
-        uint32_t inc = n;
-#pragma unroll
-        for (int s = 1; s < 32; s <<= 1) {
-            const uint32_t m = __shfl_up_sync(0xffffffffu, inc, s);
-            if (lane >= s) inc += m;
-        }
-        if (lane == 31) ws[warp] = inc;
-        __syncthreads();
-        uint32_t add = carry;
-        for (int w = 0; w < warp; ++w) add += ws[w];
-        if (k < nb) o[k] = inc - n + add;
-        __syncthreads();
-        if (threadIdx.x == 1023) carry = inc + add;
-        __syncthreads();
+        const uint32_t n = (k < (chunk + 1) * per) ? min(c[k], (uint32_t)kBkCap) : 0u;
+        uint32_t total;
+        const uint32_t ex = block_excl_scan_1024(n, ws, &total);
+        if (k < (chunk + 1) * per) o[k] = run + ex;
+        run += total;
     }
 }
 
@@ -475,7 +480,7 @@ inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* so
         if (e != cudaSuccess) return e;
         const uint32_t nsamp = (uint32_t)(N >> kBkSampleLog);
         AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B)));
-        AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)B, 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
+        AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)(B * kCdfChunks), 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
     }
     PartArgs a;
     a.vals = vals; a.in = slabs1; a.in_count = cursor1; a.overflow = overflow; a.tab = tab;
@@ -484,7 +489,8 @@ inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* so
     AGN_LAUNCH(K_SORT_PART, st, (bucket_part_kernel<0><<<bgrid((unsigned)(N / bk_part_tile(0)), B), kBkPartThreads, sizeof(PartSmem<0>), st>>>(a)));
     a.out = slabs2; a.cursor = cursor2; a.cap_out = kBkCap;
     AGN_LAUNCH(K_SORT_PART, st, (bucket_part_kernel<1><<<bgrid(g.tiles1 * g.nc, B), kBkPartThreads, sizeof(PartSmem<1>), st>>>(a)));
-    AGN_LAUNCH(K_SORT_CDF, st, (bucket_base_kernel<<<(unsigned)B, 1024, 0, st>>>(cursor2, base, g.nb)));
+    const uint32_t bchunks = g.nb >= 16384 ? 16u : (g.nb >= 1024 ? g.nb / 1024 : 1u);
+    AGN_LAUNCH(K_SORT_CDF, st, (bucket_base_kernel<<<(unsigned)(B * bchunks), 1024, 0, st>>>(cursor2, base, g.nb, bchunks)));
     AGN_LAUNCH(K_SORT_BUCKET, st, (bucket_sort_kernel<<<bgrid(g.nb, B), kBkSortThreads, sizeof(BkSmem), st>>>(
         slabs2, cursor2, base, overflow, tab, idx_out, sorted_out, (uint32_t)N, g.nb, a.M, B)));
     *overflow_out = overflow;
