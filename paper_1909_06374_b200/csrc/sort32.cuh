@@ -163,10 +163,15 @@ __global__ void __launch_bounds__(kS32Threads, 4) sweep32_kernel(Sweep32Args a) 
     const long long b = bidx();
     if (b >= a.B) return;
     if (a.gate && a.gate[b] == 0u) return;
+    // persistent: a CTA takes chunk tickets until none is left (a gated-off launch then costs a few hundred CTAs, not
+    // one per chunk); a CTA only ever waits for chunks with smaller tickets, which are held by running CTAs
+    for (;;) {
+    __syncthreads();
     if (threadIdx.x == 0) sm.tile = atomicAdd(&a.ticket[b], 1u);
     sm.hist[threadIdx.x] = 0u;
     __syncthreads();
     const uint32_t chunk = sm.tile;
+    if (chunk >= a.nchunks) break;
     const uint32_t tiles_here = min((uint32_t)kS32Chunk, a.ntiles - chunk * kS32Chunk);
     const size_t seg = (size_t)b * a.N;
     const uint32_t e00 = chunk * (kS32Chunk * kS32Tile) + s32_elem0();
@@ -240,6 +245,7 @@ __global__ void __launch_bounds__(kS32Threads, 4) sweep32_kernel(Sweep32Args a) 
         }
         __syncthreads();      // stage and goff are rewritten by the next tile
     }
+    }   // ticket loop
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -387,7 +393,7 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
     const int chunk = 1 << 16;
     AGN_LAUNCH(K_SORT_HIST, st, (digit_hist_kernel<float, 512><<<bgrid((unsigned)((N + chunk - 1) / chunk), B), 512, 0, st>>>(vals, hist, N, N, chunk, B, gate)));
     AGN_LAUNCH(K_SORT_HIST, st, (digit_scan_kernel<<<(unsigned)(B * NP), kRadix, 0, st>>>(hist, gate, NP)));
-    const dim3 grid = bgrid((unsigned)nchunks, B);
+    const dim3 grid = bgrid((unsigned)std::min<size_t>(nchunks, 592), B);
     for (int p = 0; p < NP; ++p) {
         Sweep32Args a;
         a.vals = vals;
