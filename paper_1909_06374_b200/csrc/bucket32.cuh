@@ -35,7 +35,6 @@ constexpr int kBkBins = 1 << kBkBinLog;
 constexpr int kBkSortThreads = 512;
 constexpr int kBkSlotLog = 11;
 constexpr int kBkSlots = 1 << kBkSlotLog;         // interpolation slots of the in-CTA sort
-constexpr int kBkEpt = kBkCap / kBkSortThreads;   // 16 elements per thread
 
 // Position of a key on the smoothed CDF: bin weights w = cnt * K + 1 (K = 2^24 / samples, so that the sampled mass is
 // 2^24 and the add-one mass 2^16 whatever N is: keys of an unsampled bin still spread linearly over their own

@@ -249,54 +249,8 @@ __global__ void __launch_bounds__(kS32Threads, 4) sweep32_kernel(Sweep32Args a) 
 }
 
 // ------------------------------------------------------------------------------------------------
-// L5 two-level: bin (value, dst) pairs by the top 8 bits of dst, then place
+// L5 two-level: place step (the bin step is bucket_part_kernel<2> of bucket32.cuh)
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kS32Threads, 4) scatter_bin32_kernel(const uint32_t* __restrict__ idx_new,
-                                                                       const uint32_t* __restrict__ idx_old,
-                                                                       const float* __restrict__ sorted,
-                                                                       uint2* __restrict__ pairs, uint32_t N, int shift,
-                                                                       uint32_t* __restrict__ cursor,
-                                                                       unsigned long long* __restrict__ changed,
-                                                                       long long B) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    S32Smem& sm = *reinterpret_cast<S32Smem*>(smem_raw);
-    const long long b = bidx();
-    if (b >= B) return;
-    const uint32_t base = blockIdx.x * kS32Tile;
-    const size_t seg = (size_t)b * N;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    uint2 kv[kS32Kpt];                  // x = value bits, y = dst
-    uint32_t dig[kS32Kpt], pos[kS32Kpt];
-    const size_t e0 = seg + base + s32_elem0();
-    unsigned int diff = 0;
-    if (threadIdx.x == 0) sm.diff = 0u;
-#pragma unroll
-    for (int j = 0; j < kS32Kpt; ++j) {
-        const uint32_t dst = __ldcs(idx_new + e0 + j * kS32ItemStride);
-        diff += (dst != __ldcs(idx_old + e0 + j * kS32ItemStride));
-        kv[j] = make_uint2(__float_as_uint(__ldcs(sorted + e0 + j * kS32ItemStride)), dst);
-        dig[j] = (dst >> shift) & (kRadix - 1);
-    }
-    const uint32_t cnt = s32_rank(dig, pos, sm);
-    {
-        const int d = threadIdx.x;
-        const uint32_t start = cnt ? atomicAdd(&cursor[b * kRadix + d], cnt) : 0u;
-        sm.goff[d] = ((uint32_t)d << shift) + start - sm.tile_off[d];
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) diff += __shfl_xor_sync(0xffffffffu, diff, o);
-    if (lane == 0 && diff) atomicAdd(&sm.diff, diff);        // sm.diff was zeroed before the barriers of s32_rank
-#pragma unroll
-    for (int j = 0; j < kS32Kpt; ++j) sm.stage[pos[j]] = kv[j];
-    __syncthreads();
-    if (threadIdx.x == 0 && sm.diff) atomicAdd(&changed[b], (unsigned long long)sm.diff);
-#pragma unroll 4
-    for (int s = threadIdx.x; s < kS32Tile; s += kS32Threads) {
-        const uint2 p = sm.stage[s];
-        pairs[seg + sm.goff[(p.y >> shift) & (kRadix - 1)] + (uint32_t)s] = p;
-    }
-}
-
 __global__ void __launch_bounds__(256) scatter_place32_kernel(const uint4* __restrict__ pairs2, float* __restrict__ x,
                                                               uint32_t N, uint32_t* __restrict__ cursor, long long B) {
     const long long b = bidx();
@@ -321,11 +275,9 @@ inline cudaError_t sort32_set_attrs() {
     cudaError_t e = cudaFuncSetAttribute(sweep32_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep32_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep32_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(scatter_bin32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sm);
     cudaFuncSetAttribute(sweep32_kernel<0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     cudaFuncSetAttribute(sweep32_kernel<1>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     cudaFuncSetAttribute(sweep32_kernel<2>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    cudaFuncSetAttribute(scatter_bin32_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e == cudaSuccess) e = bucket32_set_attrs();
     return e;
 }
