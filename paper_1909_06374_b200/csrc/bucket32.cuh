@@ -208,8 +208,7 @@ __global__ void __launch_bounds__(kBkPartThreads, (LEVEL == 2 ? 4 : 6)) bucket_p
             if (e0 + j * kBkPartThreads < n_in) kv[j] = __ldcs(v + e0 + j * kBkPartThreads);
     }
     __syncthreads();
-    // digit and arrival number inside the digit: lanes that share lane 0's digit (the common case for a smooth
-    // series) are counted with one atomic, the others with one each
+    // digit and arrival number inside the digit
     uint32_t dr[kBkPartEpt];            // digit << 16 | arrival number
     const uint32_t dmask = (LEVEL == 0) ? 0xffffffffu : ((1u << a.lb) - 1u);
     const uint32_t dshift = kBkSlotLog + ((LEVEL == 0) ? a.lb : 0u);
@@ -217,14 +216,17 @@ __global__ void __launch_bounds__(kBkPartThreads, (LEVEL == 2 ? 4 : 6)) bucket_p
     for (int j = 0; j < kBkPartEpt; ++j) {
         const bool valid = (LEVEL != 1) || (e0 + j * kBkPartThreads < n_in);
         const uint32_t d = (LEVEL == 2) ? (kv[j].y >> a.lb) : (valid ? ((bs_of(kv[j].x, tab, a.M) >> dshift) & dmask) : 0xffffu);
-        const uint32_t d0 = __shfl_sync(0xffffffffu, d, 0);
-        const uint32_t same = __ballot_sync(0xffffffffu, d == d0);
         uint32_t r = 0;
-        if (d0 != 0xffffu) {
+        if (LEVEL == 0) {
+            // coarse digits of neighbouring samples of a smooth series mostly agree: one atomic for lane 0's group
+            const uint32_t d0 = __shfl_sync(0xffffffffu, d, 0);
+            const uint32_t same = __ballot_sync(0xffffffffu, d == d0);
             if (lane == 0) r = atomicAdd(&sm.cnt[d0], (uint32_t)__popc(same));
             r = __shfl_sync(0xffffffffu, r, 0) + __popc(same & ((1u << lane) - 1u));
+            if (d != d0) r = atomicAdd(&sm.cnt[d], 1u);
+        } else if (valid) {
+            r = atomicAdd(&sm.cnt[d], 1u);          // fine digits / destination windows are as good as random
         }
-        if (valid && d != d0) r = atomicAdd(&sm.cnt[d], 1u);
         dr[j] = (d << 16) | r;
     }
     __syncthreads();
