@@ -11,8 +11,10 @@
 //                        A tile counts its keys per digit in shared memory, reserves one range per (tile, digit) with
 //                        one global atomic, orders the tile by digit in shared memory and writes coalesced runs.
 //   bucket_base_kernel   exclusive scan of the bucket populations -> first rank of every bucket
-//   bucket_sort_kernel   one CTA per bucket: counting sort into 2048 interpolation slots (the next 11 bits of bs_of),
-//                        then the exact rank of every pair among its few slot mates; indices written at their ranks.
+//   bucket_bounds_kernel smallest key of every bucket (inverse of bs_of at the bucket boundaries)
+//   bucket_sort_kernel   one CTA per bucket: counting sort into 2048 interpolation slots (a linear map of the key
+//                        onto the bucket's key interval), then the exact rank of every pair among its few slot
+//                        mates; indices written at their ranks.
 //
 // HBM bytes per sample: 0.5 (sample) + 12 (<0>: 4 in, 8 out) + 16 (<1>) + 12 (finish: 8 in, 4 out).
 // Order inside a slab is arbitrary (atomic cursors), so the final order is defined by the comparison of the 64-bit
@@ -301,6 +303,31 @@ __global__ void __launch_bounds__(1024) bucket_base_kernel(const uint32_t* __res
     }
 }
 
+// klo[k] = smallest key that bs_of() sends to bucket k (k = 0 .. nb; klo[nb] = 2^32 - 1): the bucket's keys lie in
+// [klo[k], klo[k+1]), so inside the finish kernel a slot is a plain linear map of the key onto that interval -- no
+// table look-up per key there.  One thread per bucket: invert umulhi(pos, M) >= k << kBkSlotLog, then the table.
+__global__ void __launch_bounds__(256) bucket_bounds_kernel(const uint2* __restrict__ tabs, uint32_t* __restrict__ klo,
+                                                            uint32_t nb, uint32_t M, long long B) {
+    const long long b = bidx();
+    if (b >= B) return;
+    const uint32_t k = blockIdx.x * 256 + threadIdx.x;
+    if (k > nb) return;
+    uint32_t* out = klo + (size_t)b * (nb + 1);
+    if (k == nb) { out[k] = 0xffffffffu; return; }
+    const uint2* tab = tabs + (size_t)b * kBkBins;
+    const unsigned long long want = ((unsigned long long)k << kBkSlotLog) << 32;
+    const unsigned long long P = (want + M - 1) / M;               // smallest pos32 with umulhi(pos32, M) >= k << slotlog
+    uint32_t lo = 0, hi = kBkBins - 1;                              // largest bin with tab[bin].x <= P
+    while (lo < hi) {
+        const uint32_t mid = (lo + hi + 1) >> 1;
+        if ((unsigned long long)tab[mid].x <= P) lo = mid; else hi = mid - 1;
+    }
+    const uint2 e = tab[lo];
+    const unsigned long long need = (P - e.x) << 9;                 // low16 * w >= need
+    const unsigned long long low = min((need + e.y - 1) / e.y, (unsigned long long)(kBkBins - 1));
+    out[k] = (lo << kBkBinLog) | (uint32_t)low;
+}
+
 struct BkSmem {
     unsigned long long pair[kBkCap];      // (key << 32) | index, grouped by slot
     uint32_t cnt[kBkSlots];               // slot populations, then slot starts, then slot ends
@@ -312,10 +339,10 @@ __global__ void __launch_bounds__(kBkSortThreads, 4) bucket_sort_kernel(const ui
                                                                         const uint32_t* __restrict__ cursor,
                                                                         const uint32_t* __restrict__ base,
                                                                         const uint32_t* __restrict__ overflow,
-                                                                        const uint2* __restrict__ tabs,
+                                                                        const uint32_t* __restrict__ klos,
                                                                         uint32_t* __restrict__ idx_out,
                                                                         float* __restrict__ sorted_out, uint32_t N,
-                                                                        uint32_t nb, uint32_t M, long long B) {
+                                                                        uint32_t nb, long long B) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     BkSmem& sm = *reinterpret_cast<BkSmem*>(smem_raw);
     const long long b = bidx();
@@ -326,8 +353,22 @@ __global__ void __launch_bounds__(kBkSortThreads, 4) bucket_sort_kernel(const ui
     if (n == 0) return;
     const uint32_t r0 = base[(size_t)b * nb + bk];
     const uint2* sl = slabs + ((size_t)b * nb + bk) * kBkCap;
-    const uint2* tab = tabs + (size_t)b * kBkBins;
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    // linear slot map of this bucket's key interval (the outermost buckets, whose interval is open-ended, borrow
+    // twice the width of their neighbour); monotone in the key, equal keys share a slot, out-of-range keys clamp
+    uint32_t klo, width;
+    {
+        const uint32_t* kb = klos + (size_t)b * (nb + 1);
+        klo = kb[bk];
+        width = kb[bk + 1] - klo;
+        if (bk + 1 == nb && nb > 1) width = 2u * min(klo - kb[bk - 1], 0x7fffffffu);
+        if (bk == 0 && nb > 2) { width = 2u * min(kb[2] - kb[1], 0x7fffffffu); klo = kb[1] > width ? kb[1] - width : 0u; width = kb[1] - klo; }
+    }
+    const float scale = (float)kBkSlots / ((float)width + 1.0f);
+    auto slot_of = [&](uint32_t key) -> uint32_t {
+        const uint32_t d = key > klo ? key - klo : 0u;
+        return min((uint32_t)(__uint2float_rz(d) * scale), (uint32_t)(kBkSlots - 1));
+    };
     constexpr int PER = kBkSlots / kBkSortThreads;
 #pragma unroll
     for (int i = 0; i < PER; ++i) sm.cnt[i * kBkSortThreads + t] = 0u;
@@ -335,7 +376,7 @@ __global__ void __launch_bounds__(kBkSortThreads, 4) bucket_sort_kernel(const ui
     // 1. slot populations (the slab stays in L2 for step 3)
 #pragma unroll 4
     for (uint32_t e = t; e < n; e += kBkSortThreads) {
-        const uint32_t s = bs_of(__ldcg(&sl[e].x), tab, M) & (uint32_t)(kBkSlots - 1);
+        const uint32_t s = slot_of(__ldcg(&sl[e].x));
         atomicAdd(&sm.cnt[s], 1u);
         sm.slot[e] = (unsigned short)s;
     }
@@ -389,7 +430,7 @@ __global__ void __launch_bounds__(kBkSortThreads, 4) bucket_sort_kernel(const ui
     for (uint32_t q = t; q < n; q += kBkSortThreads) {
         const unsigned long long v = sm.pair[q];
         const uint32_t key = (uint32_t)(v >> 32);
-        const uint32_t s = bs_of(key, tab, M) & (uint32_t)(kBkSlots - 1);
+        const uint32_t s = slot_of(key);
         const uint32_t z = sm.cnt[s];
         const uint32_t a = s ? sm.cnt[s - 1] : 0u;
         uint32_t r = q;
@@ -451,7 +492,8 @@ inline size_t bucket32_zero_bytes(long long B, long long N) {
 }
 inline size_t bucket32_ctl_bytes(long long B, long long N) {
     const size_t nb = (size_t)(N >> kBkMeanLog);
-    return align_up(bucket32_zero_bytes(B, N), 256) + align_up((size_t)B * kBkBins * 8, 256) + align_up((size_t)B * nb * 4, 256);
+    return align_up(bucket32_zero_bytes(B, N), 256) + align_up((size_t)B * kBkBins * 8, 256) + align_up((size_t)B * nb * 4, 256) +
+           align_up((size_t)B * (nb + 1) * 4, 256);
 }
 
 // vals [B][N] -> idx_out (and optionally the sorted values) for the curves whose buckets all fit; *overflow_out points
@@ -469,7 +511,8 @@ inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* so
     const size_t zero_bytes = bucket32_zero_bytes(B, N);
     w += align_up(zero_bytes, 256);
     uint2* tab = (uint2*)w; w += align_up((size_t)B * kBkBins * 8, 256);
-    uint32_t* base = (uint32_t*)w;
+    uint32_t* base = (uint32_t*)w; w += align_up((size_t)B * g.nb * 4, 256);
+    uint32_t* klo = (uint32_t*)w;
     uint2* slabs2 = pairs;
     uint2* slabs1 = pairs + (size_t)B * g.nb * kBkCap;
     cudaError_t e;
@@ -483,6 +526,7 @@ inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* so
         AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B)));
         AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)(B * kCdfChunks), 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
     }
+    AGN_LAUNCH(K_SORT_CDF, st, (bucket_bounds_kernel<<<bgrid((g.nb + 256) / 256, B), 256, 0, st>>>(tab, klo, g.nb, bucket32_magic(g.nb), B)));
     PartArgs a;
     a.vals = vals; a.in = slabs1; a.in_count = cursor1; a.overflow = overflow; a.tab = tab;
     a.N = (uint32_t)N; a.nb = g.nb; a.M = bucket32_magic(g.nb); a.lb = g.lb; a.nc = g.nc; a.cap_in = g.cap1; a.tiles_in = g.tiles1; a.B = B;
@@ -493,7 +537,7 @@ inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* so
     const uint32_t bchunks = g.nb >= 16384 ? 16u : (g.nb >= 1024 ? g.nb / 1024 : 1u);
     AGN_LAUNCH(K_SORT_CDF, st, (bucket_base_kernel<<<(unsigned)(B * bchunks), 1024, 0, st>>>(cursor2, base, g.nb, bchunks)));
     AGN_LAUNCH(K_SORT_BUCKET, st, (bucket_sort_kernel<<<bgrid(g.nb, B), kBkSortThreads, sizeof(BkSmem), st>>>(
-        slabs2, cursor2, base, overflow, tab, idx_out, sorted_out, (uint32_t)N, g.nb, a.M, B)));
+        slabs2, cursor2, base, overflow, klo, idx_out, sorted_out, (uint32_t)N, g.nb, B)));
     *overflow_out = overflow;
     return cudaGetLastError();
 }
