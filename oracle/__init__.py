@@ -28,6 +28,8 @@ def lib():
         _lib.orc_u53.argtypes = [C.c_uint32, C.c_uint32]
         _lib.orc_psd_unit_variance_A.restype = C.c_double
         _lib.orc_psd_unit_variance_A.argtypes = [C.c_int64, C.c_double, C.c_double, C.c_double, C.c_double]
+        _lib.orc_delta_rms.restype = C.c_double
+        _lib.orc_delta_rms.argtypes = [C.c_void_p, C.c_void_p, C.c_int64]
     return _lib
 
 
@@ -219,3 +221,55 @@ def periodogram_binned(x, dt, norm, edges):
     lib().orc_periodogram_binned(_p(x), C.c_int64(x.size), C.c_double(dt), C.c_int(norm), C.c_int(nb),
                                  _p(edges), _p(out), _p(cnt))
     return out, cnt
+
+
+# ---- NEXT-1: delta_i (Eq. 4) ---------------------------------------------------------------------
+def delta_rms(x_new, x_old):
+    x_new, x_old = _d(x_new), _d(x_old)
+    return lib().orc_delta_rms(_p(x_new), _p(x_old), x_new.size)
+
+
+def e13_iterate_delta(A_norm, sorted_vals, perm0, max_iter, threshold=0.0):
+    A_norm, sorted_vals = _d(A_norm), _d(sorted_vals)
+    perm = np.array(perm0, dtype=np.uint32, copy=True)
+    n = sorted_vals.size
+    x = np.empty(n)
+    iters = C.c_int32(0)
+    hist = np.zeros(max_iter, dtype=np.int64)
+    dhist = np.zeros(max_iter)
+    rc = lib().orc_e13_iterate_delta(C.c_int64(n), _p(A_norm), _p(sorted_vals), _p(perm), _p(x), C.c_int(max_iter),
+                                     C.c_double(threshold), C.byref(iters), _p(hist), _p(dhist))
+    if rc != 0:
+        raise ValueError("orc_e13_iterate_delta: bad arguments")
+    return {"x": x, "perm": perm, "iters_used": iters.value, "changed_hist": hist, "delta_hist": dhist}
+
+
+# ---- NEXT-2: structure function (Eq. A6), representative SF (Eq. 6), P(|dm| > dm_ref | tau) ---------
+def structure_function(x, lags, mag=False):
+    x = _d(x)
+    lags = np.ascontiguousarray(lags, dtype=np.int64)
+    sf2 = np.empty(lags.size)
+    pairs = np.empty(lags.size, dtype=np.int64)
+    lib().orc_structure_function(_p(x), C.c_int64(x.size), _p(lags), C.c_int(lags.size), C.c_int(1 if mag else 0),
+                                 _p(sf2), _p(pairs))
+    return sf2, pairs
+
+
+def sf_representative(sf2):
+    sf2 = _d(sf2)
+    nsim, nl = sf2.shape
+    mean, se = np.empty(nl), np.empty(nl)
+    lib().orc_sf_representative(_p(sf2), C.c_int(nsim), C.c_int(nl), _p(mean), _p(se))
+    return mean, se
+
+
+def delta_m_prob(x, lags, dm_ref, m_zero=0.0, m_cut=None):
+    x = _d(x)
+    lags = np.ascontiguousarray(lags, dtype=np.int64)
+    dm_ref = _d(dm_ref)
+    prob = np.empty((lags.size, dm_ref.size))
+    cons = np.empty(lags.size, dtype=np.int64)
+    lib().orc_delta_m_prob(_p(x), C.c_int64(x.size), _p(lags), C.c_int(lags.size), _p(dm_ref), C.c_int(dm_ref.size),
+                           C.c_double(m_zero), C.c_int(0 if m_cut is None else 1),
+                           C.c_double(0.0 if m_cut is None else m_cut), _p(prob), _p(cons))
+    return prob, cons

@@ -26,6 +26,12 @@
 //   orc_e13_step/iterate   pinned: exact-permutation invariant, amplitude invariances (scale, DC),
 //                                  |X'| == A_norm after the replace, restart reproducibility
 //   orc_periodogram        pinned: Parseval identity A5, single tone, white noise
+//   orc_delta_rms / orc_e13_iterate_delta   pinned: 0 at a fixed point, closed form for one swapped pair,
+//                                  exactly 1 for x -> 10 x (the log is log10), threshold honoured
+//   orc_structure_function pinned: brute force over all pairs, a^2 l^2 for a ramp, 2 sigma^2 (1 - cos) for a tone,
+//                                  random-walk ensemble slope beta = (alpha - 1)/2 = 1/2, magnitude invariances
+//   orc_delta_m_prob       pinned: brute force, 0 beyond 2.5 x the dynamic range, monotone in dm_ref
+//   orc_sf_representative  pinned: by hand (Eq. 6)
 //
 // Build: g++ -O2 -std=c++17 -shared -fPIC -o liboracle.so agnvar_oracle.cpp   (oracle/build.py)
 
@@ -454,6 +460,124 @@ void orc_periodogram_binned(const double* x, int64_t N, double dt, int norm, int
         for (int64_t j = j0; j < j1; ++j) acc += P[(size_t)(j - 1)];
         counts[e] = j1 - j0;
         out[e] = (j1 > j0) ? acc / (double)(j1 - j0) : 0.0;
+    }
+}
+
+// ----------------------------------------------------------------------------------------------
+// NEXT-1. The paper's own convergence measure (Eq. 4):
+//   delta_i = rms[ log( x_i(t_n) / x_{i-1}(t_n) ) ], n = 1..N,
+// "log" read as log10 (the paper speaks in dex; Q14).  rms = sqrt of the mean of the squares.
+// ----------------------------------------------------------------------------------------------
+double orc_delta_rms(const double* x_new, const double* x_old, int64_t n) {
+    double acc = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        double d = std::log10(x_new[i] / x_old[i]);
+        acc += d * d;
+    }
+    return std::sqrt(acc / (double)n);
+}
+
+// The loop of orc_e13_iterate with the paper's stopping rule added: after iteration k, delta_k is Eq. 4 between
+// x_sim,k+1 and x_sim,k; the curve stops at the first k with changed == 0 or (threshold > 0 and delta_k <= threshold).
+// delta_hist (max_iter entries): delta_k of every executed iteration, 0 afterwards.
+int orc_e13_iterate_delta(int64_t N, const double* A_norm, const double* sorted, uint32_t* perm, double* x,
+                          int max_iter, double threshold, int32_t* iters_used, int64_t* changed_hist,
+                          double* delta_hist) {
+    if (N < 2 || max_iter < 1) return 1;
+    size_t n = (size_t)N;
+    std::vector<double> xs(n), xn(n), xa(n);
+    std::vector<uint32_t> idx(n);
+    for (size_t r = 0; r < n; ++r) xs[perm[r]] = sorted[r];
+    for (int k = 0; k < max_iter; ++k) {
+        if (changed_hist) changed_hist[k] = 0;
+        if (delta_hist) delta_hist[k] = 0.0;
+    }
+    int used = max_iter;
+    for (int k = 1; k <= max_iter; ++k) {
+        int64_t ch = 0;
+        orc_e13_step(N, A_norm, sorted, perm, xs.data(), xa.data(), idx.data(), xn.data(), &ch);
+        double delta = orc_delta_rms(xn.data(), xs.data(), N);
+        std::memcpy(perm, idx.data(), n * sizeof(uint32_t));
+        xs.swap(xn);
+        if (changed_hist) changed_hist[k - 1] = ch;
+        if (delta_hist) delta_hist[k - 1] = delta;
+        if (ch == 0 || (threshold > 0.0 && delta <= threshold)) { used = k; break; }
+    }
+    std::memcpy(x, xs.data(), n * sizeof(double));
+    if (iters_used) *iters_used = used;
+    return 0;
+}
+
+// ----------------------------------------------------------------------------------------------
+// NEXT-2. Structure function (Eq. A6) of an evenly sampled series at integer lags l (tau = l dt):
+//   SF(tau)^2 = (1/P) sum over the P = N - l pairs (i, j = i + l) of [ x(t_i) - x(t_j) ]^2 .
+// mag != 0: the series is first converted to magnitudes, m = -2.5 log10(x) (for a constant
+// bolometric correction m(t2) - m(t1) = -2.5 log[L(t2)/L(t1)]; the zero point cancels in the differences).
+// A lag with no pair (l >= N) gets sf2 = 0, pairs = 0.
+// ----------------------------------------------------------------------------------------------
+void orc_structure_function(const double* x, int64_t N, const int64_t* lags, int nlags, int mag, double* sf2,
+                            int64_t* pairs) {
+    std::vector<double> v((size_t)N);
+    for (int64_t i = 0; i < N; ++i) v[(size_t)i] = mag ? -2.5 * std::log10(x[i]) : x[i];
+    for (int q = 0; q < nlags; ++q) {
+        const int64_t l = lags[q];
+        double acc = 0.0;
+        int64_t P = 0;
+        for (int64_t i = 0; i + l < N; ++i) {
+            double d = v[(size_t)i] - v[(size_t)(i + l)];
+            acc += d * d;
+            ++P;
+        }
+        sf2[q] = P > 0 ? acc / (double)P : 0.0;
+        if (pairs) pairs[q] = P;
+    }
+}
+
+// Representative structure function (Eq. 6): SF_rep(tau)^2 = mean over the N_sim realisations of
+// SF_i(tau)^2; its standard error from the scatter of the SF_i^2 (sample standard deviation / sqrt(N_sim)).
+// sf2: [nsim][nlags] row-major.
+void orc_sf_representative(const double* sf2, int nsim, int nlags, double* mean, double* stderr_) {
+    for (int q = 0; q < nlags; ++q) {
+        double m = 0.0;
+        for (int i = 0; i < nsim; ++i) m += sf2[(size_t)i * nlags + q];
+        m /= (double)nsim;
+        double var = 0.0;
+        for (int i = 0; i < nsim; ++i) {
+            double d = sf2[(size_t)i * nlags + q] - m;
+            var += d * d;
+        }
+        mean[q] = m;
+        if (stderr_) stderr_[q] = nsim > 1 ? std::sqrt(var / (double)(nsim - 1) / (double)nsim) : 0.0;
+    }
+}
+
+// P(|dm| > dm_ref given tau) (Figs 16-17): for each lag, the number of pairs separated by that lag
+// with |m_i - m_j| > dm_ref divided by the number of pairs considered, m = m_zero - 2.5 log10(x).
+// use_cut != 0 (Fig. 17): every point with m > m_cut is replaced by the upper limit m_cut, and only pairs in which
+// at least one point is detected (m <= m_cut) are considered.
+// prob: [nlags][nref]; considered: [nlags] (may be NULL).  No pair considered -> probabilities 0.
+void orc_delta_m_prob(const double* x, int64_t N, const int64_t* lags, int nlags, const double* dm_ref, int nref,
+                      double m_zero, int use_cut, double m_cut, double* prob, int64_t* considered) {
+    std::vector<double> m((size_t)N);
+    std::vector<char> det((size_t)N);
+    for (int64_t i = 0; i < N; ++i) {
+        double mi = m_zero - 2.5 * std::log10(x[i]);
+        det[(size_t)i] = (!use_cut || mi <= m_cut) ? 1 : 0;
+        if (use_cut && mi > m_cut) mi = m_cut;
+        m[(size_t)i] = mi;
+    }
+    for (int q = 0; q < nlags; ++q) {
+        const int64_t l = lags[q];
+        std::vector<int64_t> cnt((size_t)nref, 0);
+        int64_t P = 0;
+        for (int64_t i = 0; i + l < N; ++i) {
+            if (!(det[(size_t)i] || det[(size_t)(i + l)])) continue;
+            ++P;
+            double d = std::fabs(m[(size_t)i] - m[(size_t)(i + l)]);
+            for (int r = 0; r < nref; ++r) cnt[(size_t)r] += (d > dm_ref[r]);
+        }
+        for (int r = 0; r < nref; ++r) prob[(size_t)q * nref + r] = P > 0 ? (double)cnt[(size_t)r] / (double)P : 0.0;
+        if (considered) considered[q] = P;
     }
 }
 
