@@ -7,14 +7,23 @@ One "step" = one pass of the whole hot path (S1 ERDF draw + sort
 max_iter x [L1 FFT, L2 replace, L3 IFFT, L4 argsort, L5 scatter+count, L6 bookkeeping], P periodogram
 where the configuration asks for it) over one batch of synthetic curves of BASELINE.json's configuration
 (default C4: B=4, N=2^26, fp32, 50 iterations -- the configuration the metric is quoted on).
-Prints ONE JSON line (rank 0).  N > 1: launched by torchrun, one rank per GPU, every rank runs its own
-batch of curves (curve numbers rank*B ...; no data-path collective; weak scaling).
+Prints ONE JSON line (rank 0).
+
+N > 1: one rank per GPU, every rank runs its own batch of curves (curve numbers rank*B ...; no data-path
+collective; weak scaling).  Under torchrun the ranks come from the environment; `python bench.py --gpus N`
+without torchrun re-executes itself under `python -m torch.distributed.run` with N ranks on 127.0.0.1.
+
+Timed regions: (1) `value`: K steps, device-resident, CUDA events, NO per-launch tracing; (2) `e2e`: K steps through
+the public API with the result copied to pinned host memory inside the region; (3) one more step with per-launch
+CUDA-event tracing switched on, which feeds `kernels`, `stages` and `roofline` (the traced step is not part of
+`value`).
 
 --impl reference times the CPU oracle (oracle/, fp64, plain) on a bounded sample of the same workload.
 """
 import argparse
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -38,19 +47,24 @@ ALGO_BYTES_PER_SAMPLE = {
     "sort_digit_hist": 4.0,         # read keys
     "sort_onesweep": 16.0,          # read (key, idx) 8 + write (key, idx) 8 (first/last pass move less)
     "sort_cdf_tables": 0.5,         # one key in 64, a 32-byte sector each (+ small tables)
-    "sort_msd_partition": 14.0,     # mean of the two levels: (key 4 -> pair 8) and (pair 8 -> pair 8)
+    "sort_part_level0": 12.0,       # key 4 -> (key, idx) pair 8
+    "sort_part_level1": 16.0,       # pair 8 -> pair 8
+    "sort_part_onelevel": 12.0,     # key 4 -> pair 8, straight into the fine buckets
     "sort_bucket_finish": 12.0,     # read (key, idx) 8 + write idx 4
     "cta_argsort": 8.0,             # read key 4 + write idx 4
     "rank_scatter_count": 16.0,     # idx_new 4 + idx_old 4 + sorted 4 + write x 4
     "scatter_bin": 20.0,            # read 12 + write (val, dst) 8
     "scatter_place": 12.0,          # read 8 + write 4
+    "e13_onchip_loop": 0.0,         # the whole loop on chip: per-iteration HBM traffic ~0 (see "hbm_equivalent")
+    "sort_lsd_fallback_gated": 0.0, # the LSD passes behind the distribution sort: they exit at once unless a slab overflowed
 }
 # SURVEY.md 8(d) two-level model, bytes per sample per iteration, per stage (fp32)
 STAGE_MODEL_BYTES = {"fft": 26.0, "argsort": 28.0, "scatter": 32.0}
 STAGE_OF = {
     "fft_pass_strided": "fft", "fft_pass_contiguous": "fft", "amplitude_replace": "fft", "fft_mid_fused": "fft", "fft_columns": "fft",
     "sort_digit_hist": "argsort", "sort_onesweep": "argsort", "cta_argsort": "argsort",
-    "sort_msd_partition": "argsort", "sort_bucket_finish": "argsort", "sort_cdf_tables": "argsort",
+    "sort_part_level0": "argsort", "sort_part_level1": "argsort", "sort_part_onelevel": "argsort",
+    "sort_bucket_finish": "argsort", "sort_cdf_tables": "argsort", "sort_lsd_fallback_gated": "argsort",
     "rank_scatter_count": "scatter", "scatter_bin": "scatter", "scatter_place": "scatter",
 }
 
@@ -126,23 +140,50 @@ def workload_label(cfg):
 # ------------------------------------------------------------------------------------------------------
 # the CPU oracle, timed as it stands on a bounded sample (cpu_baseline leg and --impl reference)
 # ------------------------------------------------------------------------------------------------------
-def oracle_sample_inputs(cfg, logn):
+def oracle_sample_inputs(cfg, logn, curve=0):
+    """The oracle's own S1 + S2 for one curve of the configuration's parameters at N = 2^logn."""
     import numpy as np
     import oracle
     N = 1 << logn
     e, p = cfg["erdf"][0], cfg["psd"][0]
-    srt, perm0, _ = oracle.erdf_sample_sorted(e, cfg["grid_points"], N, cfg["seed"], 0, 0 if cfg["dtype"] == "f32" else 1)
-    tk = oracle.tk_generate(0.0, p["f_b"], p["alpha_low"], p["alpha_high"], N, cfg["dt"], 1, cfg["seed"], 0)
+    srt, perm0, _ = oracle.erdf_sample_sorted(e, cfg["grid_points"], N, cfg["seed"], curve, 0 if cfg["dtype"] == "f32" else 1)
+    tk = oracle.tk_generate(0.0, p["f_b"], p["alpha_low"], p["alpha_high"], N, cfg["dt"], 1, cfg["seed"], curve)
     return np.ascontiguousarray(tk["A_norm"]), srt, perm0
 
 
-def oracle_time(cfg, logn, iters, inputs=None):
+def synthetic_loop_inputs(logn, seed=0):
+    """Inputs of the right size and shape for TIMING the oracle's loop at sizes where its own S1/S2 would take minutes:
+    a sorted log-normal draw, a random permutation and red-noise amplitudes, from numpy (no arithmetic of the method)."""
+    import numpy as np
+    N = 1 << logn
+    rng = np.random.default_rng(seed)
+    srt = np.sort(10.0 ** rng.normal(-2.0, 0.7, N))
+    perm0 = rng.permutation(N).astype(np.uint32)
+    j = np.arange(N // 2 + 1, dtype=np.float64)
+    an = 1.0 / (1.0 + j)
+    return an, srt, perm0
+
+
+def oracle_time(logn, iters, inputs):
     import oracle
-    an, srt, perm0 = inputs if inputs is not None else oracle_sample_inputs(cfg, logn)
+    an, srt, perm0 = inputs
     t0 = time.perf_counter()
     oracle.e13_iterate(an, srt, perm0, iters)
     dt = time.perf_counter() - t0
     return (1 << logn) * iters / dt, dt
+
+
+def oracle_all_cores(cfg, logn, iters):
+    """One curve per host thread (the oracle itself is single-threaded; ctypes releases the GIL during the call)."""
+    from concurrent.futures import ThreadPoolExecutor
+    cores = os.cpu_count() or 1
+    inputs = synthetic_loop_inputs(logn)
+    sets = [(inputs[0], inputs[1], inputs[2].copy()) for _ in range(cores)]
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=cores) as ex:
+        list(ex.map(lambda s: oracle_time(logn, iters, s), sets))
+    dt = time.perf_counter() - t0
+    return cores * (1 << logn) * iters / dt, dt, cores
 
 
 def run_reference(args, cfg):
@@ -153,10 +194,10 @@ def run_reference(args, cfg):
     iters = 1
     inputs = oracle_sample_inputs(cfg, logn)
     for _ in range(args.warmup):
-        oracle_time(cfg, logn, iters, inputs)
+        oracle_time(logn, iters, inputs)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle_time(cfg, logn, iters, inputs)
+        oracle_time(logn, iters, inputs)
     dt = time.perf_counter() - t0
     value = args.steps * (1 << logn) * iters / dt
     sample = (f"1 curve of {cfg['name']}'s PSD/ERDF parameters at N=2^{logn}, {iters} E13 iteration per step "
@@ -172,6 +213,54 @@ def run_reference(args, cfg):
 
 
 # ------------------------------------------------------------------------------------------------------
+# fp32 free-running context numbers (reported next to the lock-step gates, never gated)
+# ------------------------------------------------------------------------------------------------------
+def fp32_context(ag, cfg, dev):
+    import numpy as np
+    import oracle
+    from paper_1909_06374_b200 import workloads
+    logn, iters = 20, 10
+    N = 1 << logn
+    c = dict(cfg, B=1, N=N, max_iter=iters, nbins=0, oversample=1, psd=cfg["psd"][:1], erdf=cfg["erdf"][:1])
+    srt, perm, _ = ag.agnvar_erdf_sample_sorted(c["erdf"], 1, N, "f32", c["seed"], 0, c["grid_points"], device=dev)
+    _, an = ag.agnvar_tk_generate(c["psd"], 1, N, c["dt"], 1, "f32", c["seed"], 0, want_xnorm=False, device=dev)
+    srt_h, an_h = srt.cpu().numpy()[0], an.cpu().numpy()[0]
+    perm_h = perm.cpu().numpy().view(np.uint32)[0].copy()
+    out = ag.agnvar_e13_iterate(an, srt, perm, iters, want_delta=True)
+    xg = out["x"].cpu().numpy()[0].astype(np.float64)
+    ref = oracle.e13_iterate_delta(an_h, srt_h, perm_h, iters, 0.0)      # same inputs (exact in fp64), fp64 arithmetic
+    xo = ref["x"]
+    edges = workloads.log_bin_edges(N, 64)
+    pg, _ = oracle.periodogram_binned(xg, c["dt"], 0, edges)
+    po, _ = oracle.periodogram_binned(xo, c["dt"], 0, edges)
+    # the target: the amplitudes the loop is asked to reach, binned the same way (P_j = 2/N^2 A_j^2, Eq. A2)
+    tgt = 2.0 / (N * float(N)) * an_h.astype(np.float64)[1:] ** 2
+    pt = np.array([tgt[edges[e] - 1:edges[e + 1] - 1].mean() for e in range(len(edges) - 1)])
+    return {"sample": f"1 curve of {cfg['name']}'s parameters, N=2^{logn}, {iters} iterations, fp32 product vs fp64 oracle, "
+                      f"same inputs, free-running (reported, not gated: the map is chaotic w.r.t. rounding)",
+            "value_equal_fraction": float(np.mean(xg == xo)),
+            "dlog10_rms_dex": float(np.sqrt(np.mean(np.log10(xg / xo) ** 2))),
+            "binned_periodogram_max_rel_diff": float(np.max(np.abs(pg / po - 1.0))),
+            # shape consistency with the target amplitudes: scatter of log10(P / P_target) over the 64
+            # bins about its mean (the level is fixed by the PDF, not by A_norm)
+            "periodogram_vs_target_shape_rms_dex": {"gpu_fp32": float(np.std(np.log10(pg / pt))),
+                                                    "oracle_fp64": float(np.std(np.log10(po / pt)))},
+            "delta_last_iteration": {"gpu_fp32": float(out["delta_hist"][0, iters - 1]),
+                                     "oracle_fp64": float(ref["delta_hist"][iters - 1])}}
+
+
+# ------------------------------------------------------------------------------------------------------
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` without torchrun: run the same command line as N ranks on this node."""
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -183,6 +272,11 @@ def main():
     ap.add_argument("--max-iter", type=int, default=None, help="override max_iter (NOT the headline configuration)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-context", action="store_true", help="skip the fp32 free-running context numbers")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="process-group backend of the N > 1 plumbing (gloo: host-side tests of the spawn path)")
+    ap.add_argument("--dry-ranks", action="store_true",
+                    help="N > 1 plumbing only (rendezvous, curve partition, max-over-ranks, one JSON line), no GPU work")
     args = ap.parse_args()
 
     from paper_1909_06374_b200 import workloads
@@ -191,14 +285,35 @@ def main():
         cfg["max_iter"] = args.max_iter
     if args.impl == "reference":
         run_reference(args, cfg)
-        return
+        return 0
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return respawn_under_torchrun(args)
 
     import torch
-    import paper_1909_06374_b200 as ag
+    from paper_1909_06374_b200 import multirank
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
+    B, N, iters = cfg["B"], cfg["N"], cfg["max_iter"]
+    curve0 = multirank.weak_curve0(B, rank)   # Philox curve numbers of this rank's rows: results do not depend on the partition
+    units_per_step = B * N * iters
+
+    if args.dry_ranks:
+        import torch.distributed as dist
+        dist.init_process_group(args.backend)
+        ms = multirank.max_over_ranks(100.0 + rank, None, dist)
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "unit": UNIT, "n_gpus": world, "dry_ranks": True, "ms_max_over_ranks": ms,
+                              "curve0_by_rank": [multirank.weak_curve0(B, r) for r in range(world)],
+                              "config": {"workload": workload_label(cfg)}}), flush=True)
+        dist.barrier()
+        dist.destroy_process_group()
+        return 0
+
+    import paper_1909_06374_b200 as ag
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
     torch.cuda.set_device(local_rank)
@@ -206,23 +321,18 @@ def main():
     dist = None
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
+        dist.init_process_group(args.backend, device_id=dev if args.backend == "nccl" else None)
     ag.lib()
-
-    B, N, iters = cfg["B"], cfg["N"], cfg["max_iter"]
-    from paper_1909_06374_b200 import multirank
-    curve0 = multirank.weak_curve0(B, rank)   # Philox curve numbers of this rank's rows: results do not depend on the partition
-    units_per_step = B * N * iters
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def step(host_out=None):
-        return ag.generate_light_curves(cfg, device=dev, host_out=host_out, curve0=curve0)
+    def step(host_out=None, want_fallbacks=False):
+        return ag.generate_light_curves(cfg, device=dev, host_out=host_out, curve0=curve0, want_fallbacks=want_fallbacks)
 
-    # ---- device-resident timing ----------------------------------------------------------------------
+    # ---- (1) device-resident timing, untraced ----------------------------------------------------------
     for _ in range(args.warmup):
         out = step()
     barrier()
@@ -230,7 +340,6 @@ def main():
     if rank == 0:
         sampler.start()
     l0 = ag.launch_count()
-    ag.trace_begin()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record()
@@ -239,7 +348,6 @@ def main():
     e1.record()
     barrier()
     ms = e0.elapsed_time(e1)
-    trace = ag.trace_end()
     launches = ag.launch_count() - l0
     clocks = sampler.stop() if rank == 0 else None
     iters_used = out["iters_used"].cpu().tolist()
@@ -247,17 +355,30 @@ def main():
     ms = multirank.max_over_ranks(ms, dev, dist)
     value = world * units_per_step * args.steps / (ms * 1e-3)
 
-    # ---- per-kernel accounting (CUDA events around every launch of the timed steps) --------------------
+    # ---- (3) one traced step: CUDA events around every launch -> per-kernel table, stages, roofline ---------
+    barrier()
+    ag.trace_begin()
+    t0e, t1e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0e.record()
+    out = step(want_fallbacks=True)
+    t1e.record()
+    torch.cuda.synchronize()
+    trace = ag.trace_end()
+    ms_traced = t0e.elapsed_time(t1e)
+    fallbacks = int(out["sort_fallbacks"].sum()) if out.get("sort_fallbacks") is not None else None
+    del out
     fam = {}
     for name, t in trace:
         f = fam.setdefault(name, [0, 0.0])
         f[0] += 1
         f[1] += t
     peak, peak_src = measured_peaks()
-    kernels = {k: {"launches": v[0], "ms_total": round(v[1], 4), "ms_avg": v[1] / v[0]} for k, v in fam.items()}
-    loop = {k: v for k, v in fam.items() if k in ALGO_BYTES_PER_SAMPLE}
+    kernels = {k: {"launches": v[0], "ms_total": round(v[1], 4), "ms_avg": v[1] / v[0],
+                   "algorithmic_bytes_per_sample": ALGO_BYTES_PER_SAMPLE.get(k)} for k, v in fam.items()}
+    loop = {k: v for k, v in fam.items() if k in STAGE_OF}
     roofline = None
     stages = {}
+    traffic_model = None
     if loop:
         top = max(loop, key=lambda k: loop[k][1])
         n_l, t_l = loop[top]
@@ -266,25 +387,31 @@ def main():
         roofline = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                     "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_ms": t_l / n_l,
-                    "share_of_step": t_l / ms}
+                    "share_of_step": t_l / ms_traced, "timing": "one traced step (CUDA events around every launch)"}
         prof = os.path.join(ROOT, "profiles", "traffic.json")     # dram bytes per launch from the committed ncu capture
         try:
             with open(prof) as f:
-                roofline["traffic"] = json.load(f).get(top)
+                tj = json.load(f)
+            roofline["traffic"] = tj.get(top)
+            roofline["traffic_source"] = "committed ncu capture (profiles/traffic.json), not measured in this run"
         except Exception:
             pass
         # stage view (the north_star target: each stage >= 60% of the HBM roofline on the 2-level byte model)
-        n_iter_total = args.steps * iters
+        st_ms, st_bytes = {}, {}
         for k, v in loop.items():
-            s = stages.setdefault(STAGE_OF[k], 0.0)
-            stages[STAGE_OF[k]] = s + v[1]
-        stages = {s: {"ms_per_iteration": t / n_iter_total,
+            st_ms[STAGE_OF[k]] = st_ms.get(STAGE_OF[k], 0.0) + v[1]
+            st_bytes[STAGE_OF[k]] = st_bytes.get(STAGE_OF[k], 0.0) + ALGO_BYTES_PER_SAMPLE[k] * v[0] / iters
+        stages = {s: {"ms_per_iteration": t / iters,
                       "model_bytes_per_sample": STAGE_MODEL_BYTES[s],
-                      "achieved_GBps": STAGE_MODEL_BYTES[s] * B * N / (t / n_iter_total * 1e-3) / 1e9,
-                      "frac_of_peak": STAGE_MODEL_BYTES[s] * B * N / (t / n_iter_total * 1e-3) / 1e9 / peak}
-                  for s, t in stages.items()}
+                      "moved_bytes_per_sample": st_bytes[s],        # what this build's kernels move (algorithmic, summed)
+                      "moved_over_model": st_bytes[s] / STAGE_MODEL_BYTES[s],
+                      "achieved_GBps": STAGE_MODEL_BYTES[s] * B * N / (t / iters * 1e-3) / 1e9,
+                      "frac_of_peak": STAGE_MODEL_BYTES[s] * B * N / (t / iters * 1e-3) / 1e9 / peak}
+                  for s, t in st_ms.items()}
+        traffic_model = {"iteration_model_bytes_per_sample": sum(STAGE_MODEL_BYTES.values()),
+                         "iteration_moved_bytes_per_sample": sum(st_bytes.values())}
 
-    # ---- end to end: host parameters in, light curves out to pinned host memory -------------------------
+    # ---- (2) end to end: host parameters in, light curves out to pinned host memory -------------------------
     e2e = None
     if not args.no_e2e:
         host = torch.empty((B, N), dtype=torch.float32 if cfg["dtype"] == "f32" else torch.float64).pin_memory()
@@ -304,12 +431,25 @@ def main():
 
     # ---- the oracle on this box's host cores (rank 0, N = 1 only) ---------------------------------------
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        logn = min(23, N.bit_length() - 1)
-        v, dt = oracle_time(cfg, logn, 1)
-        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"1 curve of {cfg['name']}'s parameters at N=2^{logn}, 1 E13 iteration, fp64, {dt:.1f} s",
-               "host_cores_available": os.cpu_count()}
+    context = None
+    if rank == 0 and world == 1:
+        if not args.no_context and cfg["dtype"] == "f32":
+            try:
+                context = fp32_context(ag, cfg, dev)
+            except Exception as exc:      # context only: never fails the bench line
+                context = {"error": repr(exc)}
+        ag.free_workspace()
+        if not args.no_cpu_baseline:
+            logn = N.bit_length() - 1                  # the workload's own N (C4: 2^26, one iteration, about a minute)
+            v, dt = oracle_time(logn, 1, synthetic_loop_inputs(logn))
+            la = min(22, logn)
+            va, dta, cores = oracle_all_cores(cfg, la, 1)
+            cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                   "sample": f"1 curve at the workload's own N=2^{logn}, 1 E13 iteration (L1-L6), fp64, 1 thread, {dt:.1f} s; "
+                             f"inputs of that size from numpy (sorted log-normal draw, random permutation, red-noise amplitudes)",
+                   "host_cores_available": os.cpu_count(),
+                   "all_cores": {"value": va, "unit": UNIT, "cores": cores,
+                                 "sample": f"{cores} curves at N=2^{la}, one per host thread, 1 E13 iteration each, {dta:.1f} s"}}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -318,13 +458,16 @@ def main():
                 "config": {"workload": workload_label(cfg), "curves_per_gpu": B, "iterations_executed": iters,
                            "iters_used": iters_used[:8], "l2": "inputs larger than L2 (every array >= 1 GiB)"
                            if B * N * 4 > 2 ** 28 else "arrays smaller than L2: not flushed between steps",
-                           "step": "S1 + S2 + max_iter x (L1..L6) + P"},
+                           "step": "S1 + S2 + max_iter x (L1..L6) + P",
+                           "timing": "value: untraced; kernels/stages/roofline: one extra traced step"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "stages": stages,
-                "cpu_baseline": cpu, "kernels": kernels}
+                "traffic_model": traffic_model, "sort_fallbacks": fallbacks, "ms_traced_step": ms_traced,
+                "cpu_baseline": cpu, "fp32_free_running_context": context, "kernels": kernels}
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+    return 0
 
 
 if __name__ == "__main__":
-    main()
+    sys.exit(main())

@@ -69,7 +69,8 @@ typedef struct {
 } agnvar_erdf;
 
 /* Bytes of scratch the given op needs.  `oversample` matters for AGNVAR_OP_TK_GENERATE only
- * (pass 1 otherwise); `aux` = grid_points for ERDF_SAMPLE_SORTED, nbins for PERIODOGRAM, else 0.
+ * (pass 1 otherwise); `aux` = grid_points for ERDF_SAMPLE_SORTED, nbins for PERIODOGRAM, 1 for E13_ITERATE
+ * with the delta_i rule / history (see agnvar_e13_opts), else 0.
  * Returns 0 for invalid arguments. */
 size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int oversample, int64_t aux);
 
@@ -95,6 +96,11 @@ int agnvar_erdf_sample_sorted(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t
                               uint64_t seed, uint32_t curve0, int grid_points, void* d_sorted,
                               uint32_t* d_perm0, void* d_draw, void* d_ws, size_t ws_bytes, void* stream);
 
+/* S1 (table only) -- the normalised cumulative table C of agnvar_erdf_sample_sorted (O4), for checking the
+ * sampler's premise against a reference: d_out [n_erdf][grid_points] fp64, C_0 = 0, C_{G-1} = 1.
+ * Same validation as agnvar_erdf_sample_sorted; no workspace. */
+int agnvar_erdf_table(const agnvar_erdf* h_erdf, int64_t n_erdf, int grid_points, double* d_out, void* stream);
+
 /* S2 -- Timmer & Koenig series and its amplitudes.  M = oversample * N;
  * X_0 = 0; X_j = sqrt(S_j/2)(g_re + i g_im), 1 <= j < M/2; X_{M/2} = sqrt(S_{M/2}) g_re;
  * S_j = Eq. 3 at f_j = j/(M dt), fp64; g from Philox tag 0, Box-Muller (O1, O3);
@@ -111,6 +117,29 @@ int agnvar_tk_generate(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_
                        int dtype, uint64_t seed, uint32_t curve0, void* d_xnorm, void* d_anorm, void* d_ws,
                        size_t ws_bytes, void* stream);
 
+/* Options of agnvar_e13_iterate (host struct, read before the call returns; NULL = all defaults).
+ *   delta_threshold  > 0: the paper's own stopping rule (Eq. 4).  After iteration k,
+ *                    delta_k = rms over the N samples of log10( x_sim,k+1[t] / x_sim,k[t] ) ("log" read as log10:
+ *                    the paper speaks in dex, Q14); curve b stops at the first k with delta_k <= delta_threshold
+ *                    (or changed = 0): iters_used[b] = k and d_x / d_perm receive the state after iteration k.
+ *                    The batch keeps running until every curve has stopped or k = max_iter (see check_every);
+ *                    <= 0: only the exact rank-change rule below.  Needs positive values in d_sorted.
+ *   d_delta_hist     out [B][max_iter] fp64 or NULL: delta_k of every executed iteration (later entries 0)
+ *   d_sort_fallbacks out [B] i32 or NULL: number of iterations in which curve b's argsort left the distribution
+ *                    sort for the LSD fallback (slab overflow: massive ties, adversarial keys); 0 in a normal run
+ *   check_every      > 0: the call SYNCHRONISES the stream after every check_every iterations and returns early
+ *                    once every curve has stopped (the only case in which a call of this library waits);
+ *                    0: never waits, max_iter iterations are enqueued (stopped curves idle: their outputs are
+ *                    already written)
+ */
+typedef struct {
+    double delta_threshold;
+    double* d_delta_hist;
+    int32_t* d_sort_fallbacks;
+    int32_t check_every;
+    int32_t reserved;
+} agnvar_e13_opts;
+
 /* L1-L6 -- the iteration (steps O6).  Per curve, k = 1..max_iter:
  *   X = DFT_N(x_sim);  X'_j = A_norm_j X_j / |X_j|  (X'_j = A_norm_j if |X_j| = 0; DC and Nyquist
  *   real);  x_adj = IDFT_N(X') with 1/N, -0 -> +0;  idx_new = stable ascending argsort of x_adj
@@ -118,7 +147,7 @@ int agnvar_tk_generate(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_
  *   x_sim[idx_new[r]] = sorted[r].
  * A curve is converged at the first k with changed = 0 (iters_used = k); a converged state is a fixed
  * point, so later iterations of a batch leave it unchanged (Q18).  Not converging within max_iter is
- * not an error: iters_used = max_iter.
+ * not an error: iters_used = max_iter.  h_opts adds the paper's delta_i rule (Eq. 4) and diagnostics.
  *   d_anorm        in  [B][N/2+1] dtype  target amplitudes (natural order, j = 0..N/2)
  *   d_sorted       in  [B][N] dtype      ascending values (the draw)
  *   d_perm         in/out [B][N] u32     in: idx_old of the first iteration (perm0); out: final permutation.
@@ -128,10 +157,14 @@ int agnvar_tk_generate(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_
  *   d_changed_hist out [B][max_iter] i64 or NULL: changed count of every iteration
  *   d_xadj_dbg     out [B][N] dtype or NULL: x_adj of the last iteration (for lock-step checks: call
  *                  with max_iter = 1 to step the product kernels one iteration at a time)
- * EINVAL: bad B/N/dtype, max_iter < 1, NULL d_anorm/d_sorted/d_perm/d_x. */
+ *   h_opts         NULL or options (above).  Workspace: query with aux = 1 when delta_threshold > 0 or
+ *                  d_delta_hist is set (two more [B][N] value buffers and one more permutation buffer).
+ * EINVAL: bad B/N/dtype, max_iter < 1, NULL d_anorm/d_sorted/d_perm/d_x, negative check_every,
+ * non-finite delta_threshold. */
 int agnvar_e13_iterate(int64_t B, int64_t N, int dtype, const void* d_anorm, const void* d_sorted,
                        uint32_t* d_perm, void* d_x, int max_iter, int32_t* d_iters_used,
-                       int64_t* d_changed_hist, void* d_xadj_dbg, void* d_ws, size_t ws_bytes, void* stream);
+                       int64_t* d_changed_hist, void* d_xadj_dbg, const agnvar_e13_opts* h_opts, void* d_ws,
+                       size_t ws_bytes, void* stream);
 
 /* P -- periodogram (Appendix A), bins j = 1..N/2 (DC excluded):
  *   norm 0 (Eq. A2):  P_j = (2/N^2) |DFT_j|^2

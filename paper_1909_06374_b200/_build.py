@@ -3,6 +3,7 @@
 Usage:  python -m paper_1909_06374_b200._build [--force]
 nvcc cross-compiles without a GPU; the built .so travels to the GPU box with the repo snapshot.
 """
+import hashlib
 import os
 import subprocess
 import sys
@@ -10,6 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libagnvar.so")
+HASHFILE = LIB + ".hash"
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
 NVCC_FLAGS = [
@@ -36,15 +38,40 @@ def _nvcc():
     return "nvcc"
 
 
+def source_hash() -> str:
+    """sha256 over the library's sources (names and contents): the staleness test of the built .so.  It is compiled
+    into the library (agnvar_version() ends with it) and kept in a sidecar file next to the .so, so that neither a
+    checkout nor a copy to another machine (which reset mtimes) can make a stale library look fresh."""
+    h = hashlib.sha256()
+    for path in sorted(_sources()):
+        h.update(os.path.relpath(path, os.path.dirname(HERE)).encode())
+        with open(path, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def is_fresh() -> bool:
+    try:
+        with open(HASHFILE) as f:
+            return os.path.exists(LIB) and f.read().strip() == source_hash()
+    except OSError:
+        return False
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    newest = max(os.path.getmtime(s) for s in _sources())
-    if (not force) and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+    """Compile if the sources changed since the .so was built.  Raises FileNotFoundError when nvcc is absent and
+    subprocess.CalledProcessError when the compilation fails (a stale .so is never silently used for edited sources)."""
+    if (not force) and is_fresh():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + ["-I", INCLUDE, "-o", LIB, os.path.join(CSRC, "agnvar.cu")]
+    digest = source_hash()
+    cmd = [_nvcc()] + NVCC_FLAGS + [f'-DAGNVAR_SRC_HASH="{digest}"', "-I", INCLUDE, "-o", LIB,
+                                    os.path.join(CSRC, "agnvar.cu")]
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")
     subprocess.run(cmd, check=True)
+    with open(HASHFILE, "w") as f:
+        f.write(digest + "\n")
     return LIB
 
 

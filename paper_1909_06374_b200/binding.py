@@ -17,7 +17,7 @@ AGNVAR_ERDF_BPL, AGNVAR_ERDF_LOGNORMAL = 0, 1
 OP_ERDF_SAMPLE_SORTED, OP_TK_GENERATE, OP_E13_ITERATE, OP_PERIODOGRAM = 1, 2, 3, 4
 
 EXPORTS = (
-    "agnvar_workspace_bytes", "agnvar_psd_bpl", "agnvar_erdf_sample_sorted", "agnvar_tk_generate",
+    "agnvar_workspace_bytes", "agnvar_psd_bpl", "agnvar_erdf_sample_sorted", "agnvar_erdf_table", "agnvar_tk_generate",
     "agnvar_e13_iterate", "agnvar_periodogram", "agnvar_philox_u32", "agnvar_strerror", "agnvar_version",
     "agnvar_launch_count", "agnvar_trace_begin", "agnvar_trace_end", "agnvar_kernel_name",
 )
@@ -39,20 +39,27 @@ class agnvar_erdf(C.Structure):
                 ("lam_min", C.c_double), ("lam_max", C.c_double)]
 
 
+class agnvar_e13_opts(C.Structure):
+    _fields_ = [("delta_threshold", C.c_double), ("d_delta_hist", C.c_void_p), ("d_sort_fallbacks", C.c_void_p),
+                ("check_every", C.c_int32), ("reserved", C.c_int32)]
+
+
 _lib = None
 
 
 def lib():
-    """Load libagnvar.so (building it with nvcc first if the sources are newer). Raises if impossible."""
+    """Load libagnvar.so, compiling it with nvcc first when the sources changed since it was built (source hash,
+    not mtimes).  Only a missing nvcc falls back to the shipped .so -- and then only if that .so was built from
+    exactly these sources; a failed compilation raises."""
     global _lib
     if _lib is not None:
         return _lib
     path = _build.LIB
     try:
         path = _build.build()
-    except Exception as exc:  # no nvcc on this machine: use the shipped .so if there is one
-        if not os.path.exists(path):
-            raise RuntimeError(f"libagnvar.so is missing and could not be built: {exc}") from exc
+    except FileNotFoundError as exc:  # no nvcc on this machine
+        if not _build.is_fresh():
+            raise RuntimeError(f"libagnvar.so is missing or stale and nvcc is not available: {exc}") from exc
     L = C.CDLL(path)
     vp, i64, u64, u32, i32, dbl, sz = C.c_void_p, C.c_int64, C.c_uint64, C.c_uint32, C.c_int, C.c_double, C.c_size_t
     L.agnvar_workspace_bytes.restype = sz
@@ -66,7 +73,10 @@ def lib():
     L.agnvar_tk_generate.argtypes = [C.POINTER(agnvar_psd), i64, i64, i64, dbl, i32, i32, u64, u32, vp, vp, vp, sz,
                                      vp]
     L.agnvar_e13_iterate.restype = i32
-    L.agnvar_e13_iterate.argtypes = [i64, i64, i32, vp, vp, vp, vp, i32, vp, vp, vp, vp, sz, vp]
+    L.agnvar_e13_iterate.argtypes = [i64, i64, i32, vp, vp, vp, vp, i32, vp, vp, vp, C.POINTER(agnvar_e13_opts), vp, sz,
+                                     vp]
+    L.agnvar_erdf_table.restype = i32
+    L.agnvar_erdf_table.argtypes = [C.POINTER(agnvar_erdf), i64, i32, vp, vp]
     L.agnvar_periodogram.restype = i32
     L.agnvar_periodogram.argtypes = [i64, i64, i32, vp, dbl, i32, i32, C.POINTER(i64), vp, vp, vp, sz, vp]
     L.agnvar_philox_u32.restype = i32
@@ -83,6 +93,8 @@ def lib():
     L.agnvar_trace_end.argtypes = [i64, vp, vp, C.POINTER(i64)]
     L.agnvar_kernel_name.restype = C.c_char_p
     L.agnvar_kernel_name.argtypes = [i32]
+    if _build.source_hash().encode() not in L.agnvar_version():
+        raise RuntimeError("libagnvar.so does not match the sources in csrc/ (stale build)")
     _lib = L
     return L
 
@@ -131,6 +143,11 @@ def _stream():
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
 
 
+def _on(device):
+    """Make `device` current for the duration of a call: the library launches on the current device."""
+    return torch.cuda.device(torch.device(device))
+
+
 def _check(st, where):
     if st != 0:
         raise AgnvarError(st, where)
@@ -168,6 +185,8 @@ def workspace_bytes(op, B, N, dtype, oversample=1, aux=0):
 def workspace(nbytes, device=None):
     """A cached uint8 device tensor of at least nbytes (one per device; grown on demand)."""
     device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+    if device.index is None:
+        device = torch.device("cuda", torch.cuda.current_device())
     cur = _ws_cache.get(device)
     if cur is None or cur.numel() < nbytes:
         _ws_cache[device] = None
@@ -183,18 +202,29 @@ def free_workspace():
 # ---- the calls of include/agnvar.h ----------------------------------------------------------------
 def agnvar_philox_u32(seed, i0, n, curve, tag, device="cuda"):
     """O1: raw Philox4x32-10 words [n][4] (int32 tensor holding the u32 bit patterns)."""
-    out = torch.empty((n, 4), dtype=torch.int32, device=device)
-    _check(lib().agnvar_philox_u32(int(seed), int(i0), int(n), int(curve), int(tag), _ptr(out), _stream()),
-           "agnvar_philox_u32")
+    with _on(device):
+        out = torch.empty((n, 4), dtype=torch.int32, device=device)
+        _check(lib().agnvar_philox_u32(int(seed), int(i0), int(n), int(curve), int(tag), _ptr(out), _stream()),
+               "agnvar_philox_u32")
     return out
 
 
 def agnvar_psd_bpl(f, psd, out=None):
     """S0: Eq. 3 at the fp64 device tensor f. psd = (A, f_b, alpha_low, alpha_high)."""
     arr, _ = _psd_array(psd)
-    if out is None:
-        out = torch.empty_like(f)
-    _check(lib().agnvar_psd_bpl(_ptr(f), f.numel(), arr, _ptr(out), _stream()), "agnvar_psd_bpl")
+    with _on(f.device):
+        if out is None:
+            out = torch.empty_like(f)
+        _check(lib().agnvar_psd_bpl(_ptr(f), f.numel(), arr, _ptr(out), _stream()), "agnvar_psd_bpl")
+    return out
+
+
+def agnvar_erdf_table(erdf, grid_points=4096, device="cuda"):
+    """S1's normalised cumulative table(s) C [n_erdf][grid_points] fp64 (O4)."""
+    arr, n = _erdf_array(erdf)
+    with _on(device):
+        out = torch.empty((n, grid_points), dtype=torch.float64, device=device)
+        _check(lib().agnvar_erdf_table(arr, n, int(grid_points), _ptr(out), _stream()), "agnvar_erdf_table")
     return out
 
 
@@ -203,14 +233,15 @@ def agnvar_erdf_sample_sorted(erdf, B, N, dtype, seed, curve0=0, grid_points=409
     """S1: returns (sorted [B][N], perm0 [B][N] u32-as-int32 | None, draw [B][N] | None)."""
     code, tdt = _dt(dtype)
     arr, n = _erdf_array(erdf)
-    srt = torch.empty((B, N), dtype=tdt, device=device)
-    perm0 = torch.empty((B, N), dtype=torch.int32, device=device) if want_perm0 else None
-    draw = torch.empty((B, N), dtype=tdt, device=device) if want_draw else None
-    nb = workspace_bytes(OP_ERDF_SAMPLE_SORTED, B, N, code, 1, grid_points)
-    ws = workspace(nb, srt.device)
-    _check(lib().agnvar_erdf_sample_sorted(arr, n, B, N, code, int(seed), int(curve0), int(grid_points), _ptr(srt),
-                                           _ptr(perm0), _ptr(draw), _ptr(ws), ws.numel(), _stream()),
-           "agnvar_erdf_sample_sorted")
+    with _on(device):
+        srt = torch.empty((B, N), dtype=tdt, device=device)
+        perm0 = torch.empty((B, N), dtype=torch.int32, device=device) if want_perm0 else None
+        draw = torch.empty((B, N), dtype=tdt, device=device) if want_draw else None
+        nb = workspace_bytes(OP_ERDF_SAMPLE_SORTED, B, N, code, 1, grid_points)
+        ws = workspace(nb, srt.device)
+        _check(lib().agnvar_erdf_sample_sorted(arr, n, B, N, code, int(seed), int(curve0), int(grid_points), _ptr(srt),
+                                               _ptr(perm0), _ptr(draw), _ptr(ws), ws.numel(), _stream()),
+               "agnvar_erdf_sample_sorted")
     return srt, perm0, draw
 
 
@@ -219,34 +250,44 @@ def agnvar_tk_generate(psd, B, N, dt, oversample, dtype, seed, curve0=0, want_xn
     """S2: returns (x_norm [B][N] | None, A_norm [B][N/2+1] | None)."""
     code, tdt = _dt(dtype)
     arr, n = _psd_array(psd)
-    xn = torch.empty((B, N), dtype=tdt, device=device) if want_xnorm else None
-    an = torch.empty((B, N // 2 + 1), dtype=tdt, device=device) if want_anorm else None
-    nb = workspace_bytes(OP_TK_GENERATE, B, N, code, oversample, 0)
-    ws = workspace(nb, device)
-    _check(lib().agnvar_tk_generate(arr, n, B, N, float(dt), int(oversample), code, int(seed), int(curve0),
-                                    _ptr(xn), _ptr(an), _ptr(ws), ws.numel(), _stream()), "agnvar_tk_generate")
+    with _on(device):
+        xn = torch.empty((B, N), dtype=tdt, device=device) if want_xnorm else None
+        an = torch.empty((B, N // 2 + 1), dtype=tdt, device=device) if want_anorm else None
+        nb = workspace_bytes(OP_TK_GENERATE, B, N, code, oversample, 0)
+        ws = workspace(nb, (xn if xn is not None else an).device)
+        _check(lib().agnvar_tk_generate(arr, n, B, N, float(dt), int(oversample), code, int(seed), int(curve0),
+                                        _ptr(xn), _ptr(an), _ptr(ws), ws.numel(), _stream()), "agnvar_tk_generate")
     return xn, an
 
 
-def agnvar_e13_iterate(anorm, sorted_vals, perm, max_iter, x=None, want_hist=False, want_xadj=False):
+def agnvar_e13_iterate(anorm, sorted_vals, perm, max_iter, x=None, want_hist=False, want_xadj=False,
+                       delta_threshold=0.0, want_delta=False, want_fallbacks=False, check_every=0):
     """L1-L6. perm is updated IN PLACE (in: idx_old of the first iteration, out: final permutation).
-    Returns dict(x, perm, iters_used, changed_hist | None, x_adj | None)."""
+    delta_threshold > 0 adds the paper's stopping rule (Eq. 4); want_delta returns delta_k of every iteration.
+    Returns dict(x, perm, iters_used, changed_hist | None, x_adj | None, delta_hist | None, sort_fallbacks | None)."""
     B, N = sorted_vals.shape
     code, tdt = _dt(sorted_vals.dtype)
     dev = sorted_vals.device
     assert anorm.dtype == tdt and anorm.shape == (B, N // 2 + 1) and anorm.is_contiguous()
     assert perm.dtype == torch.int32 and perm.shape == (B, N) and perm.is_contiguous() and sorted_vals.is_contiguous()
-    if x is None:
-        x = torch.empty((B, N), dtype=tdt, device=dev)
-    iters = torch.empty((B,), dtype=torch.int32, device=dev)
-    hist = torch.empty((B, max_iter), dtype=torch.int64, device=dev) if want_hist else None
-    xadj = torch.empty((B, N), dtype=tdt, device=dev) if want_xadj else None
-    nb = workspace_bytes(OP_E13_ITERATE, B, N, code, 1, 0)
-    ws = workspace(nb, dev)
-    _check(lib().agnvar_e13_iterate(B, N, code, _ptr(anorm), _ptr(sorted_vals), _ptr(perm), _ptr(x), int(max_iter),
-                                    _ptr(iters), _ptr(hist), _ptr(xadj), _ptr(ws), ws.numel(), _stream()),
-           "agnvar_e13_iterate")
-    return {"x": x, "perm": perm, "iters_used": iters, "changed_hist": hist, "x_adj": xadj}
+    with _on(dev):
+        if x is None:
+            x = torch.empty((B, N), dtype=tdt, device=dev)
+        iters = torch.empty((B,), dtype=torch.int32, device=dev)
+        hist = torch.empty((B, max_iter), dtype=torch.int64, device=dev) if want_hist else None
+        xadj = torch.empty((B, N), dtype=tdt, device=dev) if want_xadj else None
+        dhist = torch.empty((B, max_iter), dtype=torch.float64, device=dev) if want_delta else None
+        fb = torch.empty((B,), dtype=torch.int32, device=dev) if want_fallbacks else None
+        delta_mode = want_delta or delta_threshold > 0.0
+        opts = agnvar_e13_opts(float(delta_threshold), dhist.data_ptr() if dhist is not None else None,
+                               fb.data_ptr() if fb is not None else None, int(check_every), 0)
+        nb = workspace_bytes(OP_E13_ITERATE, B, N, code, 1, 1 if delta_mode else 0)
+        ws = workspace(nb, dev)
+        _check(lib().agnvar_e13_iterate(B, N, code, _ptr(anorm), _ptr(sorted_vals), _ptr(perm), _ptr(x), int(max_iter),
+                                        _ptr(iters), _ptr(hist), _ptr(xadj), C.byref(opts), _ptr(ws), ws.numel(),
+                                        _stream()), "agnvar_e13_iterate")
+    return {"x": x, "perm": perm, "iters_used": iters, "changed_hist": hist, "x_adj": xadj, "delta_hist": dhist,
+            "sort_fallbacks": fb}
 
 
 def agnvar_periodogram(x, dt, norm=0, bin_edges=None):
@@ -255,11 +296,12 @@ def agnvar_periodogram(x, dt, norm=0, bin_edges=None):
     code, _ = _dt(x.dtype)
     dev = x.device
     nbins = 0 if bin_edges is None else len(bin_edges) - 1
-    out = torch.empty((B, nbins if nbins else N // 2), dtype=torch.float64, device=dev)
-    counts = torch.empty((nbins,), dtype=torch.int64, device=dev) if nbins else None
-    edges = (C.c_int64 * (nbins + 1))(*[int(e) for e in bin_edges]) if nbins else None
-    nb = workspace_bytes(OP_PERIODOGRAM, B, N, code, 1, nbins)
-    ws = workspace(nb, dev)
-    _check(lib().agnvar_periodogram(B, N, code, _ptr(x), float(dt), int(norm), nbins, edges, _ptr(out), _ptr(counts),
-                                    _ptr(ws), ws.numel(), _stream()), "agnvar_periodogram")
+    with _on(dev):
+        out = torch.empty((B, nbins if nbins else N // 2), dtype=torch.float64, device=dev)
+        counts = torch.empty((nbins,), dtype=torch.int64, device=dev) if nbins else None
+        edges = (C.c_int64 * (nbins + 1))(*[int(e) for e in bin_edges]) if nbins else None
+        nb = workspace_bytes(OP_PERIODOGRAM, B, N, code, 1, nbins)
+        ws = workspace(nb, dev)
+        _check(lib().agnvar_periodogram(B, N, code, _ptr(x), float(dt), int(norm), nbins, edges, _ptr(out), _ptr(counts),
+                                        _ptr(ws), ws.numel(), _stream()), "agnvar_periodogram")
     return out if not nbins else (out, counts)

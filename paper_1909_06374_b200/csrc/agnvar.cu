@@ -37,14 +37,10 @@ inline bool valid_dtype(int d) { return d == AGNVAR_F32 || d == AGNVAR_F64; }
 inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
 inline bool valid_oversample(int o) { return o == 1 || o == 2 || o == 4 || o == 8 || o == 10 || o == 16 || o == 20; }
 
-bool g_attrs_done[16] = {false};
 template <typename T> cudaError_t ensure_attrs() {
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    int slot = (dev & 7) * 2 + (sizeof(T) == 8 ? 1 : 0);
-    if (g_attrs_done[slot]) return cudaSuccess;
-    e = fft_set_attrs<T>();
+    bool& done = dev_cache().attrs[sizeof(T) == 8 ? 1 : 0];
+    if (done) return cudaSuccess;
+    cudaError_t e = fft_set_attrs<T>();
     if (e != cudaSuccess) return e;
     e = sort_set_attrs<T>();
     if (e != cudaSuccess) return e;
@@ -54,7 +50,7 @@ template <typename T> cudaError_t ensure_attrs() {
         e = sort32_set_attrs();
         if (e != cudaSuccess) return e;
     }
-    g_attrs_done[slot] = true;
+    done = true;
     return cudaSuccess;
 }
 
@@ -66,7 +62,8 @@ template <typename T> size_t sort_ws_any(int64_t B, int64_t N) {
     if (sort32_applicable(sizeof(T), N)) s = std::max(s, sort32_ws_bytes(B, N));
     return s;
 }
-template <typename T> size_t ws_e13(int64_t B, int64_t N) {
+inline int delta_chunks(int64_t N) { return (int)((N + kDeltaChunk - 1) / kDeltaChunk); }
+template <typename T> size_t ws_e13(int64_t B, int64_t N, bool delta) {
     typedef typename Cx<T>::type C;
     Carver c(nullptr);
     c.take<C>(std::max(FftPlan<T>::table_elems(), Fft2Plan<T>::table_elems()));
@@ -75,8 +72,14 @@ template <typename T> size_t ws_e13(int64_t B, int64_t N) {
     c.take<T>((size_t)B * (N / 2 + kApPad));  // A_norm in position order
     c.take<uint32_t>((size_t)B * N);          // permutation ping-pong
     c.take<unsigned long long>((size_t)B);    // changed counters
-    c.take<int>((size_t)B);                   // first_zero
+    c.take<int>((size_t)B + 1);               // first_stop [B], n_stopped
     c.take<uint32_t>((size_t)B * kRadix);     // bin cursors of the two-level scatter
+    if (delta) {
+        c.take<T>((size_t)B * N);             // x_sim ping
+        c.take<T>((size_t)B * N);             // x_sim pong
+        c.take<uint32_t>((size_t)B * N);      // second working permutation (d_perm is output only)
+        c.take<double>((size_t)B * delta_chunks(N));
+    }
     return c.off + sort_ws_any<T>(B, N);
 }
 template <typename T> size_t ws_tk(int64_t B, int64_t N, int os) {
@@ -112,6 +115,8 @@ template <typename T> size_t ws_pgram(int64_t B, int64_t N, int64_t nbins) {
 }
 
 inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? AGNVAR_OK : AGNVAR_ECUDA; }
+// CUDA runtime call inside an int-returning implementation: a failure is AGNVAR_ECUDA
+#define CK(call) do { if ((call) != cudaSuccess) return AGNVAR_ECUDA; } while (0)
 
 // real forward FFT of B series of length N held in `Z` (in place, viewed as [B][N/2] complex);
 // result in position order.
@@ -122,12 +127,21 @@ template <typename T> void rfft_inplace(const FftPlan<T>& p, T* Z, int64_t B, cu
 }
 
 // ---- E13 -------------------------------------------------------------------------------------------
+struct E13Opts {
+    double delta_threshold = 0.0;
+    double* d_delta_hist = nullptr;
+    int32_t* d_sort_fallbacks = nullptr;
+    int check_every = 0;
+    bool delta() const { return delta_threshold > 0.0 || d_delta_hist != nullptr; }
+};
+
 template <typename T>
 int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, uint32_t* d_perm, void* d_x,
-             int max_iter, int32_t* d_iters_used, int64_t* d_changed_hist, void* d_xadj_dbg, void* d_ws,
-             size_t ws_bytes, cudaStream_t st) {
+             int max_iter, int32_t* d_iters_used, int64_t* d_changed_hist, void* d_xadj_dbg, const E13Opts& opt,
+             void* d_ws, size_t ws_bytes, cudaStream_t st) {
     typedef typename Cx<T>::type C;
-    if (ws_bytes < ws_e13<T>(B, N) || !d_ws || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
+    const bool dmode = opt.delta();
+    if (ws_bytes < ws_e13<T>(B, N, dmode) || !d_ws || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
     if (ensure_attrs<T>() != cudaSuccess) return AGNVAR_ECUDA;
     const int logL = ilog2_u64((uint64_t)N) - 1;
     const long long L = N / 2;
@@ -138,14 +152,24 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
     T* Ap = c.take<T>((size_t)B * (N / 2 + kApPad));
     uint32_t* P1 = c.take<uint32_t>((size_t)B * N);
     unsigned long long* changed = c.take<unsigned long long>((size_t)B);
-    int* first_zero = c.take<int>((size_t)B);
+    int* first_stop = c.take<int>((size_t)B + 1);
+    unsigned int* n_stopped = (unsigned int*)(first_stop + B);
     uint32_t* cursor = c.take<uint32_t>((size_t)B * kRadix);
+    T *XA = nullptr, *XB = nullptr;
+    uint32_t* P0 = nullptr;
+    double* dpartial = nullptr;
+    const int nch = delta_chunks(N);
+    if (dmode) {
+        XA = c.take<T>((size_t)B * N);
+        XB = c.take<T>((size_t)B * N);
+        P0 = c.take<uint32_t>((size_t)B * N);
+        dpartial = c.take<double>((size_t)B * nch);
+    }
     void* sort_ws = (unsigned char*)d_ws + c.off;
     const bool two_level = N >= (1ll << kTwoLevelScatterLog);
     // the binned (value, dst) pairs live in the sort's ping-pong buffers, which are idle after the sort
     T* pv = (T*)sort_ws;
     uint32_t* pd = (uint32_t*)((unsigned char*)sort_ws + 2 * align_up((size_t)B * N * sizeof(T), 256));
-    T* x = (T*)d_x;
     const T* sorted = (const T*)d_sorted;
 
     // long fp32 curves: column sub-passes in registers + fused mid kernel (fft2.cuh); otherwise the generic passes
@@ -162,25 +186,45 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
         plan = fft_plan_init<T>(logL, tables, st);
         rlv = real_level<T>(plan);
     }
-    cudaMemsetAsync(changed, 0, (size_t)B * sizeof(unsigned long long), st);
-    cudaMemsetAsync(first_zero, 0, (size_t)B * sizeof(int), st);
-    cudaMemsetAsync(cursor, 0, (size_t)B * kRadix * sizeof(uint32_t), st);
+    CK(cudaMemsetAsync(changed, 0, (size_t)B * sizeof(unsigned long long), st));
+    CK(cudaMemsetAsync(first_stop, 0, ((size_t)B + 1) * sizeof(int), st));
+    CK(cudaMemsetAsync(cursor, 0, (size_t)B * kRadix * sizeof(uint32_t), st));
+    if (opt.d_sort_fallbacks) CK(cudaMemsetAsync(opt.d_sort_fallbacks, 0, (size_t)B * sizeof(int32_t), st));
+    if (opt.d_delta_hist) CK(cudaMemsetAsync(opt.d_delta_hist, 0, (size_t)B * max_iter * sizeof(double), st));
     AGN_LAUNCH(K_PERM_ANORM, st, (perm_anorm_kernel<T><<<bgrid(cdiv(L + 1, 256), B), 256, 0, st>>>((const T*)d_anorm, Ap, plan.dg, (int)B)));
     const unsigned sg = (unsigned)std::min<long long>((N + 1023) / 1024, 148 * 16);
-    // first x_sim: the draw in draw order (Q15)
-    bool first_done = false;
-    if constexpr (sizeof(T) == 4) {
-        if (two_level && sort32_applicable(sizeof(T), N)) {
-            // same two-level scatter as in the loop (idx_old = idx_new: the change count stays 0)
-            if (rank_scatter_two_level32(d_perm, d_perm, sorted, x, B, N, (uint2*)sort_ws, cursor, changed, st) != cudaSuccess)
-                return AGNVAR_ECUDA;
-            first_done = true;
-        }
-    }
-    if (!first_done)
-        AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, false><<<bgrid(sg, B), 256, 0, st>>>(d_perm, nullptr, sorted, x, N, nullptr, (int)B)));
+    // working buffers: x_sim in the caller's d_x and the permutations in (d_perm, P1) -- or, when delta_k is wanted,
+    // everything in the workspace (x_sim,k and x_sim,k+1 must both exist, and a stopped curve's state is copied out
+    // while the batch goes on)
     uint32_t* cur = d_perm;
     uint32_t* nxt = P1;
+    T* x = (T*)d_x;
+    T* xn = (T*)d_x;
+    if (dmode) {
+        CK(cudaMemcpyAsync(P0, d_perm, (size_t)B * N * 4, cudaMemcpyDeviceToDevice, st));
+        cur = P0; x = XA; xn = XB;
+    }
+    auto rank_scatter = [&](const uint32_t* inew, const uint32_t* iold, T* xout, void* spare, bool count) -> int {
+        if constexpr (sizeof(T) == 4) {
+            if (two_level && sort32_applicable(sizeof(T), N)) {
+                if (rank_scatter_two_level32(inew, iold, sorted, xout, B, N, (uint2*)spare, cursor, changed, st) != cudaSuccess)
+                    return AGNVAR_ECUDA;
+                return AGNVAR_OK;
+            }
+        }
+        if (two_level) {
+            if (rank_scatter_two_level<T>(inew, iold, sorted, xout, B, N, pv, pd, cursor, changed, st) != cudaSuccess)
+                return AGNVAR_ECUDA;
+        } else if (count) {
+            AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(inew, iold, sorted, xout, N, changed, (int)B)));
+        } else {
+            AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, false><<<bgrid(sg, B), 256, 0, st>>>(inew, nullptr, sorted, xout, N, nullptr, (int)B)));
+        }
+        return AGNVAR_OK;
+    };
+    // first x_sim: the draw in draw order (Q15); idx_old = idx_new, so the change count stays 0
+    if (int rc = rank_scatter(cur, cur, x, sort_ws, false)) return rc;
+    int k_done = 0;
     for (int k = 1; k <= max_iter; ++k) {
         if constexpr (sizeof(T) == 4) if (use2) {
             // L1 column sub-passes (x_sim -> Z), then rows: forward FFT + L2 amplitude replace + inverse FFT
@@ -198,42 +242,53 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
             // L3 inverse FFT (Z -> x_adj, natural order, 1/L)
             fft_inverse<T>(plan, (const C*)Z, (C*)Z, L, L, (int)B, (T)(1.0 / (double)L), st);
         }
-        // L4 segmented stable argsort, L5 rank scatter + change count
-        bool done45 = false;
+        // L4 segmented stable argsort
+        void* spare = sort_ws;
+        const uint32_t* sort_gate = nullptr;       // per-curve "took the LSD fallback" flags of this iteration
+        bool sorted_here = false;
         if constexpr (sizeof(T) == 4) {
             if (sort32_applicable(sizeof(T), N)) {
-                uint2* spare = nullptr;
-                // the CDF tables are re-estimated in every iteration: reusing them for 3 out of 4 iterations was measured to
-                // overflow slabs (stale table -> LSD fallback) often enough to cost more than the 0.25 ms it saves
-                const bool reuse_cdf = false;
-                if (seg_argsort32(Z, nxt, nullptr, B, N, sort_ws, &spare, st, reuse_cdf) != cudaSuccess) return AGNVAR_ECUDA;
-                if (two_level) {
-                    if (rank_scatter_two_level32(nxt, cur, sorted, x, B, N, spare, cursor, changed, st) != cudaSuccess)
-                        return AGNVAR_ECUDA;
-                } else {
-                    AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(nxt, cur, sorted, x, N, changed, (int)B)));
-                }
-                done45 = true;
+                uint2* sp = nullptr;
+                if (seg_argsort32(Z, nxt, nullptr, B, N, sort_ws, &sp, st, &sort_gate) != cudaSuccess) return AGNVAR_ECUDA;
+                spare = sp;
+                sorted_here = true;
             }
         }
-        if (!done45) {
-        cudaError_t e = seg_argsort<T>(Z, nxt, nullptr, B, N, sort_ws, st);
-        if (e != cudaSuccess) return AGNVAR_ECUDA;
-        if (two_level) {
-            if (rank_scatter_two_level<T>(nxt, cur, sorted, x, B, N, pv, pd, cursor, changed, st) != cudaSuccess)
-                return AGNVAR_ECUDA;
-        } else {
-            AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(nxt, cur, sorted, x, N, changed, (int)B)));
-        }
-        }
+        if (!sorted_here && seg_argsort<T>(Z, nxt, nullptr, B, N, sort_ws, st) != cudaSuccess) return AGNVAR_ECUDA;
+        // L5 rank scatter + change count
+        if (int rc = rank_scatter(nxt, cur, xn, spare, true)) return rc;
+        // delta_k (Eq. 4) between x_sim,k (x) and x_sim,k+1 (xn)
+        if (dmode)
+            AGN_LAUNCH(K_DELTA, st, (delta_partial_kernel<T><<<bgrid((unsigned)nch, B), 256, 0, st>>>(x, xn, N, dpartial, nch, (int)B)));
         // L6 bookkeeping
-        AGN_LAUNCH(K_ITER_POST, st, (post_iter_kernel<<<cdiv(B, 256), 256, 0, st>>>(changed, first_zero, k, (long long*)d_changed_hist, max_iter, (int)B)));
+        PostArgs pa;
+        pa.changed = changed; pa.first_stop = first_stop; pa.hist = (long long*)d_changed_hist;
+        pa.partial = dpartial; pa.delta_hist = opt.d_delta_hist; pa.threshold = opt.delta_threshold;
+        pa.N = N; pa.nchunks = nch; pa.k = k; pa.max_iter = max_iter; pa.n_stopped = n_stopped;
+        pa.overflow = sort_gate; pa.fallbacks = opt.d_sort_fallbacks;
+        AGN_LAUNCH(K_ITER_POST, st, (post_iter_kernel<<<(unsigned)B, 256, 0, st>>>(pa)));
+        if (dmode) {
+            // curves that stopped in this iteration: their state goes out now (the batch keeps iterating them)
+            AGN_LAUNCH(K_COPY, st, (snapshot_kernel<T><<<bgrid(cdiv(N, 4096), B), 256, 0, st>>>(first_stop, k, xn, nxt, (T*)d_x, d_perm, N, (int)B)));
+            std::swap(x, xn);
+        }
         std::swap(cur, nxt);
+        k_done = k;
+        if (opt.check_every > 0 && k % opt.check_every == 0 && k < max_iter) {
+            unsigned int h_stopped = 0;
+            if (cudaStreamSynchronize(st) != cudaSuccess) return AGNVAR_ECUDA;
+            if (cudaMemcpy(&h_stopped, n_stopped, sizeof(unsigned int), cudaMemcpyDeviceToHost) != cudaSuccess) return AGNVAR_ECUDA;
+            if ((int64_t)h_stopped >= B) break;
+        }
     }
-    if (cur != d_perm) cudaMemcpyAsync(d_perm, cur, (size_t)B * N * 4, cudaMemcpyDeviceToDevice, st);
+    if (dmode) {
+        AGN_LAUNCH(K_COPY, st, (snapshot_kernel<T><<<bgrid(cdiv(N, 4096), B), 256, 0, st>>>(first_stop, 0, x, cur, (T*)d_x, d_perm, N, (int)B)));
+    } else if (cur != d_perm) {
+        CK(cudaMemcpyAsync(d_perm, cur, (size_t)B * N * 4, cudaMemcpyDeviceToDevice, st));
+    }
     if (d_xadj_dbg)
         AGN_LAUNCH(K_COPY, st, (copy_canon_kernel<T><<<cdiv(B * N, 256), 256, 0, st>>>(Z, (T*)d_xadj_dbg, (long long)B * N)));
-    if (d_iters_used) AGN_LAUNCH(K_ITER_POST, st, (finalize_iters_kernel<<<cdiv(B, 256), 256, 0, st>>>(first_zero, d_iters_used, max_iter, (int)B)));
+    if (d_iters_used) AGN_LAUNCH(K_ITER_POST, st, (finalize_iters_kernel<<<cdiv(B, 256), 256, 0, st>>>(first_stop, d_iters_used, k_done, (int)B)));
     return cuda_status(cudaGetLastError());
 }
 
@@ -293,7 +348,7 @@ int tk_impl(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_t N, double
             xsrc = xn;
         }
     }
-    if (d_xnorm) cudaMemcpyAsync(d_xnorm, xsrc, (size_t)B * N * sizeof(T), cudaMemcpyDeviceToDevice, st);
+    if (d_xnorm) CK(cudaMemcpyAsync(d_xnorm, xsrc, (size_t)B * N * sizeof(T), cudaMemcpyDeviceToDevice, st));
     if (d_anorm) {
         const int logL = ilog2_u64((uint64_t)N) - 1;
         const long long L = N / 2;
@@ -390,7 +445,10 @@ const char* agnvar_strerror(int status) {
     }
 }
 
-const char* agnvar_version(void) { return "agnvar 0.1 (sm_100a)"; }
+#ifndef AGNVAR_SRC_HASH
+#define AGNVAR_SRC_HASH "unknown"
+#endif
+const char* agnvar_version(void) { return "agnvar 0.2 (sm_100a) src:" AGNVAR_SRC_HASH; }
 
 uint64_t agnvar_launch_count(void) { return trace_state().launches; }
 
@@ -428,7 +486,7 @@ size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int overs
     if (!valid_BN(B, N) || !valid_dtype(dtype)) return 0;
     const bool f32 = dtype == AGNVAR_F32;
     switch (op) {
-        case AGNVAR_OP_E13_ITERATE: return f32 ? ws_e13<float>(B, N) : ws_e13<double>(B, N);
+        case AGNVAR_OP_E13_ITERATE: return f32 ? ws_e13<float>(B, N, aux != 0) : ws_e13<double>(B, N, aux != 0);
         case AGNVAR_OP_TK_GENERATE:
             if (!valid_oversample(oversample) || N * (int64_t)oversample > ((int64_t)1 << 28)) return 0;
             return f32 ? ws_tk<float>(B, N, oversample) : ws_tk<double>(B, N, oversample);
@@ -464,23 +522,47 @@ int agnvar_psd_bpl(const double* d_f, int64_t n, const agnvar_psd* h_p, double* 
     return cuda_status(cudaGetLastError());
 }
 
+static bool valid_erdf(const agnvar_erdf* h_erdf, int64_t n_erdf) {
+    for (int64_t i = 0; i < n_erdf; ++i) {
+        const agnvar_erdf& e = h_erdf[i];
+        if (e.kind != AGNVAR_ERDF_BPL && e.kind != AGNVAR_ERDF_LOGNORMAL) return false;
+        if (!std::isfinite(e.lam_min) || !std::isfinite(e.lam_max) || !(e.lam_min > 0.0) || !(e.lam_min < e.lam_max))
+            return false;
+        if (e.kind == AGNVAR_ERDF_BPL) {
+            if (!std::isfinite(e.lam_star) || !(e.lam_star > 0.0) || !std::isfinite(e.delta1) || !std::isfinite(e.delta2))
+                return false;
+        } else {
+            if (!std::isfinite(e.mu_log10) || !std::isfinite(e.sigma_log10) || !(e.sigma_log10 > 0.0)) return false;
+        }
+    }
+    return true;
+}
+
+int agnvar_erdf_table(const agnvar_erdf* h_erdf, int64_t n_erdf, int grid_points, double* d_out, void* stream) {
+    if (!h_erdf || n_erdf < 1 || n_erdf > ((int64_t)1 << 30) || grid_points < 2 || grid_points > 65536 || !d_out)
+        return AGNVAR_EINVAL;
+    if (!valid_erdf(h_erdf, n_erdf)) return AGNVAR_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    // the parameter structs travel as kernel arguments, kErdfArgBatch tables per launch: no device scratch is needed
+    for (int64_t i0 = 0; i0 < n_erdf; i0 += kErdfArgBatch) {
+        ErdfBatch eb;
+        const int n = (int)std::min<int64_t>(kErdfArgBatch, n_erdf - i0);
+        for (int i = 0; i < n; ++i) {
+            const agnvar_erdf& e = h_erdf[i0 + i];
+            eb.e[i] = ErdfDev{e.kind, 0, e.lam_star, e.delta1, e.delta2, e.mu_log10, e.sigma_log10,
+                              std::log10(e.lam_min), std::log10(e.lam_max)};
+        }
+        AGN_LAUNCH(K_ERDF_TABLE, st, (erdf_table_args_kernel<<<(unsigned)n, 256, 0, st>>>(eb, grid_points, d_out + (size_t)i0 * grid_points)));
+    }
+    return cuda_status(cudaGetLastError());
+}
+
 int agnvar_erdf_sample_sorted(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t B, int64_t N, int dtype,
                               uint64_t seed, uint32_t curve0, int grid_points, void* d_sorted, uint32_t* d_perm0,
                               void* d_draw, void* d_ws, size_t ws_bytes, void* stream) {
     if (!valid_BN(B, N) || !valid_dtype(dtype) || !h_erdf || !d_sorted) return AGNVAR_EINVAL;
     if (!(n_erdf == 1 || n_erdf == B) || grid_points < 2 || grid_points > 65536) return AGNVAR_EINVAL;
-    for (int64_t i = 0; i < n_erdf; ++i) {
-        const agnvar_erdf& e = h_erdf[i];
-        if (e.kind != AGNVAR_ERDF_BPL && e.kind != AGNVAR_ERDF_LOGNORMAL) return AGNVAR_EINVAL;
-        if (!std::isfinite(e.lam_min) || !std::isfinite(e.lam_max) || !(e.lam_min > 0.0) || !(e.lam_min < e.lam_max))
-            return AGNVAR_EINVAL;
-        if (e.kind == AGNVAR_ERDF_BPL) {
-            if (!std::isfinite(e.lam_star) || !(e.lam_star > 0.0) || !std::isfinite(e.delta1) || !std::isfinite(e.delta2))
-                return AGNVAR_EINVAL;
-        } else {
-            if (!std::isfinite(e.mu_log10) || !std::isfinite(e.sigma_log10) || !(e.sigma_log10 > 0.0)) return AGNVAR_EINVAL;
-        }
-    }
+    if (!valid_erdf(h_erdf, n_erdf)) return AGNVAR_EINVAL;
     size_t need = agnvar_workspace_bytes(AGNVAR_OP_ERDF_SAMPLE_SORTED, B, N, dtype, 1, grid_points);
     if (!d_ws || ws_bytes < need || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
     const size_t tail = align_up((size_t)B * N * 4, 256);
@@ -514,15 +596,23 @@ int agnvar_tk_generate(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_
 
 int agnvar_e13_iterate(int64_t B, int64_t N, int dtype, const void* d_anorm, const void* d_sorted, uint32_t* d_perm,
                        void* d_x, int max_iter, int32_t* d_iters_used, int64_t* d_changed_hist, void* d_xadj_dbg,
-                       void* d_ws, size_t ws_bytes, void* stream) {
+                       const agnvar_e13_opts* h_opts, void* d_ws, size_t ws_bytes, void* stream) {
     if (!valid_BN(B, N) || !valid_dtype(dtype) || max_iter < 1) return AGNVAR_EINVAL;
     if (!d_anorm || !d_sorted || !d_perm || !d_x) return AGNVAR_EINVAL;
     if (!aligned(d_perm, 16) || !aligned(d_x, 16) || !aligned(d_sorted, 16)) return AGNVAR_EINVAL;
+    E13Opts opt;
+    if (h_opts) {
+        if (!std::isfinite(h_opts->delta_threshold) || h_opts->check_every < 0) return AGNVAR_EINVAL;
+        opt.delta_threshold = h_opts->delta_threshold > 0.0 ? h_opts->delta_threshold : 0.0;
+        opt.d_delta_hist = h_opts->d_delta_hist;
+        opt.d_sort_fallbacks = h_opts->d_sort_fallbacks;
+        opt.check_every = h_opts->check_every;
+    }
     if (dtype == AGNVAR_F32)
         return e13_impl<float>(B, N, d_anorm, d_sorted, d_perm, d_x, max_iter, d_iters_used, d_changed_hist,
-                               d_xadj_dbg, d_ws, ws_bytes, (cudaStream_t)stream);
+                               d_xadj_dbg, opt, d_ws, ws_bytes, (cudaStream_t)stream);
     return e13_impl<double>(B, N, d_anorm, d_sorted, d_perm, d_x, max_iter, d_iters_used, d_changed_hist, d_xadj_dbg,
-                            d_ws, ws_bytes, (cudaStream_t)stream);
+                            opt, d_ws, ws_bytes, (cudaStream_t)stream);
 }
 
 int agnvar_periodogram(int64_t B, int64_t N, int dtype, const void* d_x, double dt, int norm, int nbins,

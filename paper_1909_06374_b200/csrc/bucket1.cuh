@@ -1,0 +1,322 @@
+// bucket1.cuh -- L4 for long fp32 curves (2^18 <= N <= 2^26) as a ONE-LEVEL distribution sort: every key goes straight
+// from x_adj to its equal-depth bucket (mean 8192 keys), and one CTA finishes a bucket in shared memory.
+//
+//   cdf_sample / cdf_table / bucket_bounds / bucket_base   as in bucket32.cuh (sampled piecewise-linear CDF of the keys)
+//   part1_kernel         x_adj tile of 8192 keys -> (key, time index) pairs in the bucket slabs.  A tile counts its keys
+//                        per bucket in shared memory (one 32-bit atomic per key), orders the tile by bucket in shared
+//                        memory, reserves one range per non-empty (tile, bucket) with one global atomic and writes the
+//                        runs out.  A light curve with a red PSD is smooth: the 8192 consecutive samples of a tile fall
+//                        into ~15 % of the buckets, so a run is ~6-13 pairs (50-100 bytes).  For keys with no such
+//                        locality (the i.i.d. ERDF draw that S1 sorts once per call) runs shrink to single pairs: still
+//                        exact, slower; it is not the loop's case.
+//   bucket1_sort_kernel  one CTA per bucket (slab of <= 12288 pairs, 96 KB of shared memory): counting sort into 8192
+//                        interpolation slots (linear map of the key onto the bucket's key interval; 16-bit counters packed
+//                        two per word), then the exact rank of every pair among its few slot mates by comparing the 64-bit
+//                        (key, index) words; indices written at their ranks.
+//
+// HBM bytes per sample: 0.5 (sample) + 12 (partition: 4 in, 8 out) + 12 (finish: 8 in, 4 out) = 24.5 -- below the
+// 28 of SURVEY 8(d)'s two-level model (which assumed a separate histogram read), against 40.5 for the two partition
+// levels of bucket32.cuh.  Same exactness argument as there: the order inside a slab is arbitrary, the final order is
+// defined by the (key, index) comparison alone, equal keys come out by ascending time index (O6 step 4).
+// A slab that would overflow raises the curve's `overflow` flag and the LSD passes of sort32.cuh sort that curve.
+#pragma once
+#include "common.cuh"
+#include "sort.cuh"
+#include "bucket32.cuh"
+
+namespace agn {
+
+constexpr int kB1MeanLog = 13;                    // mean bucket population 2^13
+constexpr int kB1Cap = 12288;                     // slab slots per bucket (1.5 x the mean: 5.6 sigma of the sampling noise)
+constexpr int kB1SlotLog = 13;
+constexpr int kB1Slots = 1 << kB1SlotLog;         // interpolation slots of the in-CTA sort
+constexpr int kB1MaxBuckets = 8192;               // N <= 2^26
+constexpr int kB1PartThreads = 512;
+constexpr int kB1PartEpt = 16;
+constexpr int kB1Tile = kB1PartThreads * kB1PartEpt;      // 8192 keys
+constexpr int kB1SortThreads = 1024;
+
+inline bool bucket1_applicable(size_t elem_size, long long N) {
+    return elem_size == 4 && N >= (1ll << 18) && N <= ((long long)kB1MaxBuckets << kB1MeanLog);
+}
+inline uint32_t bucket1_magic(uint32_t nb) {
+    return (uint32_t)((((unsigned __int128)nb) << (32 + kB1SlotLog + 9)) / (kBkTotalW << 16));
+}
+
+struct Part1Args {
+    const float* vals;          // [B][N]
+    uint2* out;                 // slabs [B][nb][kB1Cap]
+    uint32_t* cursor;           // [B][nb] zero on entry
+    uint32_t* overflow;         // [B]
+    const uint2* tab;           // [B][65536]
+    uint32_t N, nb, M;
+    long long B;
+};
+
+// shared memory: stage uint2[kB1Tile] | cnt u32[nb] (populations -> first stage position -> slab offset of stage position 0)
+inline size_t part1_smem(uint32_t nb) { return (size_t)kB1Tile * sizeof(uint2) + (size_t)nb * 4 + 64 * 4; }
+
+__global__ void __launch_bounds__(kB1PartThreads, 2) part1_kernel(Part1Args a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint2* stage = reinterpret_cast<uint2*>(smem_raw);
+    uint32_t* cnt = reinterpret_cast<uint32_t*>(smem_raw + (size_t)kB1Tile * sizeof(uint2));
+    uint32_t* wsum = cnt + a.nb;
+    const long long b = bidx();
+    if (b >= a.B) return;
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    const uint2* tab = a.tab + (size_t)b * kBkBins;
+    const uint32_t nb = a.nb;
+    for (uint32_t i = t; i < nb; i += kB1PartThreads) cnt[i] = 0u;
+    const uint32_t tile0 = blockIdx.x * kB1Tile;
+    const float* v = a.vals + (size_t)b * a.N + tile0;
+    uint32_t key[kB1PartEpt];
+#pragma unroll
+    for (int j = 0; j < kB1PartEpt; ++j) key[j] = key_of(__ldcs(v + j * kB1PartThreads + t));
+    __syncthreads();
+    // bucket and arrival number inside the (tile, bucket) run
+    uint32_t dr[kB1PartEpt];            // bucket << 14 | arrival number  (bucket < 2^13, arrival < 2^13)
+#pragma unroll
+    for (int j = 0; j < kB1PartEpt; ++j) {
+        const uint32_t d = min(bs_of(key[j], tab, a.M) >> kB1SlotLog, nb - 1u);
+        dr[j] = (d << 14) | atomicAdd(&cnt[d], 1u);
+    }
+    __syncthreads();
+    // exclusive scan of the populations, in place: thread t owns the buckets [t * per, (t + 1) * per)
+    constexpr int MAXPER = kB1MaxBuckets / kB1PartThreads;      // 16
+    const uint32_t per = (nb + kB1PartThreads - 1) / kB1PartThreads;
+    const uint32_t d0 = t * per;
+    uint32_t sum = 0;
+#pragma unroll
+    for (int i = 0; i < MAXPER; ++i)
+        if ((uint32_t)i < per && d0 + i < nb) sum += cnt[d0 + i];
+    uint32_t inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t m = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += m;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    uint32_t run = inc - sum;
+#pragma unroll
+    for (int w = 0; w < kB1PartThreads / 32; ++w) run += (w < warp) ? wsum[w] : 0u;
+#pragma unroll
+    for (int i = 0; i < MAXPER; ++i)
+        if ((uint32_t)i < per && d0 + i < nb) { const uint32_t c = cnt[d0 + i]; cnt[d0 + i] = run; run += c; }
+    __syncthreads();
+    // the tile ordered by bucket; an element carries its bucket and its position in the tile (the time index follows)
+#pragma unroll
+    for (int j = 0; j < kB1PartEpt; ++j) {
+        const uint32_t d = dr[j] >> 14;
+        stage[cnt[d] + (dr[j] & 0x3fffu)] = make_uint2(key[j], (d << 13) | (uint32_t)(j * kB1PartThreads + t));
+    }
+    __syncthreads();
+    // one global reservation per non-empty (tile, bucket); cnt[d] becomes (slab offset of the run) - (its stage position)
+    {
+        uint32_t st0[MAXPER + 1];       // stage starts of the own buckets and of the one after them
+#pragma unroll
+        for (int i = 0; i <= MAXPER; ++i) {
+            const uint32_t d = d0 + i;
+            st0[i] = ((uint32_t)i <= per && d <= nb) ? (d < nb ? cnt[d] : (uint32_t)kB1Tile) : 0u;
+        }
+        __syncthreads();
+        uint32_t* cur = a.cursor + (size_t)b * nb;
+#pragma unroll
+        for (int i = 0; i < MAXPER; ++i) {
+            const uint32_t d = d0 + i;
+            if ((uint32_t)i < per && d < nb) {
+                const uint32_t c = st0[i + 1] - st0[i];
+                if (c) {
+                    const uint32_t g = atomicAdd(&cur[d], c);
+                    if (g + c > (uint32_t)kB1Cap) a.overflow[b] = 1u;
+                    cnt[d] = g - st0[i];
+                }
+            }
+        }
+    }
+    __syncthreads();
+    uint2* out = a.out + (size_t)b * nb * kB1Cap;
+#pragma unroll 4
+    for (int s = t; s < kB1Tile; s += kB1PartThreads) {
+        const uint2 e = stage[s];
+        const uint32_t d = e.y >> 13;
+        const uint32_t off = cnt[d] + (uint32_t)s;
+        if (off < (uint32_t)kB1Cap) out[(size_t)d * kB1Cap + off] = make_uint2(e.x, tile0 + (e.y & 0x1fffu));
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// finish: one CTA per bucket
+// ------------------------------------------------------------------------------------------------
+struct B1Smem {
+    unsigned long long pair[kB1Cap];      // (key << 32) | index, grouped by slot
+    uint32_t cw[kB1Slots / 2];            // two 16-bit counters per word: populations, then starts, then ends of the slots
+    uint32_t wsum[kB1SortThreads / 32];
+};
+
+__global__ void __launch_bounds__(kB1SortThreads, 2) bucket1_sort_kernel(const uint2* __restrict__ slabs,
+                                                                         const uint32_t* __restrict__ cursor,
+                                                                         const uint32_t* __restrict__ base,
+                                                                         const uint32_t* __restrict__ overflow,
+                                                                         const uint32_t* __restrict__ klos,
+                                                                         uint32_t* __restrict__ idx_out,
+                                                                         float* __restrict__ sorted_out, uint32_t N,
+                                                                         uint32_t nb, long long B) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    B1Smem& sm = *reinterpret_cast<B1Smem*>(smem_raw);
+    const long long b = bidx();
+    if (b >= B) return;
+    if (overflow[b]) return;                       // this curve is sorted by the LSD passes instead
+    const uint32_t bk = blockIdx.x;
+    const uint32_t n = cursor[(size_t)b * nb + bk];          // <= kB1Cap (no overflow)
+    if (n == 0) return;
+    const uint32_t r0 = base[(size_t)b * nb + bk];
+    const uint2* sl = slabs + ((size_t)b * nb + bk) * kB1Cap;
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    // linear slot map of this bucket's key interval (the outermost buckets, whose interval is open-ended, borrow
+    // twice the width of their neighbour); monotone in the key, equal keys share a slot, out-of-range keys clamp
+    uint32_t klo, width;
+    {
+        const uint32_t* kb = klos + (size_t)b * (nb + 1);
+        klo = kb[bk];
+        width = kb[bk + 1] - klo;
+        if (bk + 1 == nb && nb > 1) width = 2u * min(klo - kb[bk - 1], 0x7fffffffu);
+        if (bk == 0 && nb > 2) { width = 2u * min(kb[2] - kb[1], 0x7fffffffu); klo = kb[1] > width ? kb[1] - width : 0u; width = kb[1] - klo; }
+    }
+    const float scale = (float)kB1Slots / ((float)width + 1.0f);
+    auto slot_of = [&](uint32_t key) -> uint32_t {
+        const uint32_t d = key > klo ? key - klo : 0u;
+        return min((uint32_t)(__uint2float_rz(d) * scale), (uint32_t)(kB1Slots - 1));
+    };
+    constexpr int WPT = kB1Slots / 2 / kB1SortThreads;      // counter words per thread in the scan (4 = one uint4)
+    static_assert(WPT == 4, "one uint4 of packed counters per thread");
+    reinterpret_cast<uint4*>(sm.cw)[t] = make_uint4(0u, 0u, 0u, 0u);
+    __syncthreads();
+    // 1. slot populations (the slab stays in L2 for step 3)
+#pragma unroll 4
+    for (uint32_t e = t; e < n; e += kB1SortThreads) {
+        const uint32_t s = slot_of(__ldcg(&sl[e].x));
+        atomicAdd(&sm.cw[s >> 1], 1u << ((s & 1u) << 4));
+    }
+    __syncthreads();
+    // 2. exclusive scan of the slot populations (8 consecutive slots per thread)
+    {
+        const uint4 w4 = reinterpret_cast<const uint4*>(sm.cw)[t];
+        const uint32_t w[4] = {w4.x, w4.y, w4.z, w4.w};
+        uint32_t sum = 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) sum += (w[i] & 0xffffu) + (w[i] >> 16);
+        uint32_t inc = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t m = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += m;
+        }
+        if (lane == 31) sm.wsum[warp] = inc;
+        __syncthreads();
+        uint32_t run = inc - sum;
+#pragma unroll
+        for (int wv = 0; wv < kB1SortThreads / 32; ++wv) run += (wv < warp) ? sm.wsum[wv] : 0u;
+        uint32_t o[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const uint32_t lo = run; run += w[i] & 0xffffu;
+            const uint32_t hi = run; run += w[i] >> 16;
+            o[i] = lo | (hi << 16);
+        }
+        reinterpret_cast<uint4*>(sm.cw)[t] = make_uint4(o[0], o[1], o[2], o[3]);
+    }
+    __syncthreads();
+    // 3. every pair into its slot's range (any order); the counter of slot s ends as the END of slot s
+#pragma unroll 4
+    for (uint32_t e = t; e < n; e += kB1SortThreads) {
+        const uint2 kv = __ldcs(sl + e);
+        const uint32_t s = slot_of(kv.x);
+        const uint32_t sh = (s & 1u) << 4;
+        const uint32_t q = (atomicAdd(&sm.cw[s >> 1], 1u << sh) >> sh) & 0xffffu;
+        sm.pair[q] = ((unsigned long long)kv.x << 32) | kv.y;
+    }
+    __syncthreads();
+    // 4. exact rank of every pair among its slot mates (they are contiguous; the 64-bit (key, index) words are all
+    //    distinct), one pair per thread at a time, and the index goes to that rank
+    uint32_t* io = idx_out + (size_t)b * N + r0;
+    float* so = sorted_out ? sorted_out + (size_t)b * N + r0 : nullptr;
+#pragma unroll 2
+    for (uint32_t q = t; q < n; q += kB1SortThreads) {
+        const unsigned long long v = sm.pair[q];
+        const uint32_t key = (uint32_t)(v >> 32);
+        const uint32_t s = slot_of(key);
+        const uint32_t w = sm.cw[s >> 1];
+        uint32_t z, a;
+        if (s & 1u) { z = w >> 16; a = w & 0xffffu; }
+        else { z = w & 0xffffu; a = s ? (sm.cw[(s >> 1) - 1] >> 16) : 0u; }
+        uint32_t r = q;
+        if (z - a > 1u) {
+            r = a;
+            for (uint32_t h = a; h < z; ++h) r += (sm.pair[h] < v);
+        }
+        io[r] = (uint32_t)v;
+        if (so) so[r] = val_of(key);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+inline cudaError_t bucket1_set_attrs() {
+    cudaFuncSetAttribute(part1_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaFuncSetAttribute(bucket1_sort_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaError_t e = cudaFuncSetAttribute(part1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)part1_smem(kB1MaxBuckets));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket1_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(B1Smem));
+    return e;
+}
+
+// pair scratch (uint2 units): slabs [B][nb][kB1Cap]
+inline size_t bucket1_pair_elems(long long B, long long N) { return (size_t)B * (size_t)(N >> kB1MeanLog) * kB1Cap; }
+
+// control words: hist [B][65536] u32 | cursor [B][nb] | overflow [B] (zeroed per call) | tab [B][65536] uint2 |
+//                base [B][nb] | klo [B][nb+1]
+inline size_t bucket1_zero_bytes(long long B, long long N) {
+    const size_t nb = (size_t)(N >> kB1MeanLog);
+    return (size_t)B * kBkBins * 4 + (size_t)B * nb * 4 + (size_t)B * 4;
+}
+inline size_t bucket1_ctl_bytes(long long B, long long N) {
+    const size_t nb = (size_t)(N >> kB1MeanLog);
+    return align_up(bucket1_zero_bytes(B, N), 256) + align_up((size_t)B * kBkBins * 8, 256) + align_up((size_t)B * nb * 4, 256) +
+           align_up((size_t)B * (nb + 1) * 4, 256);
+}
+
+// vals [B][N] -> idx_out (and optionally the sorted values) for the curves whose buckets all fit; *overflow_out points
+// at the per-curve flags (1 = not sorted here).  pairs: bucket1_pair_elems(B, N) (key, index) pairs of scratch.
+inline cudaError_t bucket1_sort(const float* vals, uint32_t* idx_out, float* sorted_out, long long B, long long N,
+                                uint2* pairs, void* ctl, const uint32_t** overflow_out, cudaStream_t st) {
+    const uint32_t nb = (uint32_t)(N >> kB1MeanLog);
+    unsigned char* w = (unsigned char*)ctl;
+    uint32_t* hist = (uint32_t*)w;
+    uint32_t* cursor = hist + (size_t)B * kBkBins;
+    uint32_t* overflow = cursor + (size_t)B * nb;
+    const size_t zero_bytes = bucket1_zero_bytes(B, N);
+    w += align_up(zero_bytes, 256);
+    uint2* tab = (uint2*)w; w += align_up((size_t)B * kBkBins * 8, 256);
+    uint32_t* base = (uint32_t*)w; w += align_up((size_t)B * nb * 4, 256);
+    uint32_t* klo = (uint32_t*)w;
+    cudaError_t e = cudaMemsetAsync(hist, 0, zero_bytes, st);
+    if (e != cudaSuccess) return e;
+    const uint32_t nsamp = (uint32_t)(N >> kBkSampleLog);
+    const uint32_t M = bucket1_magic(nb);
+    AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B)));
+    AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)(B * kCdfChunks), 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
+    AGN_LAUNCH(K_SORT_CDF, st, (bucket_bounds_kernel<<<bgrid((nb + 256) / 256, B), 256, 0, st>>>(tab, klo, nb, M, kB1SlotLog, B)));
+    Part1Args a;
+    a.vals = vals; a.out = pairs; a.cursor = cursor; a.overflow = overflow; a.tab = tab;
+    a.N = (uint32_t)N; a.nb = nb; a.M = M; a.B = B;
+    AGN_LAUNCH(K_SORT_PART_ONE, st, (part1_kernel<<<bgrid((unsigned)(N / kB1Tile), B), kB1PartThreads, part1_smem(nb), st>>>(a)));
+    const uint32_t bchunks = nb >= 1024 ? nb / 1024 : 1u;
+    AGN_LAUNCH(K_SORT_CDF, st, (bucket_base_kernel<<<(unsigned)(B * bchunks), 1024, 0, st>>>(cursor, base, nb, bchunks, (uint32_t)kB1Cap)));
+    AGN_LAUNCH(K_SORT_BUCKET, st, (bucket1_sort_kernel<<<bgrid(nb, B), kB1SortThreads, sizeof(B1Smem), st>>>(
+        pairs, cursor, base, overflow, klo, idx_out, sorted_out, (uint32_t)N, nb, B)));
+    *overflow_out = overflow;
+    return cudaGetLastError();
+}
+
+}  // namespace agn

@@ -284,18 +284,18 @@ __global__ void __launch_bounds__(kBkPartThreads, (LEVEL == 2 ? 4 : 6)) bucket_p
 // base[k] = sum of the populations of buckets < k (populations clamped to the slab).  `chunks` CTAs per curve, same
 // scheme as cdf_table_kernel: sum of everything before the chunk, then a scan of the chunk.
 __global__ void __launch_bounds__(1024) bucket_base_kernel(const uint32_t* __restrict__ cursor, uint32_t* __restrict__ base,
-                                                           uint32_t nb, uint32_t chunks) {
+                                                           uint32_t nb, uint32_t chunks, uint32_t cap) {
     __shared__ uint32_t ws[32];
     const uint32_t curve = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
     const uint32_t* c = cursor + (size_t)curve * nb;
     uint32_t* o = base + (size_t)curve * nb;
     const uint32_t per = nb / chunks;
     uint32_t before = 0;
-    for (uint32_t i = threadIdx.x; i < chunk * per; i += 1024) before += min(c[i], (uint32_t)kBkCap);
+    for (uint32_t i = threadIdx.x; i < chunk * per; i += 1024) before += min(c[i], cap);
     uint32_t run = block_sum_1024(before, ws);
     for (uint32_t k0 = chunk * per; k0 < (chunk + 1) * per; k0 += 1024) {
         const uint32_t k = k0 + threadIdx.x;
-        const uint32_t n = (k < (chunk + 1) * per) ? min(c[k], (uint32_t)kBkCap) : 0u;
+        const uint32_t n = (k < (chunk + 1) * per) ? min(c[k], cap) : 0u;
         uint32_t total;
         const uint32_t ex = block_excl_scan_1024(n, ws, &total);
         if (k < (chunk + 1) * per) o[k] = run + ex;
@@ -307,7 +307,7 @@ __global__ void __launch_bounds__(1024) bucket_base_kernel(const uint32_t* __res
 // [klo[k], klo[k+1]), so inside the finish kernel a slot is a plain linear map of the key onto that interval -- no
 // table look-up per key there.  One thread per bucket: invert umulhi(pos, M) >= k << kBkSlotLog, then the table.
 __global__ void __launch_bounds__(256) bucket_bounds_kernel(const uint2* __restrict__ tabs, uint32_t* __restrict__ klo,
-                                                            uint32_t nb, uint32_t M, long long B) {
+                                                            uint32_t nb, uint32_t M, int slot_log, long long B) {
     const long long b = bidx();
     if (b >= B) return;
     const uint32_t k = blockIdx.x * 256 + threadIdx.x;
@@ -315,7 +315,7 @@ __global__ void __launch_bounds__(256) bucket_bounds_kernel(const uint2* __restr
     uint32_t* out = klo + (size_t)b * (nb + 1);
     if (k == nb) { out[k] = 0xffffffffu; return; }
     const uint2* tab = tabs + (size_t)b * kBkBins;
-    const unsigned long long want = ((unsigned long long)k << kBkSlotLog) << 32;
+    const unsigned long long want = ((unsigned long long)k << slot_log) << 32;
     const unsigned long long P = (want + M - 1) / M;               // smallest pos32 with umulhi(pos32, M) >= k << slotlog
     uint32_t lo = 0, hi = kBkBins - 1;                              // largest bin with tab[bin].x <= P
     while (lo < hi) {
@@ -498,10 +498,8 @@ inline size_t bucket32_ctl_bytes(long long B, long long N) {
 
 // vals [B][N] -> idx_out (and optionally the sorted values) for the curves whose buckets all fit; *overflow_out points
 // at the per-curve flags (1 = not sorted here).  pairs: bucket32_pair_elems(B, N) (key, index) pairs of scratch.
-// reuse_cdf: keep the CDF tables of the previous call on the same workspace (the key distribution of x_adj barely
-// moves from one E13 iteration to the next; a stale table can only cost a slab overflow, i.e. the LSD fallback).
 inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* sorted_out, long long B, long long N,
-                                 uint2* pairs, void* ctl, const uint32_t** overflow_out, bool reuse_cdf, cudaStream_t st) {
+                                 uint2* pairs, void* ctl, const uint32_t** overflow_out, cudaStream_t st) {
     const BkGeom g = bucket32_geom(N);
     unsigned char* w = (unsigned char*)ctl;
     uint32_t* hist = (uint32_t*)w;
@@ -516,26 +514,23 @@ inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* so
     uint2* slabs2 = pairs;
     uint2* slabs1 = pairs + (size_t)B * g.nb * kBkCap;
     cudaError_t e;
-    if (reuse_cdf) {
-        e = cudaMemsetAsync(cursor2, 0, zero_bytes - (size_t)B * kBkBins * 4, st);      // cursors and flags only
-        if (e != cudaSuccess) return e;
-    } else {
-        e = cudaMemsetAsync(hist, 0, zero_bytes, st);
-        if (e != cudaSuccess) return e;
-        const uint32_t nsamp = (uint32_t)(N >> kBkSampleLog);
-        AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B)));
-        AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)(B * kCdfChunks), 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
-    }
-    AGN_LAUNCH(K_SORT_CDF, st, (bucket_bounds_kernel<<<bgrid((g.nb + 256) / 256, B), 256, 0, st>>>(tab, klo, g.nb, bucket32_magic(g.nb), B)));
+    // the CDF tables are re-estimated in every call: reusing them for 3 out of 4 E13 iterations was measured to overflow
+    // slabs (stale table -> LSD fallback) often enough to cost more than the 0.25 ms it saves
+    e = cudaMemsetAsync(hist, 0, zero_bytes, st);
+    if (e != cudaSuccess) return e;
+    const uint32_t nsamp = (uint32_t)(N >> kBkSampleLog);
+    AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B)));
+    AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)(B * kCdfChunks), 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
+    AGN_LAUNCH(K_SORT_CDF, st, (bucket_bounds_kernel<<<bgrid((g.nb + 256) / 256, B), 256, 0, st>>>(tab, klo, g.nb, bucket32_magic(g.nb), kBkSlotLog, B)));
     PartArgs a;
     a.vals = vals; a.in = slabs1; a.in_count = cursor1; a.overflow = overflow; a.tab = tab;
     a.N = (uint32_t)N; a.nb = g.nb; a.M = bucket32_magic(g.nb); a.lb = g.lb; a.nc = g.nc; a.cap_in = g.cap1; a.tiles_in = g.tiles1; a.B = B;
     a.out = slabs1; a.cursor = cursor1; a.cap_out = g.cap1;
-    AGN_LAUNCH(K_SORT_PART, st, (bucket_part_kernel<0><<<bgrid((unsigned)(N / bk_part_tile(0)), B), kBkPartThreads, sizeof(PartSmem<0>), st>>>(a)));
+    AGN_LAUNCH(K_SORT_PART0, st, (bucket_part_kernel<0><<<bgrid((unsigned)(N / bk_part_tile(0)), B), kBkPartThreads, sizeof(PartSmem<0>), st>>>(a)));
     a.out = slabs2; a.cursor = cursor2; a.cap_out = kBkCap;
-    AGN_LAUNCH(K_SORT_PART, st, (bucket_part_kernel<1><<<bgrid(g.tiles1 * g.nc, B), kBkPartThreads, sizeof(PartSmem<1>), st>>>(a)));
+    AGN_LAUNCH(K_SORT_PART1, st, (bucket_part_kernel<1><<<bgrid(g.tiles1 * g.nc, B), kBkPartThreads, sizeof(PartSmem<1>), st>>>(a)));
     const uint32_t bchunks = g.nb >= 16384 ? 16u : (g.nb >= 1024 ? g.nb / 1024 : 1u);
-    AGN_LAUNCH(K_SORT_CDF, st, (bucket_base_kernel<<<(unsigned)(B * bchunks), 1024, 0, st>>>(cursor2, base, g.nb, bchunks)));
+    AGN_LAUNCH(K_SORT_CDF, st, (bucket_base_kernel<<<(unsigned)(B * bchunks), 1024, 0, st>>>(cursor2, base, g.nb, bchunks, (uint32_t)kBkCap)));
     AGN_LAUNCH(K_SORT_BUCKET, st, (bucket_sort_kernel<<<bgrid(g.nb, B), kBkSortThreads, sizeof(BkSmem), st>>>(
         slabs2, cursor2, base, overflow, klo, idx_out, sorted_out, (uint32_t)N, g.nb, B)));
     *overflow_out = overflow;

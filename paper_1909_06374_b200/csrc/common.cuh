@@ -118,6 +118,30 @@ static inline dim3 bgrid(unsigned x, long long nb) {
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // ------------------------------------------------------------------------------------------------
+// per-device host-side state (function attributes set, SM count, occupancy-derived grid sizes): keyed by the real
+// device ordinal, so that one process may drive several devices
+// ------------------------------------------------------------------------------------------------
+struct DevCache {
+    int dev = -1;
+    bool attrs[2] = {false, false};     // by element size (4, 8)
+    int sms = 0;
+    int grid[8] = {0, 0, 0, 0, 0, 0, 0, 0};     // persistent-kernel grid sizes, by kernel slot
+};
+inline DevCache& dev_cache() {
+    static DevCache tab[64];
+    int dev = 0;
+    cudaGetDevice(&dev);
+    DevCache& c = tab[dev & 63];
+    if (c.dev != dev) {                 // first use of this ordinal (or an ordinal >= 64 aliasing a slot): start over
+        c = DevCache();
+        c.dev = dev;
+        cudaDeviceGetAttribute(&c.sms, cudaDevAttrMultiProcessorCount, dev);
+        if (c.sms < 1) c.sms = 1;
+    }
+    return c;
+}
+
+// ------------------------------------------------------------------------------------------------
 // launch trace (agnvar_trace_start / agnvar_trace_stop): when enabled, every kernel launch of the
 // library is bracketed by two CUDA events on its stream, so that a caller can read per-kernel device
 // time and launch counts of exactly the launches it timed.  Off by default (zero cost).
@@ -125,14 +149,14 @@ static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; 
 enum KernelId {
     K_FFT_STRIDED = 0, K_FFT_CONTIG, K_REPLACE, K_SORT_CTA, K_SORT_HIST, K_SORT_SWEEP, K_SCATTER, K_ITER_POST,
     K_PERM_ANORM, K_TK_FILL, K_TK_COMBINE, K_UNTANGLE_OUT, K_PSD, K_ERDF_TABLE, K_ERDF_SAMPLE, K_PGRAM, K_TABLES,
-    K_COPY, K_PHILOX, K_SCATTER_BIN, K_SCATTER_PLACE, K_FFT_COL, K_FFT_MID, K_SORT_CDF, K_SORT_PART, K_SORT_BUCKET, K_NIDS
+    K_COPY, K_PHILOX, K_SCATTER_BIN, K_SCATTER_PLACE, K_FFT_COL, K_FFT_MID, K_SORT_CDF, K_SORT_PART0, K_SORT_BUCKET, K_DELTA, K_SORT_PART1, K_SORT_PART_ONE, K_E13_ONCHIP, K_SF, K_SORT_FALLBACK, K_NIDS
 };
 static const char* const kKernelNames[K_NIDS] = {
     "fft_pass_strided", "fft_pass_contiguous", "amplitude_replace", "cta_argsort", "sort_digit_hist",
     "sort_onesweep", "rank_scatter_count", "iter_bookkeeping", "perm_anorm", "tk_fill", "tk_combine5_crop",
     "untangle_out", "psd", "erdf_table", "erdf_sample", "periodogram_scale_bin", "twiddle_tables", "copy", "philox",
-    "scatter_bin", "scatter_place", "fft_columns", "fft_mid_fused", "sort_cdf_tables", "sort_msd_partition",
-    "sort_bucket_finish"};
+    "scatter_bin", "scatter_place", "fft_columns", "fft_mid_fused", "sort_cdf_tables", "sort_part_level0",
+    "sort_bucket_finish", "delta_rms", "sort_part_level1", "sort_part_onelevel", "e13_onchip_loop", "structure_function", "sort_lsd_fallback_gated"};
 
 struct TraceRec { int id; cudaEvent_t e0, e1; };
 struct TraceState {

@@ -489,15 +489,12 @@ template <typename T> inline cudaError_t fft2_set_attrs() {
 }
 
 inline int fft2_col_grid(const void* func, int threads, int slot) {
-    static int cache[4] = {0, 0, 0, 0};
-    int& cached = cache[slot];
+    int& cached = dev_cache().grid[slot];
     if (cached) return cached;
-    int dev = 0, sms = 0, per = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    int per = 0;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, func, threads, 0);
     if (per < 1) per = 1;
-    cached = sms * per;
+    cached = dev_cache().sms * per;
     return cached;
 }
 
@@ -551,8 +548,7 @@ inline cudaError_t fft2_mid(const Fft2Plan<T>& p, typename Cx<T>::type* Z, const
     m.twpos = p.twpos; m.sp = p.sp; m.tw14 = p.tw14;
     m.rlv.tw14 = p.tw14; m.rlv.lo = p.lo_real; m.rlv.logD = p.logL + 1;
     const unsigned gx = p.logR0 == 0 ? 1u : (1u << (p.logR0 - 1));
-    static int sms = 0;
-    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+    const int sms = dev_cache().sms;
     const unsigned grid = (unsigned)std::min<long long>((long long)gx * B, sms);
     AGN_LAUNCH(K_FFT_MID, st, (fft_mid_kernel<T><<<grid, kMidThreads, kMidSmemBytes, st>>>(m)));
     return cudaGetLastError();

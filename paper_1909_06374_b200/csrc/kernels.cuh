@@ -331,21 +331,94 @@ __global__ void __launch_bounds__(256) scatter_count_kernel(const uint32_t* __re
     }
 }
 
-// L6 bookkeeping after iteration k (1-based): record the count, latch the first k with changed = 0.
-__global__ void post_iter_kernel(unsigned long long* __restrict__ changed, int* __restrict__ first_zero, int k,
-                                 long long* __restrict__ hist, int max_iter, int B) {
-    int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B) return;
-    unsigned long long c = changed[b];
-    if (hist) hist[(long long)b * max_iter + (k - 1)] = (long long)c;
-    if (c == 0 && first_zero[b] == 0) first_zero[b] = k;
-    changed[b] = 0;
+// ------------------------------------------------------------------------------------------------
+// delta_k (Eq. 4; NEXT-1): rms over the samples of log10(x_new / x_old).  Stage 1: one fixed-order
+// partial sum of squares per chunk of kDeltaChunk samples; stage 2 (inside post_iter_kernel): fixed-order sum of the
+// partials.  Deterministic (no atomics).  fp32: the ratio is formed first, then log1p(q - 1) near 1 (q - 1 is exact
+// for 1/2 <= q <= 2), so the per-sample error is an unbiased rounding of the ratio; squares accumulate in fp64.
+// ------------------------------------------------------------------------------------------------
+constexpr int kDeltaChunk = 16384;
+__device__ __forceinline__ double log10_ratio(float a, float b) {
+    const float q = a / b;
+    const float l = (q >= 0.5f && q <= 2.0f) ? log1pf(q - 1.0f) : logf(q);
+    return (double)l * 0.43429448190325182765;
 }
-__global__ void finalize_iters_kernel(const int* __restrict__ first_zero, int* __restrict__ iters_used, int max_iter,
+__device__ __forceinline__ double log10_ratio(double a, double b) { return log10(a / b); }
+
+template <typename T>
+__global__ void __launch_bounds__(256) delta_partial_kernel(const T* __restrict__ x_old, const T* __restrict__ x_new,
+                                                            long long N, double* __restrict__ partial, int nchunks, int B) {
+    __shared__ double sh[256];
+    const long long b = bidx();
+    if (b >= B) return;
+    const long long beg = (long long)blockIdx.x * kDeltaChunk;
+    const long long end = beg + kDeltaChunk < N ? beg + kDeltaChunk : N;
+    double acc = 0.0;
+    for (long long i = beg + threadIdx.x; i < end; i += 256) {
+        const double d = log10_ratio(x_new[b * N + i], x_old[b * N + i]);
+        acc += d * d;
+    }
+    const double tot = block_sum<256>(acc, sh);
+    if (threadIdx.x == 0) partial[b * nchunks + blockIdx.x] = tot;
+}
+
+// L6 bookkeeping after iteration k (1-based), one CTA per curve: record the change count (and delta_k), latch the
+// first k at which the curve stops (changed = 0, or delta_k <= threshold when a threshold is set), count the curves
+// that have stopped, count the iterations that took the LSD fallback.
+struct PostArgs {
+    unsigned long long* changed;    // [B] reset here
+    int* first_stop;                // [B] 0 = still running
+    long long* hist;                // [B][max_iter] or NULL
+    const double* partial;          // [B][nchunks] or NULL (delta not requested)
+    double* delta_hist;             // [B][max_iter] or NULL
+    double threshold;               // <= 0: off
+    long long N;
+    int nchunks, k, max_iter;
+    unsigned int* n_stopped;        // [1]
+    const uint32_t* overflow;       // [B] or NULL: the sort's per-curve fallback flag of this iteration
+    int* fallbacks;                 // [B] or NULL
+};
+__global__ void __launch_bounds__(256) post_iter_kernel(PostArgs a) {
+    __shared__ double sh[256];
+    const int b = blockIdx.x;
+    double delta = 0.0;
+    if (a.partial) {
+        double acc = 0.0;
+        for (int i = threadIdx.x; i < a.nchunks; i += 256) acc += a.partial[(long long)b * a.nchunks + i];
+        delta = sqrt(block_sum<256>(acc, sh) / (double)a.N);
+    }
+    if (threadIdx.x != 0) return;
+    const unsigned long long c = a.changed[b];
+    if (a.hist) a.hist[(long long)b * a.max_iter + (a.k - 1)] = (long long)c;
+    if (a.delta_hist) a.delta_hist[(long long)b * a.max_iter + (a.k - 1)] = delta;
+    const bool stop = (c == 0) || (a.partial && a.threshold > 0.0 && delta <= a.threshold);
+    if (stop && a.first_stop[b] == 0) {
+        a.first_stop[b] = a.k;
+        atomicAdd(a.n_stopped, 1u);
+    }
+    a.changed[b] = 0;
+    if (a.fallbacks && a.overflow && a.overflow[b]) a.fallbacks[b] += 1;
+}
+__global__ void finalize_iters_kernel(const int* __restrict__ first_stop, int* __restrict__ iters_used, int max_iter,
                                       int B) {
     int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
-    iters_used[b] = first_zero[b] ? first_zero[b] : max_iter;
+    iters_used[b] = first_stop[b] ? first_stop[b] : max_iter;
+}
+
+// delta mode: the state of curve b after iteration first_stop[b] is copied out when the curve stops (want = k), and the
+// curves that never stopped are copied out at the end (want = 0).  A CTA whose curve does not match exits at once.
+template <typename T>
+__global__ void __launch_bounds__(256) snapshot_kernel(const int* __restrict__ first_stop, int want, const T* __restrict__ x_src,
+                                                       const uint32_t* __restrict__ p_src, T* __restrict__ x_dst,
+                                                       uint32_t* __restrict__ p_dst, long long N, int B) {
+    const long long b = bidx();
+    if (b >= B || first_stop[b] != want) return;
+    const long long beg = (long long)blockIdx.x * 4096;
+    for (long long i = beg + threadIdx.x; i < beg + 4096 && i < N; i += 256) {
+        x_dst[b * N + i] = x_src[b * N + i];
+        p_dst[b * N + i] = p_src[b * N + i];
+    }
 }
 
 // x_adj + 0.0 (Q13: -0 -> +0) copy for the lock-step debug output
@@ -367,37 +440,51 @@ __device__ __forceinline__ double erdf_xi(const ErdfDev& e, double u) {
 }
 
 // One CTA per table: C_0 = 0, C_k = C_{k-1} + (p_k + p_{k-1}) D / 2, then C /= C_{G-1}.
-__global__ void erdf_table_kernel(const ErdfDev* __restrict__ erdf, int G, double* __restrict__ Ctab) {
+// p_k is evaluated once per grid point (parked in the output row), every thread adds up the trapezoids of its own
+// contiguous stretch, the stretch totals are scanned by the whole CTA (fixed order), and a last walk writes C.
+__device__ __forceinline__ void erdf_table_body(const ErdfDev& e, int G, double* __restrict__ Cc) {
     __shared__ double sh[256];
-    __shared__ double tot_sh;
-    const int t = blockIdx.x;
-    ErdfDev e = erdf[t];
-    double* Cc = Ctab + (long long)t * G;
     const double D = (e.u_hi - e.u_lo) / (double)(G - 1);
+    for (int k = threadIdx.x; k < G; k += 256) Cc[k] = erdf_xi(e, e.u_lo + (double)k * D);
+    __syncthreads();
     const int per = (G + 255) / 256;
     const int k0 = threadIdx.x * per, k1 = min(G, k0 + per);
-    double acc = 0.0;
-    for (int k = max(k0, 1); k < k1; ++k) {
-        double pk = erdf_xi(e, e.u_lo + (double)k * D), pm = erdf_xi(e, e.u_lo + (double)(k - 1) * D);
-        acc += 0.5 * (pk + pm) * D;
+    const double p_before = (k0 > 0 && k0 < G) ? Cc[k0 - 1] : 0.0;
+    double acc = 0.0, pm = p_before;
+    for (int k = k0; k < k1; ++k) {
+        const double pk = Cc[k];
+        if (k > 0) acc += 0.5 * (pk + pm) * D;
+        pm = pk;
     }
+    // inclusive scan of the stretch totals (Hillis-Steele in shared memory: the order is fixed)
     sh[threadIdx.x] = acc;
     __syncthreads();
-    if (threadIdx.x == 0) {
-        double run = 0.0;
-        for (int i = 0; i < 256; ++i) { double v = sh[i]; sh[i] = run; run += v; }
-        tot_sh = run;
+    for (int o = 1; o < 256; o <<= 1) {
+        const double v = (threadIdx.x >= o) ? sh[threadIdx.x - o] : 0.0;
+        __syncthreads();
+        sh[threadIdx.x] += v;
+        __syncthreads();
     }
-    __syncthreads();
-    double run = sh[threadIdx.x];
-    const double tot = tot_sh;
+    const double tot = sh[255];
+    double run = sh[threadIdx.x] - acc;
+    pm = p_before;
     for (int k = k0; k < k1; ++k) {
-        if (k > 0) {
-            double pk = erdf_xi(e, e.u_lo + (double)k * D), pm = erdf_xi(e, e.u_lo + (double)(k - 1) * D);
-            run += 0.5 * (pk + pm) * D;
-        }
+        const double pk = Cc[k];
+        if (k > 0) run += 0.5 * (pk + pm) * D;
+        pm = pk;
         Cc[k] = (k == G - 1) ? 1.0 : run / tot;
     }
+}
+__global__ void __launch_bounds__(256) erdf_table_kernel(const ErdfDev* __restrict__ erdf, int G, double* __restrict__ Ctab) {
+    const ErdfDev e = erdf[blockIdx.x];
+    erdf_table_body(e, G, Ctab + (long long)blockIdx.x * G);
+}
+// the same table from parameters passed by value (agnvar_erdf_table: no device scratch)
+constexpr int kErdfArgBatch = 32;
+struct ErdfBatch { ErdfDev e[kErdfArgBatch]; };
+__global__ void __launch_bounds__(256) erdf_table_args_kernel(ErdfBatch eb, int G, double* __restrict__ Ctab) {
+    const ErdfDev e = eb.e[blockIdx.x];
+    erdf_table_body(e, G, Ctab + (long long)blockIdx.x * G);
 }
 
 // One thread per Philox call = two samples (n = 2i uses words (0,1), n = 2i+1 words (2,3)).

@@ -1,0 +1,137 @@
+// sf.cuh -- NEXT-2: the observables the paper builds on the generated light curves (evenly sampled, lag l = tau / dt):
+//   structure function (Eq. A6)   SF(tau)^2 = mean over the N - l pairs (i, i + l) of [v_i - v_{i+l}]^2,
+//       v = x (L/L_Edd units) or v = -2.5 log10 x (magnitudes: the zero point cancels);
+//   representative SF (Eq. 6)      mean over the realisations of SF_i^2 and its standard error;
+//   P(|dm| > dm_ref | tau)         fraction of the pairs at lag l with |m_i - m_{i+l}| > dm_ref,
+//       optionally with a magnitude cut (points fainter than m_cut become upper limits at m_cut; only pairs with at
+//       least one detected point count).
+// Pair reductions are bandwidth-bound: every sample is read once per lag (twice when the lag exceeds the chunk); the
+// magnitudes are computed ONCE per call into the workspace (fp64), not once per lag.  All differences and sums are fp64
+// (fp32 inputs are exact in fp64); sums are fixed-order (per-chunk partials, then a fixed tree): deterministic.
+#pragma once
+#include "common.cuh"
+#include "kernels.cuh"
+
+namespace agn {
+
+constexpr int kSfChunk = 8192;          // pairs per CTA and lag
+constexpr int kSfMaxRef = 16;
+
+// v[i] = m_zero - 2.5 log10(x[i]) (fp64), optionally clipped at m_cut with a detection flag (1 = detected, m <= m_cut)
+template <typename T>
+__global__ void __launch_bounds__(256) sf_mag_kernel(const T* __restrict__ x, long long n, double m_zero, int use_cut,
+                                                     double m_cut, double* __restrict__ v, unsigned char* __restrict__ det) {
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (i >= n) return;
+    double m = m_zero - 2.5 * log10((double)x[i]);
+    if (det) det[i] = (!use_cut || m <= m_cut) ? 1 : 0;
+    if (use_cut && m > m_cut) m = m_cut;
+    v[i] = m;
+}
+
+// partial[b][q][chunk] = sum over the chunk's pairs of (v_i - v_{i+l})^2.  V = T (raw series) or double (magnitudes).
+template <typename V>
+__global__ void __launch_bounds__(256) sf_partial_kernel(const V* __restrict__ v, long long N, const long long* __restrict__ lags,
+                                                         int nlags, double* __restrict__ partial, int nchunks, int B) {
+    __shared__ double sh[256];
+    const long long b = blockIdx.z;
+    const int q = blockIdx.y;
+    const long long l = lags[q];
+    const long long P = N - l;                              // number of pairs (<= 0: none)
+    const long long beg = (long long)blockIdx.x * kSfChunk;
+    const long long end = beg + kSfChunk < P ? beg + kSfChunk : P;
+    const V* vb = v + b * N;
+    double acc = 0.0;
+    for (long long i = beg + threadIdx.x; i < end; i += 256) {
+        const double d = (double)vb[i] - (double)vb[i + l];
+        acc += d * d;
+    }
+    const double tot = block_sum<256>(acc, sh);
+    if (threadIdx.x == 0) partial[(b * nlags + q) * nchunks + blockIdx.x] = tot;
+}
+
+// sf2[b][q] = (sum of the partials) / (N - l); pairs[q] = N - l
+__global__ void __launch_bounds__(256) sf_final_kernel(const double* __restrict__ partial, int nchunks, long long N,
+                                                       const long long* __restrict__ lags, int nlags, double* __restrict__ sf2,
+                                                       long long* __restrict__ pairs) {
+    __shared__ double sh[256];
+    const long long b = blockIdx.y;
+    const int q = blockIdx.x;
+    const long long P = N - lags[q];
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < nchunks; i += 256) acc += partial[(b * nlags + q) * nchunks + i];
+    const double tot = block_sum<256>(acc, sh);
+    if (threadIdx.x == 0) {
+        sf2[b * nlags + q] = P > 0 ? tot / (double)P : 0.0;
+        if (pairs && b == 0) pairs[q] = P > 0 ? P : 0;
+    }
+}
+
+// Eq. 6: mean over the B realisations and the standard error of that mean (sample standard deviation / sqrt(B))
+__global__ void __launch_bounds__(256) sf_rep_kernel(const double* __restrict__ sf2, int B, int nlags, double* __restrict__ mean,
+                                                     double* __restrict__ se) {
+    __shared__ double sh[256];
+    const int q = blockIdx.x;
+    double acc = 0.0;
+    for (int b = threadIdx.x; b < B; b += 256) acc += sf2[(long long)b * nlags + q];
+    const double m = block_sum<256>(acc, sh) / (double)B;
+    double var = 0.0;
+    for (int b = threadIdx.x; b < B; b += 256) { const double d = sf2[(long long)b * nlags + q] - m; var += d * d; }
+    const double tv = block_sum<256>(var, sh);
+    if (threadIdx.x == 0) {
+        if (mean) mean[q] = m;
+        if (se) se[q] = B > 1 ? sqrt(tv / (double)(B - 1) / (double)B) : 0.0;
+    }
+}
+
+// counts[b][q][r] += #{pairs of the chunk considered with |m_i - m_{i+l}| > ref_r}; considered[b][q] += #{pairs considered}
+struct DmRefs { double ref[kSfMaxRef]; };
+__global__ void __launch_bounds__(256) dm_count_kernel(const double* __restrict__ m, const unsigned char* __restrict__ det,
+                                                       long long N, const long long* __restrict__ lags, int nlags, DmRefs refs,
+                                                       int nref, unsigned long long* __restrict__ counts,
+                                                       unsigned long long* __restrict__ considered, int B) {
+    const long long b = blockIdx.z;
+    const int q = blockIdx.y;
+    const long long l = lags[q];
+    const long long P = N - l;
+    const long long beg = (long long)blockIdx.x * kSfChunk;
+    const long long end = beg + kSfChunk < P ? beg + kSfChunk : P;
+    const double* mb = m + b * N;
+    const unsigned char* db = det + b * N;
+    unsigned int c[kSfMaxRef];
+#pragma unroll
+    for (int r = 0; r < kSfMaxRef; ++r) c[r] = 0u;
+    unsigned int np = 0u;
+    for (long long i = beg + threadIdx.x; i < end; i += 256) {
+        if (!(db[i] | db[i + l])) continue;
+        ++np;
+        const double d = fabs(mb[i] - mb[i + l]);
+#pragma unroll
+        for (int r = 0; r < kSfMaxRef; ++r) c[r] += (r < nref && d > refs.ref[r]) ? 1u : 0u;
+    }
+    // warp totals, then one integer atomic per warp and counter (integer sums are order-independent: deterministic)
+#pragma unroll
+    for (int r = 0; r < kSfMaxRef; ++r) {
+        if (r < nref) {
+            unsigned int t = c[r];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+            if ((threadIdx.x & 31) == 0 && t) atomicAdd(&counts[(b * nlags + q) * nref + r], (unsigned long long)t);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) np += __shfl_xor_sync(0xffffffffu, np, o);
+    if ((threadIdx.x & 31) == 0 && np) atomicAdd(&considered[b * nlags + q], (unsigned long long)np);
+}
+
+__global__ void dm_final_kernel(const unsigned long long* __restrict__ counts, const unsigned long long* __restrict__ considered,
+                                long long n_bq, int nref, double* __restrict__ prob, long long* __restrict__ considered_out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_bq * nref) return;
+    const long long bq = i / nref;
+    const unsigned long long P = considered[bq];
+    prob[i] = P ? (double)counts[i] / (double)P : 0.0;
+    if (considered_out && i % nref == 0) considered_out[bq] = (long long)P;
+}
+
+}  // namespace agn

@@ -12,6 +12,7 @@
 #include "common.cuh"
 #include "sort.cuh"
 #include "bucket32.cuh"
+#include "bucket1.cuh"
 
 namespace agn {
 
@@ -279,6 +280,7 @@ inline cudaError_t sort32_set_attrs() {
     cudaFuncSetAttribute(sweep32_kernel<1>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     cudaFuncSetAttribute(sweep32_kernel<2>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e == cudaSuccess) e = bucket32_set_attrs();
+    if (e == cudaSuccess) e = bucket1_set_attrs();
     return e;
 }
 
@@ -290,9 +292,11 @@ inline bool sort32_applicable(size_t elem_size, long long N) {
 inline size_t sort32_ws_bytes(long long B, long long N) {
     const size_t ntiles = (size_t)(N / kS32Tile);
     size_t s = 2 * align_up((size_t)B * N * sizeof(uint2), 256);
-    if (bucket32_applicable(4, N)) s = std::max(s, align_up(bucket32_pair_elems(B, N) * sizeof(uint2), 256));
+    if (bucket1_applicable(4, N)) s = std::max(s, align_up(bucket1_pair_elems(B, N) * sizeof(uint2), 256));
+    else if (bucket32_applicable(4, N)) s = std::max(s, align_up(bucket32_pair_elems(B, N) * sizeof(uint2), 256));
     s += align_up((size_t)B * 4 * kRadix * 4 + (size_t)B * 4 * 4 + (size_t)B * 4 * ntiles * kRadix * 4, 256);
-    if (bucket32_applicable(4, N)) s += bucket32_ctl_bytes(B, N);
+    if (bucket1_applicable(4, N)) s += bucket1_ctl_bytes(B, N);
+    else if (bucket32_applicable(4, N)) s += bucket32_ctl_bytes(B, N);
     return s;
 }
 
@@ -316,35 +320,43 @@ __global__ void __launch_bounds__(kRadix) lsd_clear_kernel(uint32_t* __restrict_
 
 // vals [B][N] -> idx_out [B][N]; optionally the sorted values.  Returns the free pair buffer (for the scatter) in *spare.
 inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* sorted_out, long long B, long long N,
-                                 void* ws, uint2** spare, cudaStream_t st, bool reuse_cdf = false) {
+                                 void* ws, uint2** spare, cudaStream_t st, const uint32_t** gate_out = nullptr) {
     constexpr int NP = 4;
     unsigned char* w = (unsigned char*)ws;
     uint2* pa = (uint2*)w; w += align_up((size_t)B * N * sizeof(uint2), 256);
     uint2* pb = (uint2*)w; w += align_up((size_t)B * N * sizeof(uint2), 256);
-    if (bucket32_applicable(4, N)) w = (unsigned char*)ws + std::max((size_t)(w - (unsigned char*)ws), align_up(bucket32_pair_elems(B, N) * sizeof(uint2), 256));
+    const bool one_level = bucket1_applicable(4, N);
+    if (one_level) w = (unsigned char*)ws + std::max((size_t)(w - (unsigned char*)ws), align_up(bucket1_pair_elems(B, N) * sizeof(uint2), 256));
+    else if (bucket32_applicable(4, N)) w = (unsigned char*)ws + std::max((size_t)(w - (unsigned char*)ws), align_up(bucket32_pair_elems(B, N) * sizeof(uint2), 256));
     const size_t ntiles = (size_t)(N / kS32Tile);
     uint32_t* hist = (uint32_t*)w;
     uint32_t* ticket = hist + (size_t)B * NP * kRadix;
     uint32_t* status = ticket + (size_t)B * NP;
     const size_t ctl = (size_t)B * NP * kRadix * 4 + (size_t)B * NP * 4 + (size_t)B * NP * ntiles * kRadix * 4;
     cudaError_t e;
-    // long curves: two-level bucket sort (bucket32.cuh); the LSD passes below then only run for curves it gave up on
+    // long curves: distribution sort, one partition level (bucket1.cuh; N <= 2^26) or two (bucket32.cuh; N = 2^27); the
+    // LSD passes below then only run for curves it gave up on
     const uint32_t* gate = nullptr;
-    if (bucket32_applicable(4, N)) {
-        e = bucket32_sort(vals, idx_out, sorted_out, B, N, pa, w + align_up(ctl, 256), &gate, reuse_cdf, st);
+    if (one_level) {
+        e = bucket1_sort(vals, idx_out, sorted_out, B, N, pa, w + align_up(ctl, 256), &gate, st);
+        if (e != cudaSuccess) return e;
+    } else if (bucket32_applicable(4, N)) {
+        e = bucket32_sort(vals, idx_out, sorted_out, B, N, pa, w + align_up(ctl, 256), &gate, st);
         if (e != cudaSuccess) return e;
     }
     const size_t nchunks = (ntiles + kS32Chunk - 1) / kS32Chunk;
     if (gate) {
-        AGN_LAUNCH(K_SORT_HIST, st, (lsd_clear_kernel<<<bgrid((unsigned)std::min<size_t>(NP * nchunks, 512), B), kRadix, 0, st>>>(
+        AGN_LAUNCH(K_SORT_FALLBACK, st, (lsd_clear_kernel<<<bgrid((unsigned)std::min<size_t>(NP * nchunks, 512), B), kRadix, 0, st>>>(
             hist, ticket, status, gate, (uint32_t)nchunks, (size_t)B * ntiles * kRadix, B)));
     } else {
         e = cudaMemsetAsync(hist, 0, ctl, st);
         if (e != cudaSuccess) return e;
     }
     const int chunk = 1 << 16;
-    AGN_LAUNCH(K_SORT_HIST, st, (digit_hist_kernel<float, 512><<<bgrid((unsigned)((N + chunk - 1) / chunk), B), 512, 0, st>>>(vals, hist, N, N, chunk, B, gate)));
-    AGN_LAUNCH(K_SORT_HIST, st, (digit_scan_kernel<<<(unsigned)(B * NP), kRadix, 0, st>>>(hist, gate, NP)));
+    // with a gate these launches are the fallback of the distribution sort: they exit at once unless a slab overflowed
+    const int id_hist = gate ? K_SORT_FALLBACK : K_SORT_HIST, id_sweep = gate ? K_SORT_FALLBACK : K_SORT_SWEEP;
+    AGN_LAUNCH(id_hist, st, (digit_hist_kernel<float, 512><<<bgrid((unsigned)((N + chunk - 1) / chunk), B), 512, 0, st>>>(vals, hist, N, N, chunk, B, gate)));
+    AGN_LAUNCH(id_hist, st, (digit_scan_kernel<<<(unsigned)(B * NP), kRadix, 0, st>>>(hist, gate, NP)));
     const dim3 grid = bgrid((unsigned)std::min<size_t>(nchunks, 592), B);
     for (int p = 0; p < NP; ++p) {
         Sweep32Args a;
@@ -357,11 +369,12 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
         a.status = status + (size_t)p * B * ntiles * kRadix;
         a.ticket = ticket + (size_t)p * B;
         a.ntiles = (uint32_t)ntiles; a.nchunks = (uint32_t)nchunks; a.B = B; a.gate = gate;
-        if (p == 0) AGN_LAUNCH(K_SORT_SWEEP, st, (sweep32_kernel<0><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
-        else if (p == NP - 1) AGN_LAUNCH(K_SORT_SWEEP, st, (sweep32_kernel<2><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
-        else AGN_LAUNCH(K_SORT_SWEEP, st, (sweep32_kernel<1><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
+        if (p == 0) AGN_LAUNCH(id_sweep, st, (sweep32_kernel<0><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
+        else if (p == NP - 1) AGN_LAUNCH(id_sweep, st, (sweep32_kernel<2><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
+        else AGN_LAUNCH(id_sweep, st, (sweep32_kernel<1><<<grid, kS32Threads, sizeof(S32Smem), st>>>(a)));
     }
     if (spare) *spare = pb;
+    if (gate_out) *gate_out = gate;
     return cudaGetLastError();
 }
 

@@ -8,7 +8,8 @@ from . import binding as _b
 from . import workloads as _w
 
 
-def generate_light_curves(cfg, device="cuda", host_out=None, want_hist=False, curve0=0):
+def generate_light_curves(cfg, device="cuda", host_out=None, want_hist=False, curve0=0, want_fallbacks=False,
+                          delta_threshold=0.0, want_delta=False):
     """Run erdf_sample_sorted -> tk_generate -> e13_iterate (-> periodogram if cfg['nbins']) for cfg
     (a dict from workloads.config).  Returns dict(x, perm, iters_used, changed_hist, pbin, counts).
 
@@ -21,7 +22,8 @@ def generate_light_curves(cfg, device="cuda", host_out=None, want_hist=False, cu
                                                 cfg["grid_points"], device=device)
     _, anorm = _b.agnvar_tk_generate(cfg["psd"], B, N, cfg["dt"], cfg["oversample"], cfg["dtype"], cfg["seed"],
                                      curve0, want_xnorm=False, device=device)
-    out = _b.agnvar_e13_iterate(anorm, srt, perm, cfg["max_iter"], want_hist=want_hist)
+    out = _b.agnvar_e13_iterate(anorm, srt, perm, cfg["max_iter"], want_hist=want_hist, want_fallbacks=want_fallbacks,
+                                delta_threshold=delta_threshold, want_delta=want_delta)
     out["pbin"] = out["counts"] = None
     if cfg.get("nbins", 0):
         out["pbin"], out["counts"] = _b.agnvar_periodogram(out["x"], cfg["dt"], 0,

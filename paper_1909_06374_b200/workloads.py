@@ -1,24 +1,42 @@
 """Seeded synthetic workloads: BASELINE.json's five configurations as plain parameter sets.
 
-This module holds NONE of the method's arithmetic (no PSD, ERDF, FFT, sort, Philox): it only names
-shapes and parameters and draws per-curve parameters with numpy's own generator, so that the CUDA
-path (tests, bench.py) and the CPU oracle (tests) can be fed the same inputs without sharing code.
+This module holds NONE of the method's arithmetic (no PSD, ERDF, FFT, sort): it only names shapes and
+parameters and draws the per-curve parameters of C2 / C5, so that the CUDA path (tests, bench.py) and the
+CPU oracle (tests) can be fed the same inputs without sharing code.  The per-curve draws follow SURVEY.md
+8(d): parameter p of curve b is the uniform made from words (0, 1) of Philox4x32-10 with counter (p, 0, b, 2)
+and key (seed lo, seed hi) -- a small generator of this module's own (neither the oracle's nor the
+library's), so the workloads do not depend on any numpy version.
 The paper measures on no public benchmark; these shapes stand in for its workloads (Table 1 / Table 2,
 PAPER.md:261-270, :407-421; PTF-like and LSST-like cadences).  See DESIGN.md.
 """
 import math
 
-import numpy as np
-
 BPL, LOGNORMAL = 0, 1
+_M32 = 0xFFFFFFFF
 
 
-def _uniform(rng, lo, hi, n):
-    return lo + (hi - lo) * rng.random(n)
+def _philox_words(seed, c0, c1, c2, c3):
+    """Philox4x32-10 (published algorithm: Salmon et al. 2011), plain Python integers."""
+    k0, k1 = seed & _M32, (seed >> 32) & _M32
+    for _ in range(10):
+        p0, p1 = 0xD2511F53 * c0, 0xCD9E8D57 * c2
+        c0, c1, c2, c3 = ((p1 >> 32) ^ c1 ^ k0) & _M32, p1 & _M32, ((p0 >> 32) ^ c3 ^ k1) & _M32, p0 & _M32
+        k0, k1 = (k0 + 0x9E3779B9) & _M32, (k1 + 0xBB67AE85) & _M32
+    return c0, c1, c2, c3
 
 
-def _loguniform(rng, lo, hi, n):
-    return 10.0 ** (math.log10(lo) + (math.log10(hi) - math.log10(lo)) * rng.random(n))
+def param_uniform(seed, p, b):
+    """Uniform in (0, 1) for parameter number p of curve b (stream tag 2)."""
+    w = _philox_words(seed, p, 0, b, 2)
+    return (2 * ((w[0] << 20) + (w[1] >> 12)) + 1) * 2.0 ** -53
+
+
+def _uniform(seed, p, lo, hi, n):
+    return [lo + (hi - lo) * param_uniform(seed, p, b) for b in range(n)]
+
+
+def _loguniform(seed, p, lo, hi, n):
+    return [10.0 ** (math.log10(lo) + (math.log10(hi) - math.log10(lo)) * param_uniform(seed, p, b)) for b in range(n)]
 
 
 def config(name, B=None):
@@ -32,10 +50,9 @@ def config(name, B=None):
                  psd=[dict(A=0.0, f_b=1.0 / 300.0, alpha_low=1.0, alpha_high=2.0)],
                  erdf=[dict(kind=BPL, lam_star=0.1, delta1=0.4, delta2=2.4, lam_min=1e-4, lam_max=1.0)])
     elif name == "C2":  # PTF/iPTF-like
-        Bf = 4096
-        rng = np.random.default_rng(2)
-        fb = _loguniform(rng, 1.0 / 1000.0, 1.0 / 50.0, Bf)
-        c = dict(B=Bf, N=2 ** 14, dt=1.0, oversample=10, dtype="f32", max_iter=200, seed=2,
+        Bf = 4096 if B is None else min(int(B), 4096)     # curve b's parameters do not depend on the subset size
+        fb = _loguniform(2, 0, 1.0 / 1000.0, 1.0 / 50.0, Bf)
+        c = dict(B=4096, N=2 ** 14, dt=1.0, oversample=10, dtype="f32", max_iter=200, seed=2,
                  psd=[dict(A=0.0, f_b=float(f), alpha_low=1.0, alpha_high=2.5) for f in fb],
                  erdf=[dict(kind=BPL, lam_star=10 ** -1.5, delta1=0.45, delta2=2.5, lam_min=1e-5, lam_max=1.0)])
     elif name == "C3":  # LSST-like
@@ -48,12 +65,11 @@ def config(name, B=None):
                  psd=[dict(A=0.0, f_b=1.0 / (365.0 * 1e3), alpha_low=1.0, alpha_high=2.0)],
                  erdf=[dict(kind=BPL, lam_star=0.05, delta1=0.2, delta2=2.2, lam_min=1e-6, lam_max=1.0)])
     elif name == "C5":  # parameter sweep
-        Bf = 65536
-        rng = np.random.default_rng(7)
-        alo, ahi = _uniform(rng, 0.5, 1.5, Bf), _uniform(rng, 2.0, 3.0, Bf)
-        fb = _loguniform(rng, 1e-3, 1e-1, Bf)
-        d1, d2 = _uniform(rng, 0.1, 0.6, Bf), _uniform(rng, 2.0, 3.0, Bf)
-        c = dict(B=Bf, N=1024, dt=1.0, oversample=1, dtype="f32", max_iter=100, seed=7,
+        Bf = 65536 if B is None else min(int(B), 65536)
+        alo, ahi = _uniform(7, 0, 0.5, 1.5, Bf), _uniform(7, 1, 2.0, 3.0, Bf)
+        fb = _loguniform(7, 2, 1e-3, 1e-1, Bf)
+        d1, d2 = _uniform(7, 3, 0.1, 0.6, Bf), _uniform(7, 4, 2.0, 3.0, Bf)
+        c = dict(B=65536, N=1024, dt=1.0, oversample=1, dtype="f32", max_iter=100, seed=7,
                  psd=[dict(A=0.0, f_b=float(fb[i]), alpha_low=float(alo[i]), alpha_high=float(ahi[i]))
                       for i in range(Bf)],
                  erdf=[dict(kind=BPL, lam_star=10 ** -1.5, delta1=float(d1[i]), delta2=float(d2[i]), lam_min=1e-5,

@@ -30,12 +30,28 @@ def test_reference_arm_line():
     assert d["config"]["workload"].startswith("C4")
 
 
+def test_gpus_flag_spawns_ranks():
+    """`python bench.py --gpus 2` with no torchrun around it must run TWO ranks (re-exec under
+    torch.distributed.run on 127.0.0.1) and print ONE line with n_gpus = 2.  Host-side plumbing only (gloo, no GPU
+    work): rendezvous, the weak-scaling curve partition and the max-over-ranks reduction."""
+    env_clean = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-ranks", "--backend", "gloo"],
+                         capture_output=True, text=True, timeout=600, cwd=ROOT, env=env_clean)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.strip().startswith("{")]
+    assert len(lines) == 1, out.stdout
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["curve0_by_rank"] == [0, 4]
+    assert d["ms_max_over_ranks"] == 101.0          # the slowest rank's time
+
+
 @pytest.mark.gpu
 def test_product_arm_line():
     """The product arm on the small fp64 configuration: every key of the contract is there and sane."""
     d = _run(["--workload", "C1", "--steps", "2", "--warmup", "3", "--no-cpu-baseline"], 900)
     for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
-              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "stages", "kernels"):
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "stages", "kernels",
+              "traffic_model", "sort_fallbacks", "fp32_free_running_context"):
         assert k in d, k
     assert d["steps"] == 2 and d["warmup"] == 3 and d["n_gpus"] == 1 and d["scaling"] == "weak"
     assert d["value"] > 0 and d["ms_per_step"] > 0 and d["gpu_launches"] > 0

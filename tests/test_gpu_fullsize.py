@@ -1,13 +1,17 @@
-"""Full-size parity (-m gpu): BASELINE.json's metric configuration C4 (B=4 curves x N=2^26, fp32) in the launch
-configuration bench.py times.  At this size the oracle cannot redo the whole batch, so the test checks
+"""Full-size parity (-m gpu): BASELINE.json's configurations at the sizes bench.py times, in the same launch
+configuration.  At these sizes the oracle cannot redo a whole batch, so the tests check
 
-  * properties that hold at any size and pin the result uniquely, on every curve (computed with torch on the GPU
-    from the C-ABI outputs only): the permutation is valid; x_adj read along it is non-decreasing and equal keys
-    appear by ascending time index (so it is THE stable argsort of the GPU's own x_adj, SURVEY 8(c) clause ii);
-    x_sim,k+1[idx[r]] = sorted[r] bit-exactly (clause iv); the change count equals the number of differing
-    entries of the two permutations (clause v);
-  * one curve against the fp64 oracle, one whole step from the GPU's own x_sim (lock-step, P1):
-    relative L2 of x_adj <= 1e-5 (clause i) and eps-sortedness of the GPU order on the exact x_adj (clause iii).
+  * C4 (B=4 x N=2^26, fp32), lock-step at iterations k = 2, 25 and 50 (= max_iter) of one run of the product kernels:
+    properties that hold at any size and pin the result uniquely, on every curve (computed with torch on the GPU from
+    the C-ABI outputs only): the permutation is valid; x_adj read along it is non-decreasing and equal keys appear by
+    ascending time index (so it is THE stable argsort of the GPU's own x_adj, SURVEY 8(c) clause ii);
+    x_sim,k+1[idx[r]] = sorted[r] bit-exactly (clause iv); the change count equals the number of differing entries of
+    the two permutations (clause v); no curve left the distribution sort for the LSD fallback;
+    and ONE CURVE AGAINST THE fp64 ORACLE, one whole step from the GPU's own x_sim (P1): relative L2 of
+    x_adj <= 1e-5 (clause i) and eps-sortedness of the GPU order on the exact x_adj (clause iii);
+  * S2 at C4's own size: one curve of agnvar_tk_generate at N = 2^26 (the three-pass generic FFT with split hi/lo
+    twiddle tables) against the oracle's TK95 series and amplitudes;
+  * P at C3's size: the periodogram and its 64-bin form at N = 2^20 against the oracle.
 """
 import numpy as np
 import pytest
@@ -20,49 +24,96 @@ def u32(t):
     return t.cpu().numpy().view(np.uint32)
 
 
-def test_c4_full_size_step(orc):
+def rel_l2(a, b):
+    a, b = np.asarray(a, dtype=np.float64), np.asarray(b, dtype=np.float64)
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def test_c4_tk_generate_full_size(orc):
+    import paper_1909_06374_b200 as ag
+    from paper_1909_06374_b200 import workloads
+    cfg = workloads.config("C4")
+    N, p = cfg["N"], cfg["psd"][0]
+    assert N == 2 ** 26
+    xn, an = ag.agnvar_tk_generate(cfg["psd"], 1, N, cfg["dt"], cfg["oversample"], "f32", cfg["seed"], 1)
+    ref = orc.tk_generate(0.0, p["f_b"], p["alpha_low"], p["alpha_high"], N, cfg["dt"], cfg["oversample"], cfg["seed"], 1)
+    ex, ea = rel_l2(xn[0].cpu().numpy(), ref["x_norm"]), rel_l2(an[0].cpu().numpy(), ref["A_norm"])
+    print(f"S2 at N=2^26: x_norm rel L2 {ex:.2e}, A_norm rel L2 {ea:.2e}")
+    assert ex <= 1e-5 and ea <= 1e-5
+    ag.free_workspace()
+
+
+def test_c3_periodogram_full_size(orc):
+    import paper_1909_06374_b200 as ag
+    from paper_1909_06374_b200 import workloads
+    cfg = workloads.config("C3", B=2)
+    B, N = cfg["B"], cfg["N"]
+    assert N == 2 ** 20 and cfg["nbins"] == 64
+    out = ag.generate_light_curves(dict(cfg, max_iter=3))
+    x = out["x"].cpu().numpy()
+    edges = workloads.log_bin_edges(N, 64)
+    P = ag.agnvar_periodogram(out["x"], cfg["dt"], 1).cpu().numpy()
+    pb, cnt = out["pbin"].cpu().numpy(), out["counts"].cpu().numpy()
+    for b in range(B):
+        ref = orc.periodogram(x[b].astype(np.float64), cfg["dt"], 1)
+        assert rel_l2(P[b], ref) <= 1e-5
+        rb, rc = orc.periodogram_binned(x[b].astype(np.float64), cfg["dt"], 0, edges)
+        assert (cnt == rc).all()
+        assert np.max(np.abs(pb[b] / rb - 1.0)) <= 1e-5
+    ag.free_workspace()
+
+
+def test_c4_full_size_lockstep(orc):
     import paper_1909_06374_b200 as ag
     from paper_1909_06374_b200 import workloads
     cfg = workloads.config("C4")
     B, N = cfg["B"], cfg["N"]
-    assert (B, N) == (4, 2 ** 26)
+    assert (B, N, cfg["max_iter"]) == (4, 2 ** 26, 50)
     srt, perm, _ = ag.agnvar_erdf_sample_sorted(cfg["erdf"], B, N, "f32", cfg["seed"], 0, cfg["grid_points"])
     _, an = ag.agnvar_tk_generate(cfg["psd"], B, N, cfg["dt"], cfg["oversample"], "f32", cfg["seed"], 0,
                                   want_xnorm=False)
-    # S1 at full size: the sorted draw is ascending and perm0 is a valid permutation
+    # S1 at full size: the sorted draw is ascending
     assert bool((srt[:, 1:] >= srt[:, :-1]).all())
-    # first step (fills x_sim,2 and the permutation after one iteration), then the step that is checked
-    o1 = ag.agnvar_e13_iterate(an, srt, perm, 1, want_hist=True)
-    perm_prev = perm.clone()
-    x_prev = o1["x"].clone()
-    del o1
-    out = ag.agnvar_e13_iterate(an, srt, perm, 1, want_hist=True, want_xadj=True)
-    torch.cuda.synchronize()
-    xadj, x, hist = out["x_adj"], out["x"], out["changed_hist"]
-    ar = torch.arange(N, device="cuda")
-    for b in range(B):
-        p = perm[b].long()
-        seen = torch.zeros(N, dtype=torch.uint8, device="cuda")
-        seen[p] = 1
-        assert bool(seen.all()), "not a permutation"
-        del seen
-        xa = (xadj[b] + 0.0)[p]                        # -0 -> +0 (Q13)
-        assert bool((xa[1:] >= xa[:-1]).all()), "x_adj is not sorted along the permutation"
-        tie = xa[1:] == xa[:-1]
-        assert bool((p[1:][tie] > p[:-1][tie]).all()), "equal keys are not in time-index order"
-        del xa, tie
-        assert torch.equal(x[b][p], srt[b]), "rank scatter"
-        assert int(hist[b, 0]) == int((perm[b] != perm_prev[b]).sum()), "change count"
-        del p
-    del ar
-    # one curve, one whole step, against the fp64 oracle started from the GPU's own x_sim
-    b = 1
-    xadj64, _, _, _ = orc.e13_step(an[b].cpu().numpy(), srt[b].cpu().numpy(), u32(perm_prev[b]).copy(),
-                                   x_prev[b].cpu().numpy())
-    xg = xadj[b].cpu().numpy().astype(np.float64)
-    rel = np.linalg.norm(xg - xadj64) / np.linalg.norm(xadj64)
-    assert rel <= 1e-5, rel
-    eps = np.max(np.abs(xg - xadj64))
-    pn = u32(perm[b])
-    assert (np.diff(xadj64[pn]) >= -2.0 * eps).all()
-    print(f"C4 full size: x_adj rel L2 {rel:.2e}, eps {eps:.2e}, changed {hist[:, 0].tolist()}")
+    b_chk = 1
+    an_h, srt_h = an[b_chk].cpu().numpy(), srt[b_chk].cpu().numpy()
+    done = 0
+    for k_check in (2, 25, 50):
+        # the product kernels up to iteration k_check - 1, then the step that is checked
+        o = ag.agnvar_e13_iterate(an, srt, perm, k_check - 1 - done, want_fallbacks=True)
+        assert int(o["sort_fallbacks"].sum()) == 0, "a curve left the distribution sort"
+        done = k_check - 1
+        perm_prev = perm.clone()
+        x_prev = o["x"].clone()
+        del o
+        out = ag.agnvar_e13_iterate(an, srt, perm, 1, want_hist=True, want_xadj=True, want_fallbacks=True)
+        done += 1
+        torch.cuda.synchronize()
+        xadj, x, hist = out["x_adj"], out["x"], out["changed_hist"]
+        assert int(out["sort_fallbacks"].sum()) == 0
+        for b in range(B):
+            p = perm[b].long()
+            seen = torch.zeros(N, dtype=torch.uint8, device="cuda")
+            seen[p] = 1
+            assert bool(seen.all()), "not a permutation"
+            del seen
+            xa = (xadj[b] + 0.0)[p]                        # -0 -> +0 (Q13)
+            assert bool((xa[1:] >= xa[:-1]).all()), "x_adj is not sorted along the permutation"
+            tie = xa[1:] == xa[:-1]
+            assert bool((p[1:][tie] > p[:-1][tie]).all()), "equal keys are not in time-index order"
+            del xa, tie
+            assert torch.equal(x[b][p], srt[b]), "rank scatter"
+            assert int(hist[b, 0]) == int((perm[b] != perm_prev[b]).sum()), "change count"
+            del p
+        # one curve, one whole step, against the fp64 oracle started from the GPU's own x_sim
+        xadj64, _, xnext64, _ = orc.e13_step(an_h, srt_h, u32(perm_prev[b_chk]).copy(), x_prev[b_chk].cpu().numpy())
+        xg = xadj[b_chk].cpu().numpy().astype(np.float64)
+        rel = np.linalg.norm(xg - xadj64) / np.linalg.norm(xadj64)
+        assert rel <= 1e-5, rel
+        eps = np.max(np.abs(xg - xadj64))
+        pn = u32(perm[b_chk])
+        assert (np.diff(xadj64[pn]) >= -2.0 * eps).all()
+        eq = float(np.mean(x[b_chk].cpu().numpy().astype(np.float64) == xnext64))
+        print(f"C4 full size, iteration {k_check}: x_adj rel L2 {rel:.2e}, eps {eps:.2e}, one-step value-equal "
+              f"fraction {eq:.4f}, changed {hist[:, 0].tolist()}")
+        del xadj, x, out, x_prev, perm_prev, xadj64, xnext64, xg
+    ag.free_workspace()

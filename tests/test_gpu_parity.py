@@ -54,16 +54,45 @@ def test_psd_bpl(ag, orc):
 
 
 # ---- S1 -------------------------------------------------------------------------------------------
+BASE_DRAW_TOL = {"f32": 1e-6, "f64": 1e-12}          # BASELINE / SURVEY 8(c): lambda draws, relative
+CAP_DRAW_TOL = {"f32": 1e-6, "f64": 1e-9}
+
+
 def _draw_tol(dtype, u_k, C_k, U):
     """Per-sample relative tolerance of lambda = 10^u, u = u_k + (U - C_k)/(C_{k+1} - C_k) D (DESIGN.md
     "tolerances"): both sides build C by a 4096-term fp64 sum of pow() values that differ in the last
-    ulp (libm vs device), so C carries an absolute error e_C ~ 64 ulp(1); the interpolation divides it
-    by the bin mass, and d(lambda)/lambda = ln(10) du.  fp32 output adds half an ulp of fp32."""
+    ulp (libm vs device), so C carries an absolute error e_C ~ 64 ulp(1) (the premise -- the two tables agree to
+    1e-13 -- is test_erdf_table_matches_oracle below); the interpolation divides it by the bin mass, and
+    d(lambda)/lambda = ln(10) du.  fp32 output adds half an ulp of fp32.  Capped: never looser than 1e-9 (fp64) /
+    1e-6 (fp32), whatever the bin mass."""
     k = np.clip(np.searchsorted(C_k, U, side="right") - 1, 0, C_k.size - 2)
     D = u_k[1] - u_k[0]
     e_C = 64 * 2.220446049250313e-16
     tol = 1e-13 + np.log(10.0) * D * 2.0 * e_C / (C_k[k + 1] - C_k[k])
-    return tol + (6e-8 if dtype == "f32" else 0.0)
+    return np.minimum(tol + (6e-8 if dtype == "f32" else 0.0), CAP_DRAW_TOL[dtype])
+
+
+@pytest.mark.parametrize("erdf", [BPL, LOGN, dict(kind=0, lam_star=0.05, delta1=0.2, delta2=2.2, lam_min=1e-6, lam_max=1.0)],
+                         ids=["bpl", "lognormal", "c4"])
+@pytest.mark.parametrize("G", [2, 1000, 4096, 65536])
+def test_erdf_table_matches_oracle(ag, orc, erdf, G):
+    """The GPU's own cumulative table (through agnvar_erdf_table: the kernel body agnvar_erdf_sample_sorted runs)
+    against the oracle's: <= 1e-13 (SURVEY 8(c) "PSD table and CDF table ... relative <= 1e-13")."""
+    got = ag.agnvar_erdf_table(erdf, G).cpu().numpy()[0]
+    _, _, ref = orc.erdf_table(erdf, G)
+    assert got[0] == 0.0 and got[-1] == 1.0
+    err = np.max(np.abs(got - ref))          # C is in [0, 1]: absolute on that scale
+    rel = np.max(np.abs(got[1:] / ref[1:] - 1.0))
+    print(f"G={G}: CDF table max abs err {err:.2e}, max rel err {rel:.2e}")
+    assert err <= 1e-13 and rel <= 1e-12
+
+
+def test_erdf_table_per_curve(ag, orc):
+    from paper_1909_06374_b200 import workloads
+    cfg = workloads.config("C5", B=40)         # more tables than one argument batch of the table kernel
+    got = ag.agnvar_erdf_table(cfg["erdf"], 4096).cpu().numpy()
+    for b in (0, 1, 31, 32, 39):
+        assert np.max(np.abs(got[b] - orc.erdf_table(cfg["erdf"][b], 4096)[2])) <= 1e-13
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
@@ -74,14 +103,23 @@ def test_erdf_sample_sorted(ag, orc, dtype, N, erdf):
     srt, perm0, draw = ag.agnvar_erdf_sample_sorted(erdf, B, N, dtype, seed, curve0, 4096, want_draw=True)
     srt, perm0, draw = srt.cpu().numpy(), u32(perm0), draw.cpu().numpy()
     u_k, _, C_k = orc.erdf_table(erdf, 4096)
+    worst, n_over = 0.0, 0
     for b in range(B):
         lam, U = orc.erdf_draw(erdf, 4096, N, seed, curve0 + b, 0 if dtype == "f32" else 1)
-        assert np.max(np.abs(draw[b].astype(np.float64) / lam - 1.0)) <= _draw_tol(dtype, u_k, C_k, U).max()
-        assert np.all(np.abs(draw[b].astype(np.float64) / lam - 1.0) <= _draw_tol(dtype, u_k, C_k, U))
+        err = np.abs(draw[b].astype(np.float64) / lam - 1.0)
+        assert np.all(err <= _draw_tol(dtype, u_k, C_k, U))
+        worst = max(worst, float(err.max()))
+        n_over += int(np.count_nonzero(err > BASE_DRAW_TOL[dtype]))
         # order and perm0 bit-exact given the same lambda array (the GPU's own draw)
         ref_perm = orc.stable_argsort(draw[b].astype(np.float64))
         assert (perm0[b] == ref_perm).all()
         assert (srt[b] == draw[b][ref_perm]).all()
+    print(f"{dtype} N={N}: max relative lambda error {worst:.2e}; samples above the BASELINE tolerance "
+          f"{BASE_DRAW_TOL[dtype]:g}: {n_over} of {B * N}")
+    # observed on B200 (round 2): fp64 max 4.1e-12 with 0.1-0.4 % of the samples above 1e-12 (ulp-level pow()
+    # differences in the 4096-term table sum, divided by the cell mass); fp32 max 6e-8, none above 1e-6
+    assert worst <= (2e-11 if dtype == "f64" else 1e-6)
+    assert n_over <= max(2, B * N // 100)
 
 
 def test_erdf_per_curve_tables(ag, orc):
@@ -106,6 +144,26 @@ def test_tk_generate(ag, orc, dtype, N, os_):
         ref = orc.tk_generate(0.0, PSD["f_b"], 1.0, 2.0, N, 1.0, os_, seed, curve0 + b)
         assert rel_l2(xn[b], ref["x_norm"]) <= TOL[dtype]
         assert rel_l2(an[b], ref["A_norm"]) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("name,B", [("C2", 4), ("C5", 8)])
+def test_tk_generate_per_curve_psd(ag, orc, name, B):
+    """n_psd == B: every curve has its own (f_b, alpha_low, alpha_high) -- the path C2 (4096 different f_b) and C5
+    (65536 different slopes and bends) take through psd[b] in the fill and normalisation kernels."""
+    from paper_1909_06374_b200 import workloads
+    cfg = workloads.config(name, B=B)
+    assert len(cfg["psd"]) == B and len({p["f_b"] for p in cfg["psd"]}) == B
+    N, os_, dtype = cfg["N"], cfg["oversample"], cfg["dtype"]
+    xn, an = ag.agnvar_tk_generate(cfg["psd"], B, N, cfg["dt"], os_, dtype, cfg["seed"], 5)
+    xn, an = xn.cpu().numpy(), an.cpu().numpy()
+    for b in range(B):
+        p = cfg["psd"][b]
+        ref = orc.tk_generate(0.0, p["f_b"], p["alpha_low"], p["alpha_high"], N, cfg["dt"], os_, cfg["seed"], 5 + b)
+        assert rel_l2(xn[b], ref["x_norm"]) <= TOL[dtype]
+        assert rel_l2(an[b], ref["A_norm"]) <= TOL[dtype]
+    # and the same curves are reproduced one at a time (psd[b] really is curve b's)
+    x1, a1 = ag.agnvar_tk_generate(cfg["psd"][2], 1, N, cfg["dt"], os_, dtype, cfg["seed"], 7)
+    assert np.array_equal(x1.cpu().numpy()[0], xn[2]) and np.array_equal(a1.cpu().numpy()[0], an[2])
 
 
 # ---- P --------------------------------------------------------------------------------------------
@@ -157,6 +215,19 @@ def test_e13_fp64_trajectory_identical(ag, orc, N, os_):
         assert (perm[b] == ref["perm"]).all()
         assert (x[b] == ref["x"]).all()
         assert (np.sort(x[b]) == srt_h[b]).all()
+
+
+def test_e13_fp64_long_curve_trajectory(ag, orc):
+    """fp64 above the one-CTA sort (N = 2^22: generic FFT passes, LSD sweeps, two-level rank scatter): the
+    trajectory is still the oracle's, bit for bit."""
+    N, B, max_iter = 2 ** 22, 1, 2
+    srt, perm0, an = _inputs(ag, BPL, PSD, B, N, 1, "f64", 4)
+    srt_h, perm_h, an_h = srt.cpu().numpy(), u32(perm0).copy(), an.cpu().numpy()
+    out = ag.agnvar_e13_iterate(an, srt, perm0, max_iter, want_hist=True)
+    ref = orc.e13_iterate(an_h[0], srt_h[0], perm_h[0], max_iter)
+    assert (out["changed_hist"].cpu().numpy()[0] == ref["changed_hist"]).all()
+    assert (u32(out["perm"])[0] == ref["perm"]).all()
+    assert (out["x"].cpu().numpy()[0] == ref["x"]).all()
 
 
 @pytest.mark.parametrize("N,os_,erdf", [(1024, 1, BPL), (4096, 10, BPL), (2 ** 14, 10, BPL), (2 ** 15, 1, LOGN),
@@ -304,8 +375,65 @@ def test_error_codes(ag):
     a = torch.zeros((1, 513), device="cuda")
     ws = torch.zeros(256, dtype=torch.uint8, device="cuda")
     vp = lambda t: C.c_void_p(t.data_ptr())
-    st = L.agnvar_e13_iterate(1, 1024, 0, vp(a), vp(x), vp(p), vp(x), 1, None, None, None, vp(ws), 256, None)
+    st = L.agnvar_e13_iterate(1, 1024, 0, vp(a), vp(x), vp(p), vp(x), 1, None, None, None, None, vp(ws), 256, None)
     assert st == 2                                                # workspace too small
-    st = L.agnvar_e13_iterate(1, 1024, 0, vp(a), vp(x), vp(p), vp(x), 0, None, None, None, vp(ws), 256, None)
+    st = L.agnvar_e13_iterate(1, 1024, 0, vp(a), vp(x), vp(p), vp(x), 0, None, None, None, None, vp(ws), 256, None)
     assert st == 1                                                # max_iter < 1
     assert ag.strerror(2).startswith("workspace")
+
+
+# ---- NEXT-1: delta_i (Eq. 4) -------------------------------------------------------
+@pytest.mark.parametrize("N,os_", [(256, 1), (1024, 1), (4096, 10), (2 ** 14, 1)])
+def test_delta_fp64_trajectory_and_threshold(ag, orc, N, os_):
+    """fp64: delta_k of every iteration equals the oracle's (<= 1e-12 relative: device log10 vs libm), and a
+    threshold stops each curve at the oracle's k with the oracle's state."""
+    B, max_iter = 3, 30
+    srt, perm0, an = _inputs(ag, BPL, PSD, B, N, os_, "f64", 6)
+    srt_h, perm_h, an_h = srt.cpu().numpy(), u32(perm0).copy(), an.cpu().numpy()
+    free = ag.agnvar_e13_iterate(an, srt, perm0.clone(), max_iter, want_hist=True, want_delta=True)
+    dh = free["delta_hist"].cpu().numpy()
+    refs = [orc.e13_iterate_delta(an_h[b], srt_h[b], perm_h[b], max_iter, 0.0) for b in range(B)]
+    for b in range(B):
+        k = refs[b]["iters_used"]
+        assert int(free["iters_used"][b]) == k
+        assert np.allclose(dh[b][:k], refs[b]["delta_hist"][:k], rtol=1e-12, atol=0)
+        assert (u32(free["perm"])[b] == refs[b]["perm"]).all()
+    # a threshold that different curves reach at different iterations (well away from any delta_k: no tie-breaking)
+    thr = float(np.sqrt(refs[0]["delta_hist"][3] * refs[0]["delta_hist"][4]))
+    out = ag.agnvar_e13_iterate(an, srt, perm0.clone(), max_iter, want_hist=True, want_delta=True, delta_threshold=thr)
+    for b in range(B):
+        ref = orc.e13_iterate_delta(an_h[b], srt_h[b], perm_h[b], max_iter, thr)
+        k = ref["iters_used"]
+        assert int(out["iters_used"][b]) == k
+        assert (u32(out["perm"])[b] == ref["perm"]).all()
+        assert (out["x"][b].cpu().numpy() == ref["x"]).all()
+        assert np.allclose(out["delta_hist"][b].cpu().numpy()[:k], ref["delta_hist"][:k], rtol=1e-12, atol=0)
+    # check_every > 0: the call returns early once every curve has stopped, with the same result
+    early = ag.agnvar_e13_iterate(an, srt, perm0.clone(), max_iter, delta_threshold=thr, check_every=2)
+    assert torch.equal(early["iters_used"], out["iters_used"]) and torch.equal(early["x"], out["x"])
+    assert torch.equal(early["perm"], out["perm"])
+
+
+@pytest.mark.parametrize("N,erdf", [(1024, BPL), (2 ** 15, LOGN), (2 ** 18, BPL), (2 ** 22, BPL)])
+def test_delta_fp32_lockstep(ag, orc, N, erdf):
+    """fp32: delta_k is a function of the two consecutive series the GPU itself produced (exact fp32 values), so it is
+    compared with the oracle's Eq. 4 evaluated on those very series: <= 1e-6 relative."""
+    B, K = 2, 3
+    srt, perm, an = _inputs(ag, erdf, PSD, B, N, 1, "f32", 8)
+    srt_h = srt.cpu().numpy()
+    x_prev = np.empty((B, N), dtype=np.float32)
+    p0 = u32(perm)
+    for b in range(B):
+        x_prev[b][p0[b]] = srt_h[b]
+    for k in range(K):
+        out = ag.agnvar_e13_iterate(an, srt, perm, 1, want_delta=True)
+        x = out["x"].cpu().numpy()
+        d = out["delta_hist"].cpu().numpy()[:, 0]
+        for b in range(B):
+            want = orc.delta_rms(x[b].astype(np.float64), x_prev[b].astype(np.float64))
+            assert d[b] == pytest.approx(want, rel=1e-6)
+        x_prev = x.copy()
+    # delta mode leaves the trajectory itself untouched
+    srt2, perm2, an2 = _inputs(ag, erdf, PSD, B, N, 1, "f32", 8)
+    plain = ag.agnvar_e13_iterate(an2, srt2, perm2, K)
+    assert torch.equal(plain["x"], out["x"]) and torch.equal(perm2, perm)

@@ -50,17 +50,31 @@ def test_workspace_query_and_validation(L):
     assert L.agnvar_tk_generate(C.byref(good), 1, 1, 1000, 1.0, 1, 0, 0, 0, one, one, one, 1 << 40, None) == 1
     assert L.agnvar_tk_generate(C.byref(good), 1, 1, 1024, 1.0, 1, 0, 0, 0, None, None, one, 1 << 40, None) == 1
     assert L.agnvar_tk_generate(C.byref(good), 1, 1, 2 ** 27, 1.0, 4, 0, 0, 0, one, one, one, 1 << 40, None) == 4
-    assert L.agnvar_e13_iterate(1, 1024, 0, one, one, one, one, 0, None, None, None, one, 1 << 40, None) == 1
-    assert L.agnvar_e13_iterate(1, 1024, 7, one, one, one, one, 1, None, None, None, one, 1 << 40, None) == 1
-    assert L.agnvar_e13_iterate(1, 1024, 0, one, one, one, one, 1, None, None, None, one, 16, None) == 2
+    assert L.agnvar_e13_iterate(1, 1024, 0, one, one, one, one, 0, None, None, None, None, one, 1 << 40, None) == 1
+    assert L.agnvar_e13_iterate(1, 1024, 7, one, one, one, one, 1, None, None, None, None, one, 1 << 40, None) == 1
+    assert L.agnvar_e13_iterate(1, 1024, 0, one, one, one, one, 1, None, None, None, None, one, 16, None) == 2
+    bad = b.agnvar_e13_opts(float("nan"), None, None, 0, 0)
+    assert L.agnvar_e13_iterate(1, 1024, 0, one, one, one, one, 1, None, None, None, C.byref(bad), one, 1 << 40, None) == 1
+    bad = b.agnvar_e13_opts(0.0, None, None, -1, 0)
+    assert L.agnvar_e13_iterate(1, 1024, 0, one, one, one, one, 1, None, None, None, C.byref(bad), one, 1 << 40, None) == 1
+    # the delta_i rule needs more scratch (two value buffers, one permutation)
+    assert b.workspace_bytes(b.OP_E13_ITERATE, 2, 4096, "f32", 1, 1) >= b.workspace_bytes(b.OP_E13_ITERATE, 2, 4096, "f32") + 3 * 2 * 4096 * 4
     e = b.agnvar_erdf(0, 0, 0.1, 0.4, 2.4, 0.0, 1.0, 1e-4, 1e-5)
     assert L.agnvar_erdf_sample_sorted(C.byref(e), 1, 1, 1024, 0, 0, 0, 4096, one, one, None, one, 1 << 40, None) == 1
+    assert L.agnvar_erdf_table(C.byref(e), 1, 4096, one, None) == 1
     edges = (C.c_int64 * 3)(1, 5, 4)
     assert L.agnvar_periodogram(1, 1024, 0, one, 1.0, 0, 2, edges, one, None, one, 1 << 40, None) == 1
     assert L.agnvar_psd_bpl(None, -1, C.byref(good), None, None) == 1
     assert L.agnvar_philox_u32(0, 0, -1, 0, 0, None, None) == 1
     assert L.agnvar_strerror(1).decode() == "invalid argument"
     assert b"sm_100a" in L.agnvar_version()
+
+
+def test_library_is_built_from_these_sources(L):
+    """The staleness test is a hash of the sources compiled into the library, not file times."""
+    from paper_1909_06374_b200 import _build
+    assert _build.source_hash().encode() in L.agnvar_version()
+    assert _build.is_fresh()
 
 
 def test_workloads_are_seeded_and_shaped():
@@ -70,5 +84,14 @@ def test_workloads_are_seeded_and_shaped():
     assert all(1e-3 <= p["f_b"] <= 2e-2 for p in c2a["psd"])
     c4 = w.config("C4")
     assert (c4["B"], c4["N"], c4["max_iter"], c4["dtype"]) == (4, 2 ** 26, 50, "f32")
+    # per-curve parameters come from Philox stream tag 2; the module's own generator reproduces the
+    # published known-answer vectors, and curve b's parameters do not depend on the subset size
+    assert [hex(v) for v in w._philox_words(0, 0, 0, 0, 0)] == ["0x6627e8d5", "0xe169c58d", "0xbc57ac4c", "0x9b00dbd8"]
+    assert [hex(v) for v in w._philox_words(0xa4093822 | (0x299f31d0 << 32), 0x243f6a88, 0x85a308d3, 0x13198a2e,
+                                            0x03707344)] == ["0xd16cfe09", "0x94fdcceb", "0x5001e420", "0x24126ea1"]
+    assert w.config("C2", B=3)["psd"] == c2a["psd"][:3]
+    c5 = w.config("C5", B=4)
+    assert all(0.5 <= p["alpha_low"] <= 1.5 and 2.0 <= p["alpha_high"] <= 3.0 and 1e-3 <= p["f_b"] <= 1e-1 for p in c5["psd"])
+    assert all(0.1 <= q["delta1"] <= 0.6 and 2.0 <= q["delta2"] <= 3.0 for q in c5["erdf"])
     e = w.log_bin_edges(2 ** 20, 64)
     assert e[0] == 1 and e[-1] == 2 ** 19 + 1 and all(a < b for a, b in zip(e, e[1:]))
