@@ -46,7 +46,9 @@ typedef enum {
     AGNVAR_OP_ERDF_SAMPLE_SORTED = 1,
     AGNVAR_OP_TK_GENERATE = 2,
     AGNVAR_OP_E13_ITERATE = 3,
-    AGNVAR_OP_PERIODOGRAM = 4
+    AGNVAR_OP_PERIODOGRAM = 4,
+    AGNVAR_OP_STRUCTURE_FUNCTION = 5,
+    AGNVAR_OP_DELTA_M_PROB = 6
 } agnvar_op;
 
 /* Eq. 3: PSD(f) = A [ (f/f_b)^alpha_low + (f/f_b)^alpha_high ]^-1.
@@ -70,7 +72,7 @@ typedef struct {
 
 /* Bytes of scratch the given op needs.  `oversample` matters for AGNVAR_OP_TK_GENERATE only
  * (pass 1 otherwise); `aux` = grid_points for ERDF_SAMPLE_SORTED, nbins for PERIODOGRAM, 1 for E13_ITERATE
- * with the delta_i rule / history (see agnvar_e13_opts), else 0.
+ * with the delta_i rule / history (see agnvar_e13_opts), nlags for STRUCTURE_FUNCTION and DELTA_M_PROB, else 0.
  * Returns 0 for invalid arguments. */
 size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int oversample, int64_t aux);
 
@@ -177,6 +179,32 @@ int agnvar_e13_iterate(int64_t B, int64_t N, int dtype, const void* d_anorm, con
 int agnvar_periodogram(int64_t B, int64_t N, int dtype, const void* d_x, double dt, int norm, int nbins,
                        const int64_t* h_bin_edges_j, double* d_out, int64_t* d_counts, void* d_ws,
                        size_t ws_bytes, void* stream);
+
+/* SF -- structure function of evenly sampled light curves (Eq. A6) at nlags integer lags l (tau = l dt):
+ *   SF(tau)^2 = (1/P) sum over the P = N - l pairs (i, i + l) of [ v_i - v_{i+l} ]^2,
+ * v = x (L/L_Edd units, mag = 0) or v = -2.5 log10 x (magnitudes, mag = 1; for a constant bolometric
+ * correction m(t2) - m(t1) = -2.5 log10[L(t2)/L(t1)], the zero point cancels; needs x > 0).  Differences and sums in fp64.
+ *   h_lags       nlags integers, 1 <= l; a lag l >= N has no pair: sf2 = 0, pairs = 0
+ *   d_sf2        out [B][nlags] fp64
+ *   d_pairs      out [nlags] i64 or NULL: P = N - l
+ *   d_rep_mean, d_rep_stderr   out [nlags] fp64 or NULL: the representative SF over the B realisations (Eq. 6,
+ *                PAPER.md:244-251): mean of SF_i(tau)^2 and its standard error (sample std / sqrt(B); 0 for B = 1)
+ * EINVAL: bad B/N/dtype, nlags < 1 or > 4096, a lag < 1, NULL h_lags/d_x/d_sf2. */
+int agnvar_structure_function(int64_t B, int64_t N, int dtype, const void* d_x, const int64_t* h_lags, int nlags, int mag,
+                              double* d_sf2, int64_t* d_pairs, double* d_rep_mean, double* d_rep_stderr, void* d_ws,
+                              size_t ws_bytes, void* stream);
+
+/* dM -- P(|dm| > dm_ref given tau) (Figs 16-17): per curve and lag, the number of pairs (i, i + l)
+ * with |m_i - m_{i+l}| > dm_ref divided by the number of pairs considered, m = m_zero - 2.5 log10 x (fp64).
+ * use_cut != 0: every point with m > m_cut is replaced by the upper limit m_cut and only pairs in which at least one
+ * point is detected (m <= m_cut) are considered (Fig. 17); use_cut = 0: all N - l pairs.
+ *   h_dm_ref      nref thresholds (1 <= nref <= 16)
+ *   d_prob        out [B][nlags][nref] fp64 (0 where no pair is considered)
+ *   d_considered  out [B][nlags] i64 or NULL
+ * EINVAL: as above, nref out of range, non-finite m_zero / m_cut / dm_ref, NULL h_dm_ref/d_prob. */
+int agnvar_delta_m_prob(int64_t B, int64_t N, int dtype, const void* d_x, const int64_t* h_lags, int nlags,
+                        const double* h_dm_ref, int nref, double m_zero, int use_cut, double m_cut, double* d_prob,
+                        int64_t* d_considered, void* d_ws, size_t ws_bytes, void* stream);
 
 /* O1 -- the raw random words every other call consumes (for bit-exact checks of the generator):
  * d_out[4 i + w] = word w of Philox4x32-10 with counter (lo(i0+i), hi(i0+i), curve, tag) and key

@@ -14,12 +14,13 @@ from . import _build
 
 AGNVAR_F32, AGNVAR_F64 = 0, 1
 AGNVAR_ERDF_BPL, AGNVAR_ERDF_LOGNORMAL = 0, 1
-OP_ERDF_SAMPLE_SORTED, OP_TK_GENERATE, OP_E13_ITERATE, OP_PERIODOGRAM = 1, 2, 3, 4
+OP_ERDF_SAMPLE_SORTED, OP_TK_GENERATE, OP_E13_ITERATE, OP_PERIODOGRAM, OP_STRUCTURE_FUNCTION, OP_DELTA_M_PROB = 1, 2, 3, 4, 5, 6
 
 EXPORTS = (
     "agnvar_workspace_bytes", "agnvar_psd_bpl", "agnvar_erdf_sample_sorted", "agnvar_erdf_table", "agnvar_tk_generate",
     "agnvar_e13_iterate", "agnvar_periodogram", "agnvar_philox_u32", "agnvar_strerror", "agnvar_version",
     "agnvar_launch_count", "agnvar_trace_begin", "agnvar_trace_end", "agnvar_kernel_name",
+    "agnvar_structure_function", "agnvar_delta_m_prob",
 )
 
 
@@ -79,6 +80,11 @@ def lib():
     L.agnvar_erdf_table.argtypes = [C.POINTER(agnvar_erdf), i64, i32, vp, vp]
     L.agnvar_periodogram.restype = i32
     L.agnvar_periodogram.argtypes = [i64, i64, i32, vp, dbl, i32, i32, C.POINTER(i64), vp, vp, vp, sz, vp]
+    L.agnvar_structure_function.restype = i32
+    L.agnvar_structure_function.argtypes = [i64, i64, i32, vp, C.POINTER(i64), i32, i32, vp, vp, vp, vp, vp, sz, vp]
+    L.agnvar_delta_m_prob.restype = i32
+    L.agnvar_delta_m_prob.argtypes = [i64, i64, i32, vp, C.POINTER(i64), i32, C.POINTER(dbl), i32, dbl, i32, dbl, vp, vp,
+                                      vp, sz, vp]
     L.agnvar_philox_u32.restype = i32
     L.agnvar_philox_u32.argtypes = [u64, u64, i64, u32, u32, vp, vp]
     L.agnvar_strerror.restype = C.c_char_p
@@ -305,3 +311,40 @@ def agnvar_periodogram(x, dt, norm=0, bin_edges=None):
         _check(lib().agnvar_periodogram(B, N, code, _ptr(x), float(dt), int(norm), nbins, edges, _ptr(out), _ptr(counts),
                                         _ptr(ws), ws.numel(), _stream()), "agnvar_periodogram")
     return out if not nbins else (out, counts)
+
+
+def agnvar_structure_function(x, lags, mag=False, want_rep=False):
+    """NEXT-2 (Eq. A6): x [B][N] -> dict(sf2 [B][nlags] fp64, pairs [nlags] i64, rep_mean / rep_stderr [nlags] | None)."""
+    B, N = x.shape
+    code, _ = _dt(x.dtype)
+    dev = x.device
+    nl = len(lags)
+    arr = (C.c_int64 * nl)(*[int(l) for l in lags])
+    with _on(dev):
+        sf2 = torch.empty((B, nl), dtype=torch.float64, device=dev)
+        pairs = torch.empty((nl,), dtype=torch.int64, device=dev)
+        mean = torch.empty((nl,), dtype=torch.float64, device=dev) if want_rep else None
+        se = torch.empty((nl,), dtype=torch.float64, device=dev) if want_rep else None
+        ws = workspace(workspace_bytes(OP_STRUCTURE_FUNCTION, B, N, code, 1, nl), dev)
+        _check(lib().agnvar_structure_function(B, N, code, _ptr(x), arr, nl, 1 if mag else 0, _ptr(sf2), _ptr(pairs),
+                                               _ptr(mean), _ptr(se), _ptr(ws), ws.numel(), _stream()),
+               "agnvar_structure_function")
+    return {"sf2": sf2, "pairs": pairs, "rep_mean": mean, "rep_stderr": se}
+
+
+def agnvar_delta_m_prob(x, lags, dm_ref, m_zero=0.0, m_cut=None):
+    """NEXT-2 (PAPER.md:465-473): x [B][N] -> (prob [B][nlags][nref] fp64, considered [B][nlags] i64)."""
+    B, N = x.shape
+    code, _ = _dt(x.dtype)
+    dev = x.device
+    nl, nr = len(lags), len(dm_ref)
+    larr = (C.c_int64 * nl)(*[int(l) for l in lags])
+    rarr = (C.c_double * nr)(*[float(r) for r in dm_ref])
+    with _on(dev):
+        prob = torch.empty((B, nl, nr), dtype=torch.float64, device=dev)
+        cons = torch.empty((B, nl), dtype=torch.int64, device=dev)
+        ws = workspace(workspace_bytes(OP_DELTA_M_PROB, B, N, code, 1, nl), dev)
+        _check(lib().agnvar_delta_m_prob(B, N, code, _ptr(x), larr, nl, rarr, nr, float(m_zero), 0 if m_cut is None else 1,
+                                         0.0 if m_cut is None else float(m_cut), _ptr(prob), _ptr(cons), _ptr(ws),
+                                         ws.numel(), _stream()), "agnvar_delta_m_prob")
+    return prob, cons

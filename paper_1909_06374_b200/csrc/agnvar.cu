@@ -9,6 +9,7 @@
 #include "kernels.cuh"
 #include "fft2.cuh"
 #include "sort32.cuh"
+#include "sf.cuh"
 
 #include <cmath>
 #include <cstring>
@@ -427,6 +428,68 @@ int pgram_impl(int64_t B, int64_t N, const void* d_x, double dt, int norm, int n
     return cuda_status(cudaGetLastError());
 }
 
+// ---- NEXT-2: structure function, Delta-m probabilities --------------------------------------------------------
+inline int sf_chunks(int64_t N) { return (int)((N + kSfChunk - 1) / kSfChunk); }
+inline size_t ws_sf(int64_t B, int64_t N, int64_t nlags, bool counts) {
+    Carver c(nullptr);
+    c.take<long long>((size_t)nlags);
+    c.take<double>((size_t)B * N);                                  // magnitudes
+    c.take<unsigned char>((size_t)B * N);                           // detection flags
+    if (counts) {
+        c.take<unsigned long long>((size_t)B * nlags * kSfMaxRef);
+        c.take<unsigned long long>((size_t)B * nlags);
+    } else {
+        c.take<double>((size_t)B * nlags * sf_chunks(N));
+    }
+    return c.off;
+}
+
+template <typename T>
+int sf_impl(int64_t B, int64_t N, const void* d_x, const int64_t* h_lags, int nlags, int mag, double* d_sf2,
+            int64_t* d_pairs, double* d_mean, double* d_se, void* d_ws, size_t ws_bytes, cudaStream_t st) {
+    if (ws_bytes < ws_sf(B, N, nlags, false) || !d_ws || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
+    Carver c(d_ws);
+    long long* lags = c.take<long long>((size_t)nlags);
+    double* mags = c.take<double>((size_t)B * N);
+    c.take<unsigned char>((size_t)B * N);
+    const int nch = sf_chunks(N);
+    double* partial = c.take<double>((size_t)B * nlags * nch);
+    CK(cudaMemcpyAsync(lags, h_lags, (size_t)nlags * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    const dim3 grid((unsigned)nch, (unsigned)nlags, (unsigned)B);
+    if (mag) {
+        AGN_LAUNCH(K_SF, st, (sf_mag_kernel<T><<<cdiv(B * N, 256), 256, 0, st>>>((const T*)d_x, (long long)B * N, 0.0, 0, 0.0, mags, nullptr)));
+        AGN_LAUNCH(K_SF, st, (sf_partial_kernel<double><<<grid, 256, 0, st>>>(mags, N, lags, nlags, partial, nch, (int)B)));
+    } else {
+        AGN_LAUNCH(K_SF, st, (sf_partial_kernel<T><<<grid, 256, 0, st>>>((const T*)d_x, N, lags, nlags, partial, nch, (int)B)));
+    }
+    AGN_LAUNCH(K_SF, st, (sf_final_kernel<<<dim3((unsigned)nlags, (unsigned)B), 256, 0, st>>>(partial, nch, N, lags, nlags, d_sf2, (long long*)d_pairs)));
+    if (d_mean || d_se) AGN_LAUNCH(K_SF, st, (sf_rep_kernel<<<(unsigned)nlags, 256, 0, st>>>(d_sf2, (int)B, nlags, d_mean, d_se)));
+    return cuda_status(cudaGetLastError());
+}
+
+template <typename T>
+int dm_impl(int64_t B, int64_t N, const void* d_x, const int64_t* h_lags, int nlags, const double* h_ref, int nref,
+            double m_zero, int use_cut, double m_cut, double* d_prob, int64_t* d_considered, void* d_ws, size_t ws_bytes,
+            cudaStream_t st) {
+    if (ws_bytes < ws_sf(B, N, nlags, true) || !d_ws || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
+    Carver c(d_ws);
+    long long* lags = c.take<long long>((size_t)nlags);
+    double* mags = c.take<double>((size_t)B * N);
+    unsigned char* det = c.take<unsigned char>((size_t)B * N);
+    unsigned long long* counts = c.take<unsigned long long>((size_t)B * nlags * kSfMaxRef);
+    unsigned long long* cons = c.take<unsigned long long>((size_t)B * nlags);
+    CK(cudaMemcpyAsync(lags, h_lags, (size_t)nlags * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    CK(cudaMemsetAsync(counts, 0, (size_t)B * nlags * kSfMaxRef * sizeof(unsigned long long), st));
+    CK(cudaMemsetAsync(cons, 0, (size_t)B * nlags * sizeof(unsigned long long), st));
+    DmRefs refs;
+    for (int r = 0; r < kSfMaxRef; ++r) refs.ref[r] = r < nref ? h_ref[r] : 0.0;
+    AGN_LAUNCH(K_SF, st, (sf_mag_kernel<T><<<cdiv(B * N, 256), 256, 0, st>>>((const T*)d_x, (long long)B * N, m_zero, use_cut, m_cut, mags, det)));
+    const dim3 grid((unsigned)sf_chunks(N), (unsigned)nlags, (unsigned)B);
+    AGN_LAUNCH(K_SF, st, (dm_count_kernel<<<grid, 256, 0, st>>>(mags, det, N, lags, nlags, refs, nref, counts, cons, (int)B)));
+    AGN_LAUNCH(K_SF, st, (dm_final_kernel<<<cdiv(B * nlags * nref, 256), 256, 0, st>>>(counts, cons, (long long)B * nlags, nref, d_prob, (long long*)d_considered)));
+    return cuda_status(cudaGetLastError());
+}
+
 }  // namespace
 
 // =====================================================================================================
@@ -497,6 +560,12 @@ size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int overs
         case AGNVAR_OP_PERIODOGRAM:
             if (aux < 0 || aux > 4096) return 0;
             return f32 ? ws_pgram<float>(B, N, aux) : ws_pgram<double>(B, N, aux);
+        case AGNVAR_OP_STRUCTURE_FUNCTION:
+            if (aux < 1 || aux > 4096 || B > 65535) return 0;
+            return ws_sf(B, N, aux, false);
+        case AGNVAR_OP_DELTA_M_PROB:
+            if (aux < 1 || aux > 4096 || B > 65535) return 0;
+            return ws_sf(B, N, aux, true);
         default: return 0;
     }
 }
@@ -613,6 +682,38 @@ int agnvar_e13_iterate(int64_t B, int64_t N, int dtype, const void* d_anorm, con
                                d_xadj_dbg, opt, d_ws, ws_bytes, (cudaStream_t)stream);
     return e13_impl<double>(B, N, d_anorm, d_sorted, d_perm, d_x, max_iter, d_iters_used, d_changed_hist, d_xadj_dbg,
                             opt, d_ws, ws_bytes, (cudaStream_t)stream);
+}
+
+static bool valid_lags(const int64_t* h_lags, int nlags) {
+    if (!h_lags || nlags < 1 || nlags > 4096) return false;
+    for (int q = 0; q < nlags; ++q)
+        if (h_lags[q] < 1) return false;
+    return true;
+}
+
+int agnvar_structure_function(int64_t B, int64_t N, int dtype, const void* d_x, const int64_t* h_lags, int nlags, int mag,
+                              double* d_sf2, int64_t* d_pairs, double* d_rep_mean, double* d_rep_stderr, void* d_ws,
+                              size_t ws_bytes, void* stream) {
+    if (!valid_BN(B, N) || B > 65535 || !valid_dtype(dtype) || !d_x || !d_sf2 || !valid_lags(h_lags, nlags)) return AGNVAR_EINVAL;
+    if (dtype == AGNVAR_F32)
+        return sf_impl<float>(B, N, d_x, h_lags, nlags, mag, d_sf2, d_pairs, d_rep_mean, d_rep_stderr, d_ws, ws_bytes,
+                              (cudaStream_t)stream);
+    return sf_impl<double>(B, N, d_x, h_lags, nlags, mag, d_sf2, d_pairs, d_rep_mean, d_rep_stderr, d_ws, ws_bytes,
+                           (cudaStream_t)stream);
+}
+
+int agnvar_delta_m_prob(int64_t B, int64_t N, int dtype, const void* d_x, const int64_t* h_lags, int nlags,
+                        const double* h_dm_ref, int nref, double m_zero, int use_cut, double m_cut, double* d_prob,
+                        int64_t* d_considered, void* d_ws, size_t ws_bytes, void* stream) {
+    if (!valid_BN(B, N) || B > 65535 || !valid_dtype(dtype) || !d_x || !d_prob || !valid_lags(h_lags, nlags)) return AGNVAR_EINVAL;
+    if (!h_dm_ref || nref < 1 || nref > kSfMaxRef || !std::isfinite(m_zero) || (use_cut && !std::isfinite(m_cut))) return AGNVAR_EINVAL;
+    for (int r = 0; r < nref; ++r)
+        if (!std::isfinite(h_dm_ref[r])) return AGNVAR_EINVAL;
+    if (dtype == AGNVAR_F32)
+        return dm_impl<float>(B, N, d_x, h_lags, nlags, h_dm_ref, nref, m_zero, use_cut, m_cut, d_prob, d_considered, d_ws,
+                              ws_bytes, (cudaStream_t)stream);
+    return dm_impl<double>(B, N, d_x, h_lags, nlags, h_dm_ref, nref, m_zero, use_cut, m_cut, d_prob, d_considered, d_ws,
+                           ws_bytes, (cudaStream_t)stream);
 }
 
 int agnvar_periodogram(int64_t B, int64_t N, int dtype, const void* d_x, double dt, int norm, int nbins,

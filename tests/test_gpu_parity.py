@@ -437,3 +437,43 @@ def test_delta_fp32_lockstep(ag, orc, N, erdf):
     srt2, perm2, an2 = _inputs(ag, erdf, PSD, B, N, 1, "f32", 8)
     plain = ag.agnvar_e13_iterate(an2, srt2, perm2, K)
     assert torch.equal(plain["x"], out["x"]) and torch.equal(perm2, perm)
+
+
+# ---- NEXT-2: structure function (Eq. A6), representative SF (Eq. 6), P(|dm| > dm_ref | tau) ------------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("N", [64, 4096, 2 ** 17])
+def test_structure_function(ag, orc, dtype, N):
+    """Pair sums in fp64 on both sides (fp32 inputs are exact in fp64): <= 1e-12 relative; pair counts exact."""
+    B = 5
+    srt, perm0, an = _inputs(ag, BPL, PSD, B, N, 1, dtype, 12)
+    x = ag.agnvar_e13_iterate(an, srt, perm0, 5)["x"]
+    xh = x.cpu().numpy().astype(np.float64)
+    lags = sorted({1, 2, 3, 7, 31, 64, N // 3, N - 1, N, 2 * N} | {int(round(10 ** e)) for e in np.linspace(0, np.log10(N // 2), 12)})
+    for mag in (False, True):
+        out = ag.agnvar_structure_function(x, lags, mag=mag, want_rep=True)
+        sf2, pairs = out["sf2"].cpu().numpy(), out["pairs"].cpu().numpy()
+        ref = np.stack([orc.structure_function(xh[b], lags, mag)[0] for b in range(B)])
+        assert (pairs == orc.structure_function(xh[0], lags, mag)[1]).all()
+        assert np.allclose(sf2, ref, rtol=1e-12, atol=0)
+        mean, se = orc.sf_representative(ref)
+        assert np.allclose(out["rep_mean"].cpu().numpy(), mean, rtol=1e-12, atol=0)
+        assert np.allclose(out["rep_stderr"].cpu().numpy(), se, rtol=1e-10, atol=1e-300)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_delta_m_probability(ag, orc, dtype):
+    """Integer pair counts: the probabilities are exact ratios of the oracle's counts (both sides classify in fp64)."""
+    B, N = 3, 2 ** 15
+    srt, perm0, an = _inputs(ag, BPL, PSD, B, N, 1, dtype, 13)
+    x = ag.agnvar_e13_iterate(an, srt, perm0, 5)["x"]
+    xh = x.cpu().numpy().astype(np.float64)
+    lags = [1, 5, 50, 365, 3650, N - 2, N + 5]
+    refs = [0.0, 0.1, 0.5, 1.0, 2.5, 5.0, 9.9, 10.1]           # the ERDF spans 4 dex: |dm| <= 10 mag
+    for m_zero, m_cut in ((0.0, None), (18.0, 22.0), (18.0, 19.0)):
+        prob, cons = ag.agnvar_delta_m_prob(x, lags, refs, m_zero, m_cut)
+        prob, cons = prob.cpu().numpy(), cons.cpu().numpy()
+        for b in range(B):
+            rp, rc = orc.delta_m_prob(xh[b], lags, refs, m_zero, m_cut)
+            assert (cons[b] == rc).all()
+            assert np.array_equal(prob[b], rp)
+        assert (prob[:, :, -1] == 0).all()
