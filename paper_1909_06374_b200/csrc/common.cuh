@@ -125,7 +125,7 @@ struct DevCache {
     int dev = -1;
     bool attrs[2] = {false, false};     // by element size (4, 8)
     int sms = 0;
-    int grid[8] = {0, 0, 0, 0, 0, 0, 0, 0};     // persistent-kernel grid sizes, by kernel slot
+    int grid[16] = {0};                 // persistent-kernel grid sizes, by kernel slot
 };
 inline DevCache& dev_cache() {
     static DevCache tab[64];

@@ -1,0 +1,304 @@
+// onchip.cuh -- the whole E13 loop (L1-L6) of one short fp32 light curve inside ONE CTA (256 <= N <= 2^14):
+// x_sim, the spectrum, the sort's (key, index) pairs, the slot counters and the previous permutation all live in shared
+// memory (12 N bytes: 12 KB at N = 1024, 192 KB at N = 2^14); HBM sees perm0 and the result once per call, and per
+// iteration only A_norm (2 B per sample) and sorted[] (4 B per sample), both re-read through L1/L2.  A curve leaves the
+// loop at its own first k with changed = 0 (L6 decided on chip; no other curve waits for it), CTAs take curves from a
+// ticket counter.  This is SURVEY section 7 steps 4-5 / 8(d): "one curve per CTA: on-chip loop".
+//
+// Per iteration:
+//   L1  forward FFT of z[n] = x[2n] + i x[2n+1] (L = N/2 points): Stockham radix-8/4/2 stages in shared memory
+//   L2  real-FFT untangle + amplitude replace + re-tangle on the pairs (k, L - k), natural order
+//   L3  inverse FFT (swap trick), 1/L; x_adj + 0.0 (Q13)
+//   L4  stable argsort of x_adj as an interpolation counting sort: slot = monotone linear map of the VALUE onto
+//       [mean - 4 sigma, mean + 4 sigma] (N slots, clamped; any monotone map gives the same result, this one keeps the
+//       slots about equally full for the near-Gaussian x_adj), 16-bit slot counters packed two per word, pairs grouped
+//       by slot, then the exact rank of every pair among its slot mates by the 64-bit (key, index) comparison: ties come
+//       out by ascending time index (O6 step 4), bit-identical to std::stable_sort.  Cost grows with the square of a
+//       slot's population: an input with massive ties (all keys equal) is still sorted exactly, slowly.
+//   L5  changed += (idx_new[r] != idx_old[r]);  x_sim[idx_new[r]] = sorted[r]
+//   L6  changed = 0 -> converged (iters_used = k)
+#pragma once
+#include "common.cuh"
+#include "fft.cuh"
+#include "kernels.cuh"
+
+namespace agn {
+
+template <int LOGN> struct OnchipCfg {
+    static constexpr int N = 1 << LOGN, L = N / 2;
+    static constexpr int THREADS = (N / 8 > 1024) ? 1024 : N / 8;
+    static constexpr int KPT = N / THREADS;             // keys per thread (8 or 16)
+    static constexpr int EPT = L / THREADS;             // complex points per thread in an FFT stage (4 or 8)
+    static constexpr int RP = L + (L >> 4);             // padded row
+    static constexpr int WARPS = THREADS / 32;
+    // region A: spectrum / x_sim (complex RP) in the FFT half of an iteration, (key, index) pairs (u64 N) in the sort half
+    static constexpr size_t bytesA = (size_t)N * 8;
+    static constexpr size_t smem = bytesA + (size_t)N * 2 /* packed slot counters */ + (size_t)N * 2 /* idx_old u16 */ +
+                                   (size_t)(2 * 32 + 32) * 8 /* reduction scratch */;
+};
+
+struct OnchipArgs {
+    const float* anorm;         // [B][L+1] natural order
+    const float* sorted;        // [B][N]
+    uint32_t* perm;             // [B][N] in: perm0, out: final permutation
+    float* x;                   // [B][N] out
+    float* xadj_dbg;            // [B][N] or NULL: x_adj of the last executed iteration
+    int32_t* iters_used;        // [B] or NULL
+    long long* hist;            // [B][max_iter] or NULL (zeroed by the host)
+    const float2* tw14;         // exp(-2 pi i m / 2^14)
+    unsigned int* ticket;       // zero on entry
+    int max_iter;
+    long long B;
+};
+
+// float index of time sample j inside the padded complex row
+__device__ __forceinline__ int xpos(int j) { const int n = j >> 1; return 2 * (n + (n >> 4)) + (j & 1); }
+
+// all Stockham stages of one row of L = 2^logL points (natural in -> natural out, forward sign)
+template <int THREADS, int EPT>
+__device__ __forceinline__ void onchip_fft(float2* s, int logL, int Rp, const float2* __restrict__ tw14) {
+    constexpr int RAD = EPT >= 8 ? 8 : EPT;
+    constexpr int LOGRAD = RAD == 8 ? 3 : (RAD == 4 ? 2 : 1);
+    int logNs = 0;
+    while (logL - logNs >= LOGRAD) {
+        fft_stage<float, RAD, THREADS, EPT, true>(s, logL, logNs, 0, Rp, tw14);
+        logNs += LOGRAD;
+    }
+    if (logL - logNs == 2) fft_stage<float, 4, THREADS, EPT, true>(s, logL, logNs, 0, Rp, tw14);
+    else if (logL - logNs == 1) fft_stage<float, 2, THREADS, EPT, true>(s, logL, logNs, 0, Rp, tw14);
+}
+
+template <int LOGN>
+__global__ void __launch_bounds__(OnchipCfg<LOGN>::THREADS) e13_onchip_kernel(OnchipArgs a) {
+    typedef OnchipCfg<LOGN> Cfg;
+    constexpr int N = Cfg::N, L = Cfg::L, THREADS = Cfg::THREADS, KPT = Cfg::KPT, RP = Cfg::RP, WARPS = Cfg::WARPS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2* Z = reinterpret_cast<float2*>(smem_raw);
+    float* Zf = reinterpret_cast<float*>(smem_raw);
+    unsigned long long* pair = reinterpret_cast<unsigned long long*>(smem_raw);
+    uint32_t* cw = reinterpret_cast<uint32_t*>(smem_raw + Cfg::bytesA);                  // [N/2]
+    unsigned short* perm_s = reinterpret_cast<unsigned short*>(smem_raw + Cfg::bytesA + (size_t)N * 2);      // [N]
+    double* red = reinterpret_cast<double*>(smem_raw + Cfg::bytesA + (size_t)N * 4);     // [64] + [32]
+    __shared__ unsigned int s_curve;
+    __shared__ float s_lo, s_scale;
+    __shared__ unsigned int s_changed;
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+
+    for (;;) {
+    __syncthreads();
+    if (t == 0) s_curve = atomicAdd(a.ticket, 1u);
+    __syncthreads();
+    const long long b = s_curve;
+    if (b >= a.B) break;
+    const float* An = a.anorm + b * (L + 1);
+    const float* srt = a.sorted + b * N;
+    uint32_t* pg = a.perm + b * N;
+    // x_sim,1: the draw in draw order (Q15); idx_old = perm0
+    for (int r = t; r < N; r += THREADS) {
+        const uint32_t i = pg[r];
+        perm_s[r] = (unsigned short)i;
+        Zf[xpos((int)i)] = srt[r];
+    }
+    int used = a.max_iter;
+    for (int k = 1; k <= a.max_iter; ++k) {
+        __syncthreads();
+        // ---- L1 forward FFT
+        onchip_fft<THREADS, Cfg::EPT>(Z, LOGN - 1, RP, a.tw14);
+        // ---- L2 untangle + amplitude replace + re-tangle (the stage's trailing barrier has been passed)
+        for (int kk = t; kk <= L / 2; kk += THREADS) {
+            if (kk == 0) {
+                const float2 z0 = Z[0];
+                const float x0 = z0.x + z0.y, xl = z0.x - z0.y;
+                const float a0 = An[0], al = An[L];
+                const float y0 = (x0 != 0.f) ? (x0 > 0.f ? a0 : -a0) : a0;
+                const float yl = (xl != 0.f) ? (xl > 0.f ? al : -al) : al;
+                Z[0] = make_float2(0.5f * (y0 + yl), 0.5f * (y0 - yl));
+            } else {
+                const int k2 = L - kk;
+                const int p1 = kk + (kk >> 4), p2 = k2 + (k2 >> 4);
+                float2 z1 = Z[p1], z2 = Z[p2];
+                replace_pair<float>(z1, z2, a.tw14[kk << (kLogTw - LOGN)], An[kk], An[k2]);      // w_N^k
+                Z[p1] = z1;
+                if (k2 != kk) Z[p2] = z2;
+            }
+        }
+        __syncthreads();
+        // ---- L3 inverse FFT: swap, forward stages, swap and 1/L (folded into the key read below)
+        for (int n = t; n < L; n += THREADS) { const int p = n + (n >> 4); Z[p] = cswap(Z[p]); }
+        __syncthreads();
+        onchip_fft<THREADS, Cfg::EPT>(Z, LOGN - 1, RP, a.tw14);
+        // ---- L4 keys into registers: x_adj[j] = (1/L) * swapped component, + 0.0 (Q13)
+        float v[KPT];
+        const float invL = 1.0f / (float)L;
+        float sum = 0.f, sq = 0.f;
+#pragma unroll
+        for (int i = 0; i < KPT; ++i) {
+            const int j = i * THREADS + t;
+            const int n = j >> 1;
+            // element j of the real series is the (j & 1) component of the UNSWAPPED result = the other one of Z
+            v[i] = Zf[2 * (n + (n >> 4)) + ((j & 1) ^ 1)] * invL + 0.0f;
+            sum += v[i];
+            sq = fmaf(v[i], v[i], sq);
+        }
+        if (a.xadj_dbg) {
+#pragma unroll
+            for (int i = 0; i < KPT; ++i) a.xadj_dbg[b * N + i * THREADS + t] = v[i];
+        }
+        // mean and sigma of x_adj (any values give a correct sort: they only place the slots)
+        {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) { sum += __shfl_xor_sync(0xffffffffu, sum, o); sq += __shfl_xor_sync(0xffffffffu, sq, o); }
+            if (lane == 0) { red[warp] = (double)sum; red[32 + warp] = (double)sq; }
+            if (t == 0) s_changed = 0u;
+            __syncthreads();            // also: every thread has read its keys out of region A
+            if (warp == 0) {
+                double s1 = lane < WARPS ? red[lane] : 0.0, s2 = lane < WARPS ? red[32 + lane] : 0.0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) { s1 += __shfl_xor_sync(0xffffffffu, s1, o); s2 += __shfl_xor_sync(0xffffffffu, s2, o); }
+                if (lane == 0) {
+                    const double mu = s1 / (double)N;
+                    double var = s2 / (double)N - mu * mu;
+                    if (!(var > 0.0)) var = 0.0;
+                    const double sg = sqrt(var);
+                    const double lo = mu - 4.0 * sg, width = 8.0 * sg;
+                    s_lo = (float)lo;
+                    s_scale = (width > 0.0 && isfinite(width)) ? (float)((double)N / width) : 0.f;
+                }
+            }
+            for (int i = t; i < N / 2; i += THREADS) cw[i] = 0u;
+            __syncthreads();
+        }
+        const float lo = s_lo, scale = s_scale;
+        auto slot_of = [&](float x) -> uint32_t {
+            const float f = (x - lo) * scale;                      // monotone in x; NaN / negative -> slot 0
+            return (f >= 1.0f) ? min((uint32_t)f, (uint32_t)(N - 1)) : 0u;
+        };
+        // slot populations
+#pragma unroll
+        for (int i = 0; i < KPT; ++i) {
+            const uint32_t s = slot_of(v[i]);
+            atomicAdd(&cw[s >> 1], 1u << ((s & 1u) << 4));
+        }
+        __syncthreads();
+        // exclusive scan of the N slot populations: thread t owns the WPT consecutive words [t * WPT, (t + 1) * WPT)
+        {
+            constexpr int WPT = N / 2 / THREADS;        // 4 or 8 words = 8 or 16 slots
+            uint32_t w[WPT];
+            uint32_t tot = 0;
+#pragma unroll
+            for (int i = 0; i < WPT / 4; ++i) {
+                const uint4 q = reinterpret_cast<const uint4*>(cw)[t * (WPT / 4) + i];
+                w[4 * i] = q.x; w[4 * i + 1] = q.y; w[4 * i + 2] = q.z; w[4 * i + 3] = q.w;
+            }
+#pragma unroll
+            for (int i = 0; i < WPT; ++i) tot += (w[i] & 0xffffu) + (w[i] >> 16);
+            uint32_t inc = tot;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t m = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += m;
+            }
+            uint32_t* wsum = reinterpret_cast<uint32_t*>(red + 64);
+            if (lane == 31) wsum[warp] = inc;
+            __syncthreads();
+            uint32_t run = inc - tot;
+#pragma unroll
+            for (int wv = 0; wv < WARPS; ++wv) run += (wv < warp) ? wsum[wv] : 0u;
+#pragma unroll
+            for (int i = 0; i < WPT; ++i) {
+                const uint32_t l0 = run; run += w[i] & 0xffffu;
+                const uint32_t h0 = run; run += w[i] >> 16;
+                w[i] = l0 | (h0 << 16);
+            }
+#pragma unroll
+            for (int i = 0; i < WPT / 4; ++i)
+                reinterpret_cast<uint4*>(cw)[t * (WPT / 4) + i] = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
+        }
+        __syncthreads();
+        // pairs grouped by slot (any order inside a slot); counters end as the END of each slot
+#pragma unroll
+        for (int i = 0; i < KPT; ++i) {
+            const uint32_t s = slot_of(v[i]), sh = (s & 1u) << 4;
+            const uint32_t q = (atomicAdd(&cw[s >> 1], 1u << sh) >> sh) & 0xffffu;
+            pair[q] = ((unsigned long long)key_of(v[i]) << 32) | (uint32_t)(i * THREADS + t);
+        }
+        __syncthreads();
+        // exact rank among the slot mates; L5 on the fly: change count, idx_old <- idx_new, value for x_sim
+        uint32_t oidx[KPT];
+        float oval[KPT];
+        uint32_t diff = 0;
+#pragma unroll
+        for (int i = 0; i < KPT; ++i) {
+            const int q = i * THREADS + t;
+            const unsigned long long pv = pair[q];
+            const uint32_t s = slot_of(val_of((uint32_t)(pv >> 32)));
+            const uint32_t w = cw[s >> 1];
+            uint32_t z, st0;
+            if (s & 1u) { z = w >> 16; st0 = w & 0xffffu; }
+            else { z = w & 0xffffu; st0 = s ? (cw[(s >> 1) - 1] >> 16) : 0u; }
+            uint32_t r = (uint32_t)q;
+            if (z - st0 > 1u) {
+                r = st0;
+                for (uint32_t h = st0; h < z; ++h) r += (pair[h] < pv);
+            }
+            const uint32_t idx = (uint32_t)pv;
+            diff += ((uint32_t)perm_s[r] != idx);
+            perm_s[r] = (unsigned short)idx;
+            oidx[i] = idx;
+            oval[i] = srt[r];
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) diff += __shfl_xor_sync(0xffffffffu, diff, o);
+        if (lane == 0 && diff) atomicAdd(&s_changed, diff);
+        __syncthreads();                // every pair has been read: region A becomes x_sim again
+#pragma unroll
+        for (int i = 0; i < KPT; ++i) Zf[xpos((int)oidx[i])] = oval[i];
+        const uint32_t changed = s_changed;
+        if (t == 0 && a.hist) a.hist[b * a.max_iter + (k - 1)] = (long long)changed;
+        // ---- L6
+        if (changed == 0u) { used = k; break; }
+    }
+    __syncthreads();
+    // results: x_sim and the final permutation
+    for (int j = t; j < N; j += THREADS) {
+        a.x[b * N + j] = Zf[xpos(j)];
+        pg[j] = (uint32_t)perm_s[j];
+    }
+    if (t == 0 && a.iters_used) a.iters_used[b] = used;
+    }   // curve loop
+}
+
+inline bool onchip_applicable(size_t elem_size, long long N) { return elem_size == 4 && N >= 256 && N <= 16384; }
+
+template <int LOGN> inline cudaError_t onchip_launch(const OnchipArgs& a, int slot, cudaStream_t st) {
+    typedef OnchipCfg<LOGN> Cfg;
+    int& grid = dev_cache().grid[slot];
+    if (!grid) {
+        cudaError_t e = cudaFuncSetAttribute(e13_onchip_kernel<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem);
+        if (e != cudaSuccess) return e;
+        cudaFuncSetAttribute(e13_onchip_kernel<LOGN>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        int per = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, e13_onchip_kernel<LOGN>, Cfg::THREADS, Cfg::smem);
+        if (e != cudaSuccess) return e;
+        if (per < 1) return cudaErrorInvalidConfiguration;
+        grid = dev_cache().sms * per;
+    }
+    const unsigned g = (unsigned)std::min<long long>(a.B, grid);
+    AGN_LAUNCH(K_E13_ONCHIP, st, (e13_onchip_kernel<LOGN><<<g, Cfg::THREADS, Cfg::smem, st>>>(a)));
+    return cudaGetLastError();
+}
+
+inline cudaError_t onchip_run(int logN, const OnchipArgs& a, cudaStream_t st) {
+    switch (logN) {
+        case 8: return onchip_launch<8>(a, 3, st);
+        case 9: return onchip_launch<9>(a, 3 + 1, st);
+        case 10: return onchip_launch<10>(a, 3 + 2, st);
+        case 11: return onchip_launch<11>(a, 3 + 3, st);
+        case 12: return onchip_launch<12>(a, 3 + 4, st);
+        case 13: return onchip_launch<13>(a, 3 + 5, st);
+        case 14: return onchip_launch<14>(a, 3 + 6, st);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace agn

@@ -18,9 +18,10 @@ def generate_light_curves(cfg, device="cuda", host_out=None, want_hist=False, cu
     return -- this is the end-to-end entry point timed by bench.py's e2e leg.
     """
     B, N = cfg["B"], cfg["N"]
-    srt, perm, _ = _b.agnvar_erdf_sample_sorted(cfg["erdf"], B, N, cfg["dtype"], cfg["seed"], curve0,
+    psd_c, erdf_c = _b.marshal_params(cfg)
+    srt, perm, _ = _b.agnvar_erdf_sample_sorted(erdf_c, B, N, cfg["dtype"], cfg["seed"], curve0,
                                                 cfg["grid_points"], device=device)
-    _, anorm = _b.agnvar_tk_generate(cfg["psd"], B, N, cfg["dt"], cfg["oversample"], cfg["dtype"], cfg["seed"],
+    _, anorm = _b.agnvar_tk_generate(psd_c, B, N, cfg["dt"], cfg["oversample"], cfg["dtype"], cfg["seed"],
                                      curve0, want_xnorm=False, device=device)
     out = _b.agnvar_e13_iterate(anorm, srt, perm, cfg["max_iter"], want_hist=want_hist, want_fallbacks=want_fallbacks,
                                 delta_threshold=delta_threshold, want_delta=want_delta)

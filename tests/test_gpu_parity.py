@@ -230,9 +230,10 @@ def test_e13_fp64_long_curve_trajectory(ag, orc):
     assert (out["x"].cpu().numpy()[0] == ref["x"]).all()
 
 
-@pytest.mark.parametrize("N,os_,erdf", [(1024, 1, BPL), (4096, 10, BPL), (2 ** 14, 10, BPL), (2 ** 15, 1, LOGN),
+@pytest.mark.parametrize("N,os_,erdf", [(256, 1, BPL), (512, 4, LOGN), (1024, 1, BPL), (2048, 1, LOGN), (4096, 10, BPL),
+                                        (8192, 2, BPL), (2 ** 14, 10, BPL), (2 ** 15, 1, LOGN),
                                         (2 ** 17, 1, BPL), (2 ** 20, 1, LOGN), (2 ** 22, 1, BPL)],
-                         ids=["1k", "4k", "16k", "32k", "128k", "1M", "4M"])
+                         ids=["256", "512", "1k", "2k", "4k", "8k", "16k", "32k", "128k", "1M", "4M"])
 def test_e13_fp32_lockstep(ag, orc, N, os_, erdf):
     """fp32: free-running comparison is not meaningful (the map is chaotic w.r.t. rounding); every clause
     of the definition is checked on the GPU's own trajectory, one product-kernel iteration at a time."""
@@ -477,3 +478,38 @@ def test_delta_m_probability(ag, orc, dtype):
             assert (cons[b] == rc).all()
             assert np.array_equal(prob[b], rp)
         assert (prob[:, :, -1] == 0).all()
+
+
+# ---- the on-chip loop (fp32, 256 <= N <= 2^14): per-curve early exit ----------------------------------
+@pytest.mark.parametrize("N", [256, 1024, 4096])
+def test_onchip_loop_early_exit_is_a_fixed_point(ag, orc, N):
+    """Short fp32 curves run the whole loop inside one CTA and leave it at their own first k with changed = 0.
+    What the early exit must guarantee: the history is consistent (last recorded count 0 at k = iters_used, zeros after),
+    the output is an exact permutation of the draw, and the state it returns is a fixed point of the map -- one more
+    iteration (product kernels) changes nothing, and neither does one more iteration of the fp64 oracle's argsort applied
+    to the GPU's own x_adj."""
+    B, max_iter = 48, 100
+    srt, perm, an = _inputs(ag, BPL, dict(PSD, f_b=1.0 / 50.0), B, N, 1, "f32", 21)
+    out = ag.agnvar_e13_iterate(an, srt, perm, max_iter, want_hist=True)
+    iters, hist = out["iters_used"].cpu().numpy(), out["changed_hist"].cpu().numpy()
+    x, p = out["x"].clone(), perm.clone()
+    assert (np.sort(out["x"].cpu().numpy(), axis=1) == srt.cpu().numpy()).all()
+    conv = iters < max_iter
+    print(f"N={N}: {int(conv.sum())} of {B} curves converged within {max_iter}; iterations used: median {np.median(iters):.0f}, "
+          f"min {iters.min()}, max {iters.max()}")
+    assert conv.sum() >= (B // 2 if N <= 1024 else 1)
+    for b in range(B):
+        k = iters[b]
+        assert (hist[b][:k - 1] > 0).all()
+        if conv[b]:
+            assert hist[b][k - 1] == 0 and (hist[b][k:] == 0).all()
+        else:
+            assert hist[b][k - 1] > 0
+    again = ag.agnvar_e13_iterate(an, srt, perm, 1, want_hist=True, want_xadj=True)
+    h1 = again["changed_hist"].cpu().numpy()[:, 0]
+    assert (h1[conv] == 0).all()
+    assert torch.equal(again["x"][torch.tensor(conv)], x[torch.tensor(conv)])
+    assert torch.equal(perm[torch.tensor(conv)], p[torch.tensor(conv)])
+    xadj = again["x_adj"].cpu().numpy()
+    for b in np.flatnonzero(conv)[:6]:
+        assert (u32(p)[b] == orc.stable_argsort(xadj[b].astype(np.float64))).all()
