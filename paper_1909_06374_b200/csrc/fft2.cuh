@@ -153,12 +153,18 @@ __global__ void __launch_bounds__(THREADS, (MAXLOG >= 6 ? 3 : (MAXLOG == 5 ? 4 :
 
 // ------------------------------------------------------------------------------------------------
 // mid kernel: rows of R1 = 2^13 = 16 * 16 * 32, two rows per CTA, 512 threads
+// Rows (64 KB, contiguous in HBM) and their target amplitudes (32 KB) arrive by BULK ASYNCHRONOUS COPIES
+// (cp.async.bulk global -> shared, completion on an mbarrier): one elected thread issues one copy per row, no LSU
+// instruction and no register is spent on the transfer, and the copy of the next work item's rows overlaps the
+// last butterflies and the stores of the current one.  A bulk copy lands linearly, so the rows are not padded:
+// bank conflicts are avoided by an XOR swizzle of the low five index bits with the next five (mid_swz), which
+// forward stage 1 applies on its write (it reads the linear landing layout, conflict-free as it is; a warp only ever
+// touches its own sixteen 32-element groups in that stage, so the linear -> swizzled rewrite is safe in place).
 // ------------------------------------------------------------------------------------------------
 constexpr int kMidThreads = 512;
 constexpr int kMidL1 = 4, kMidL2 = 4, kMidL3 = 5;        // log2 of the stage radices
-constexpr int kMidPadShift = 5;                           // one pad element per 32
-__host__ __device__ constexpr int mid_pad(int a) { return a + (a >> kMidPadShift); }
-constexpr int kMidRowElems = (1 << kLogR1) + (1 << (kLogR1 - kMidPadShift));
+__host__ __device__ constexpr int mid_swz(int a) { return a ^ ((a >> 5) & 31); }
+constexpr int kMidRowElems = 1 << kLogR1;
 constexpr size_t kMidSmemBytes = 2 * (size_t)kMidRowElems * sizeof(float2) + 2 * ((size_t)1 << kLogR1) * sizeof(float);   // rows + their A_norm
 
 template <typename T> struct MidArgs {
@@ -174,56 +180,83 @@ template <typename T> struct MidArgs {
     TwLevel<T> rlv;               // w_N (N = 2L) for the row factor w_N^{k0}
 };
 
+// mbarrier + bulk-copy primitives (sm_90+ PTX; SASS: SYNCS.* and UBLKCP)
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(a), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+
 template <typename T>
 __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
     typedef typename Cx<T>::type C;
+    static_assert(sizeof(T) == 4, "fp32 rows");
     constexpr int R1 = 1 << kLogR1;
     constexpr int RAD1 = 1 << kMidL1, RAD2 = 1 << kMidL2, RAD3 = 1 << kMidL3;
     constexpr int J1 = R1 / RAD1;                 // 512 butterflies per row in stages 1 and 2
     constexpr int LOG23 = kMidL2 + kMidL3;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr unsigned kRowBytes = R1 * sizeof(C), kAmpBytes = R1 * sizeof(T);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     C* s = reinterpret_cast<C*>(smem_raw);
     __shared__ C s_wrow[2];
+    __shared__ __align__(8) unsigned long long s_bar[3];      // row 0, row 1, amplitudes
     const int t = threadIdx.x;
     const int R0 = 1 << a.logR0;
     const int nrows = (R0 == 1) ? 1 : 2;
     const int gx = (R0 == 1) ? 1 : (R0 >> 1);
     const long long total = (long long)a.B * gx;
     T* sA = reinterpret_cast<T*>(smem_raw + 2 * (size_t)kMidRowElems * sizeof(C));
-    // Persistent CTA (one per SM: 196 KB of shared memory): work item = (curve b, row pair pid).  The rows and the
-    // target amplitudes of the NEXT item are fetched with cp.async while the current one is still being finished:
-    // the amplitudes after the replace step has released sA, each row right after this thread has read its own 16
-    // elements of it in inverse stage 1 (stage 1 touches thread-private positions only, forward and inverse).
+    // Persistent CTA (one per SM: 192 KB of shared memory): work item = (curve b, row pair pid).
     auto row_pos = [&](int pid, int r) -> int {
         const int k = (r == 0) ? pid : ((pid == 0) ? (R0 >> 1) : (R0 - pid));
         return (R0 == 1) ? 0 : (int)k2pos(a.dcol, (uint32_t)k);
     };
+    // issued by thread 0 only, after a CTA barrier that follows the last generic-proxy access to the destination
     auto fetch_row = [&](long long bb, int rp_, int r) {
-        const C* z = a.Z + bb * a.bstride + ((long long)rp_ << kLogR1);
-#pragma unroll
-        for (int i = 0; i < RAD1; ++i) {
-            const unsigned d = (unsigned)__cvta_generic_to_shared(s + r * kMidRowElems + mid_pad(i * J1 + t));
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(z + i * J1 + t) : "memory");
-        }
+        fence_proxy_async();
+        mbar_expect_tx(&s_bar[r], kRowBytes);
+        bulk_g2s(s + r * kMidRowElems, a.Z + bb * a.bstride + ((long long)rp_ << kLogR1), kRowBytes, &s_bar[r]);
     };
-    auto fetch_amp = [&](long long bb, int rp_, int r) {
-        const T* Ar = a.Ap + bb * (a.bstride + kApPad) + ((long long)rp_ << kLogR1);
-        static_assert(sizeof(T) == 4, "16-byte copies of four fp32 amplitudes");
-#pragma unroll
-        for (int p = 4 * t; p < R1; p += 4 * kMidThreads) {
-            const unsigned d = (unsigned)__cvta_generic_to_shared(sA + r * R1 + p);
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(Ar + p) : "memory");
-        }
+    auto fetch_amps = [&](long long bb, int pid_) {
+        fence_proxy_async();
+        mbar_expect_tx(&s_bar[2], kAmpBytes * (unsigned)nrows);
+        for (int r = 0; r < nrows; ++r)
+            bulk_g2s(sA + r * R1, a.Ap + bb * (a.bstride + kApPad) + ((long long)row_pos(pid_, r) << kLogR1), kAmpBytes, &s_bar[2]);
     };
     long long work = blockIdx.x;
     if (work >= total) return;
-    {
+    if (t == 0) {
+        mbar_init(&s_bar[0], 1); mbar_init(&s_bar[1], 1); mbar_init(&s_bar[2], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+    if (t == 0) {
         const long long b0 = work / gx;
         const int pid0 = (int)(work - b0 * gx);
-        for (int r = 0; r < nrows; ++r) { const int q = row_pos(pid0, r); fetch_row(b0, q, r); fetch_amp(b0, q, r); }
-        asm volatile("cp.async.commit_group;\n" ::: "memory");
+        for (int r = 0; r < nrows; ++r) fetch_row(b0, row_pos(pid0, r), r);
+        fetch_amps(b0, pid0);
     }
-    for (; work < total; work += gridDim.x) {
+    unsigned phase = 0;
+    for (; work < total; work += gridDim.x, phase ^= 1u) {
     const long long b = work / gx;
     const int pid = (int)(work - b * gx);         // 0: rows 0 and R0/2 (self-paired); else rows pid, R0 - pid
     const long long work_n = work + gridDim.x;
@@ -238,23 +271,25 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
     zrow[0] = a.Z + b * a.bstride + ((long long)rp[0] << kLogR1);
     zrow[1] = a.Z + b * a.bstride + ((long long)rp[1] << kLogR1);
     if (t < 2) s_wrow[t] = tw_lookup<T>(a.rlv, (uint32_t)(t == 0 ? k0[0] : k0[1]));      // no dynamic index: k0 stays in registers
-    asm volatile("cp.async.wait_group 0;\n" ::: "memory");      // this item's rows and amplitudes have landed
     C pw[16];
 
-    // ---- forward stage 1: thread j = t owns (d2, d3) = j, butterfly over d1 (stride J1)
+    // ---- forward stage 1: thread j = t owns (d2, d3) = j, butterfly over d1 (stride J1).  Reads the LINEAR landing
+    //      layout, writes the swizzled working layout (same 32-element groups: private to this warp).
     pow16<T, C>(a.tw14[t << (kLogTw - kLogR1)], pw);
 #pragma unroll
     for (int r = 0; r < 2; ++r) {
         if (r < nrows) {
+            mbar_wait(&s_bar[r], phase);          // this item's row r has landed
             C v[RAD1];
 #pragma unroll
-            for (int i = 0; i < RAD1; ++i) v[i] = s[r * kMidRowElems + mid_pad(i * J1 + t)];
+            for (int i = 0; i < RAD1; ++i) v[i] = s[r * kMidRowElems + i * J1 + t];
+            __syncwarp();
             fft_reg_dif<T, RAD1, C>(v);
 #pragma unroll
             for (int k = 0; k < RAD1; ++k) {
                 C x = v[bitrev<RAD1>(k)];
                 if (k > 0) x = cmul(x, pw[k]);
-                s[r * kMidRowElems + mid_pad(k * J1 + t)] = x;
+                s[r * kMidRowElems + mid_swz(k * J1 + t)] = x;
             }
         }
     }
@@ -268,13 +303,13 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
             C v[RAD2];
             C* sr = s + r * kMidRowElems;
 #pragma unroll
-            for (int i = 0; i < RAD2; ++i) v[i] = sr[mid_pad((k1 << LOG23) + (i << kMidL3) + d3)];
+            for (int i = 0; i < RAD2; ++i) v[i] = sr[mid_swz((k1 << LOG23) + (i << kMidL3) + d3)];
             fft_reg_dif<T, RAD2, C>(v);
 #pragma unroll
             for (int k = 0; k < RAD2; ++k) {
                 C x = v[bitrev<RAD2>(k)];
                 if (k > 0) x = cmul(x, pw[k]);
-                sr[mid_pad((k1 << LOG23) + (k << kMidL3) + d3)] = x;
+                sr[mid_swz((k1 << LOG23) + (k << kMidL3) + d3)] = x;
             }
         }
     }
@@ -283,15 +318,17 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
     const int r3 = t >> (kLogR1 - kMidL3), u = t & ((R1 >> kMidL3) - 1);
     if (r3 < nrows) {
         C v[RAD3];
-        C* sr = s + r3 * kMidRowElems + u * (RAD3 + 1);        // mid_pad(u * 32 + i) = u * 33 + i
+        C* sr = s + r3 * kMidRowElems + u * RAD3;              // group u: element i sits at i ^ (u & 31)
+        const int x5 = u & (RAD3 - 1);
 #pragma unroll
-        for (int i = 0; i < RAD3; ++i) v[i] = sr[i];
+        for (int i = 0; i < RAD3; ++i) v[i] = sr[i ^ x5];
         fft_reg_dif<T, RAD3, C>(v);
 #pragma unroll
-        for (int k = 0; k < RAD3; ++k) sr[k] = v[bitrev<RAD3>(k)];
+        for (int k = 0; k < RAD3; ++k) sr[k ^ x5] = v[bitrev<RAD3>(k)];
     }
     __syncthreads();
     // ---- L2: untangle + amplitude replace on the pairs (K, L - K)
+    mbar_wait(&s_bar[2], phase);                  // the amplitudes of this item have landed
     {
         const T* Ab = a.Ap + b * (a.bstride + kApPad);
         if (pid != 0) {
@@ -302,10 +339,10 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
 #pragma unroll 4
             for (int p = t; p < R1; p += kMidThreads) {
                 const int p2 = R1 - 1 - p;
-                C z1 = s[mid_pad(p)], z2 = s[kMidRowElems + mid_pad(p2)];
+                C z1 = s[mid_swz(p)], z2 = s[kMidRowElems + mid_swz(p2)];
                 replace_pair<T>(z1, z2, cmul(wrow, a.twpos[p]), A1p[p], A2p[p2]);
-                s[mid_pad(p)] = z1;
-                s[kMidRowElems + mid_pad(p2)] = z2;
+                s[mid_swz(p)] = z1;
+                s[kMidRowElems + mid_swz(p2)] = z2;
             }
         } else {
             // row 0: bin k pairs with (R1 - k) mod R1 (table sp); k = 0 holds DC and Nyquist
@@ -321,10 +358,10 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
                     T yl = (xl != (T)0) ? (xl > (T)0 ? al : -al) : al;
                     s[0] = mk<T>((T)0.5 * (y0 + yl), (T)0.5 * (y0 - yl));
                 } else {
-                    C z1 = s[mid_pad(p)], z2 = s[mid_pad(p2)];
+                    C z1 = s[mid_swz(p)], z2 = s[mid_swz(p2)];
                     replace_pair<T>(z1, z2, a.twpos[p], A1p[p], A1p[p2]);       // w_N^{0} = 1
-                    s[mid_pad(p)] = z1;
-                    s[mid_pad(p2)] = z2;
+                    s[mid_swz(p)] = z1;
+                    s[mid_swz(p2)] = z2;
                 }
             }
             if (nrows == 2) {
@@ -334,27 +371,26 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
                 C* sr = s + kMidRowElems;
                 for (int p = t; p < R1 / 2; p += kMidThreads) {
                     const int p2 = R1 - 1 - p;
-                    C z1 = sr[mid_pad(p)], z2 = sr[mid_pad(p2)];
+                    C z1 = sr[mid_swz(p)], z2 = sr[mid_swz(p2)];
                     replace_pair<T>(z1, z2, cmul(wrow, a.twpos[p]), A2p[p], A2p[p2]);
-                    sr[mid_pad(p)] = z1;
-                    sr[mid_pad(p2)] = z2;
+                    sr[mid_swz(p)] = z1;
+                    sr[mid_swz(p2)] = z2;
                 }
             }
         }
     }
     __syncthreads();
-    if (has_next) {
-        for (int r = 0; r < nrows; ++r) fetch_amp(b_n, row_pos(pid_n, r), r);        // sA is free now
-    }
+    if (has_next && t == 0) fetch_amps(b_n, pid_n);        // sA is free now
     // ---- inverse stage 3
     if (r3 < nrows) {
         C v[RAD3];
-        C* sr = s + r3 * kMidRowElems + u * (RAD3 + 1);
+        C* sr = s + r3 * kMidRowElems + u * RAD3;
+        const int x5 = u & (RAD3 - 1);
 #pragma unroll
-        for (int i = 0; i < RAD3; ++i) v[i] = cswap(sr[i]);
+        for (int i = 0; i < RAD3; ++i) v[i] = cswap(sr[i ^ x5]);
         fft_reg_dif<T, RAD3, C>(v);
 #pragma unroll
-        for (int n = 0; n < RAD3; ++n) sr[n] = cswap(v[bitrev<RAD3>(n)]);
+        for (int n = 0; n < RAD3; ++n) sr[n ^ x5] = cswap(v[bitrev<RAD3>(n)]);
     }
     __syncthreads();
     // ---- inverse stage 2 (pw still holds w_{512}^{k d3})
@@ -365,17 +401,18 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
             C* sr = s + r * kMidRowElems;
 #pragma unroll
             for (int k = 0; k < RAD2; ++k) {
-                C x = sr[mid_pad((k1 << LOG23) + (k << kMidL3) + d3)];
+                C x = sr[mid_swz((k1 << LOG23) + (k << kMidL3) + d3)];
                 if (k > 0) x = cmulc(x, pw[k]);
                 v[k] = cswap(x);
             }
             fft_reg_dif<T, RAD2, C>(v);
 #pragma unroll
-            for (int n = 0; n < RAD2; ++n) sr[mid_pad((k1 << LOG23) + (n << kMidL3) + d3)] = cswap(v[bitrev<RAD2>(n)]);
+            for (int n = 0; n < RAD2; ++n) sr[mid_swz((k1 << LOG23) + (n << kMidL3) + d3)] = cswap(v[bitrev<RAD2>(n)]);
         }
     }
     __syncthreads();
-    // ---- inverse stage 1
+    // ---- inverse stage 1: results go straight from registers to HBM; as soon as every thread has read its inputs of
+    //      row r, the bulk copy of the next item's row r is started (it overlaps the butterflies and stores that follow)
     pow16<T, C>(a.tw14[t << (kLogTw - kLogR1)], pw);
 #pragma unroll
     for (int r = 0; r < 2; ++r) {
@@ -383,17 +420,17 @@ __global__ void __launch_bounds__(kMidThreads, 1) fft_mid_kernel(MidArgs<T> a) {
             C v[RAD1];
 #pragma unroll
             for (int k = 0; k < RAD1; ++k) {
-                C x = s[r * kMidRowElems + mid_pad(k * J1 + t)];
+                C x = s[r * kMidRowElems + mid_swz(k * J1 + t)];
                 if (k > 0) x = cmulc(x, pw[k]);
                 v[k] = cswap(x);
             }
-            if (has_next) fetch_row(b_n, row_pos(pid_n, r), r);     // this thread's 16 positions of row r are free now
+            __syncthreads();
+            if (has_next && t == 0) fetch_row(b_n, row_pos(pid_n, r), r);
             fft_reg_dif<T, RAD1, C>(v);
 #pragma unroll
             for (int n = 0; n < RAD1; ++n) zrow[r][n * J1 + t] = cswap(v[bitrev<RAD1>(n)]);
         }
     }
-    asm volatile("cp.async.commit_group;\n" ::: "memory");
     }   // work loop
 }
 
