@@ -273,3 +273,24 @@ def delta_m_prob(x, lags, dm_ref, m_zero=0.0, m_cut=None):
                            C.c_double(m_zero), C.c_int(0 if m_cut is None else 1),
                            C.c_double(0.0 if m_cut is None else m_cut), _p(prob), _p(cons))
     return prob, cons
+
+
+# ---- NEXT-4: ensemble SF of masked sub-segments (Fig. 7-8), output-PDF moments (Fig. 2) -----------------
+def ensemble_sf(x, n_sub, keep, seed, curve0, lags, mag=False):
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    B, N = x.shape
+    lags = np.ascontiguousarray(lags, dtype=np.int64)
+    sf2 = np.empty(lags.size)
+    pairs = np.empty(lags.size, dtype=np.int64)
+    offs = np.empty(B, dtype=np.int64)
+    lib().orc_ensemble_sf(_p(x), C.c_int64(B), C.c_int64(N), C.c_int64(n_sub), C.c_double(keep), C.c_uint64(seed),
+                          C.c_uint32(curve0), _p(lags), C.c_int(lags.size), C.c_int(1 if mag else 0), _p(sf2), _p(pairs),
+                          _p(offs))
+    return sf2, pairs, offs
+
+
+def moments(x):
+    x = _d(x)
+    out = np.empty(4)
+    lib().orc_moments(_p(x), C.c_int64(x.size), _p(out))
+    return out

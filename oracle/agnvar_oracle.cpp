@@ -32,6 +32,10 @@
 //                                  random-walk ensemble slope beta = (alpha - 1)/2 = 1/2, magnitude invariances
 //   orc_delta_m_prob       pinned: brute force, 0 beyond 2.5 x the dynamic range, monotone in dm_ref
 //   orc_sf_representative  pinned: by hand (Eq. 6)
+//   orc_ensemble_sf        pinned: reduces to orc_structure_function for one curve, whole series, keep fraction 1;
+//                                  brute force with the mask rebuilt from the (KAT-pinned) Philox words; pooled pair
+//                                  count ~ p^2 (n_sub - l) B; unbiased for a random-walk ensemble
+//   orc_moments            pinned: closed forms (two-point and uniform distributions), scipy.stats on random data
 //
 // Build: g++ -O2 -std=c++17 -shared -fPIC -o liboracle.so agnvar_oracle.cpp   (oracle/build.py)
 
@@ -579,6 +583,69 @@ void orc_delta_m_prob(const double* x, int64_t N, const int64_t* lags, int nlags
         for (int r = 0; r < nref; ++r) prob[(size_t)q * nref + r] = P > 0 ? (double)cnt[(size_t)r] / (double)P : 0.0;
         if (considered) considered[q] = P;
     }
+}
+
+// ----------------------------------------------------------------------------------------------
+// NEXT-4. Ensemble structure function of sparsely sampled sub-segments (PAPER.md:253-259 sec. 3.2.5-3.2.6, :276,
+// Fig. 7-8): from every light curve a CONSECUTIVE sub-sample of n_sub points is selected at a random position, the
+// sub-sample is masked to mimic sparse measurements (a random fraction `keep` of its points is kept: 0.5 %, 1 %, 10 %
+// in Fig. 8), and the SF at lag l is Eq. A6 over ALL pairs of kept points separated by l, in all the curves at once
+// ("considering simultaneously all the pairs of data points separated by a corresponding time lag, in all the sources").
+// The paper does not say how the positions and the mask are drawn; reading (Q23): Philox stream tag 3, call 0
+// of curve b: offset_b = floor(u (N - n_sub + 1)), u from words (0, 1); tag 4: point j of the sub-sample is kept iff
+// u_j < keep, u_j from call j >> 1 of curve b, words (0, 1) if j is even, (2, 3) if odd.
+// x: [B][N] row-major.  sf2[q] = pooled mean (0 if no pair), pairs[q] = pooled number of pairs; offsets[b] may be NULL.
+// ----------------------------------------------------------------------------------------------
+void orc_ensemble_sf(const double* x, int64_t B, int64_t N, int64_t n_sub, double keep, uint64_t seed, uint32_t curve0,
+                     const int64_t* lags, int nlags, int mag, double* sf2, int64_t* pairs, int64_t* offsets) {
+    std::vector<double> acc((size_t)nlags, 0.0);
+    std::vector<int64_t> cnt((size_t)nlags, 0);
+    std::vector<double> v((size_t)n_sub);
+    std::vector<char> kept((size_t)n_sub);
+    for (int64_t b = 0; b < B; ++b) {
+        uint32_t w[4];
+        orc_philox_stream(seed, 0, curve0 + (uint32_t)b, 3u, w);
+        const int64_t off = (int64_t)std::floor(orc_u53(w[0], w[1]) * (double)(N - n_sub + 1));
+        if (offsets) offsets[b] = off;
+        for (int64_t j = 0; j < n_sub; ++j) {
+            orc_philox_stream(seed, (uint64_t)(j >> 1), curve0 + (uint32_t)b, 4u, w);
+            const double u = (j & 1) ? orc_u53(w[2], w[3]) : orc_u53(w[0], w[1]);
+            kept[(size_t)j] = (u < keep) ? 1 : 0;
+            const double xv = x[(size_t)b * (size_t)N + (size_t)(off + j)];
+            v[(size_t)j] = mag ? -2.5 * std::log10(xv) : xv;
+        }
+        for (int q = 0; q < nlags; ++q) {
+            const int64_t l = lags[q];
+            for (int64_t j = 0; j + l < n_sub; ++j) {
+                if (!(kept[(size_t)j] && kept[(size_t)(j + l)])) continue;
+                const double d = v[(size_t)j] - v[(size_t)(j + l)];
+                acc[(size_t)q] += d * d;
+                cnt[(size_t)q] += 1;
+            }
+        }
+    }
+    for (int q = 0; q < nlags; ++q) {
+        sf2[q] = cnt[(size_t)q] > 0 ? acc[(size_t)q] / (double)cnt[(size_t)q] : 0.0;
+        if (pairs) pairs[q] = cnt[(size_t)q];
+    }
+}
+
+// Moments of the value distribution of a series (the TK95 output-PDF check of sec. 3.2.1 / Fig. 2):
+// mean, variance (1/N), skewness m3 / m2^1.5, excess kurtosis m4 / m2^2 - 3, central moments m_k = (1/N) sum (x - mean)^k.
+void orc_moments(const double* x, int64_t N, double out[4]) {
+    double mu = 0.0;
+    for (int64_t i = 0; i < N; ++i) mu += x[i];
+    mu /= (double)N;
+    double m2 = 0.0, m3 = 0.0, m4 = 0.0;
+    for (int64_t i = 0; i < N; ++i) {
+        const double d = x[i] - mu, d2 = d * d;
+        m2 += d2; m3 += d2 * d; m4 += d2 * d2;
+    }
+    m2 /= (double)N; m3 /= (double)N; m4 /= (double)N;
+    out[0] = mu;
+    out[1] = m2;
+    out[2] = m2 > 0.0 ? m3 / (m2 * std::sqrt(m2)) : 0.0;
+    out[3] = m2 > 0.0 ? m4 / (m2 * m2) - 3.0 : 0.0;
 }
 
 }  // extern "C"

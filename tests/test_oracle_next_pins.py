@@ -142,3 +142,71 @@ def test_delta_m_probability(orc):
         for r, ref in enumerate(refs):
             assert prob_c[q, r] == pytest.approx(np.mean(d > ref) if d.size else 0.0, abs=1e-15)
     assert (cons_c < cons).all()
+
+
+# ---- NEXT-4 ---------------------------------------------------------------------------------------
+def test_ensemble_sf_reduces_to_plain_sf_and_bruteforce(orc):
+    rng = np.random.default_rng(5)
+    B, N = 6, 300
+    x = 10.0 ** rng.uniform(-2, 0, (B, N))
+    lags = np.array([1, 2, 9, 40, 299, 300])
+    # one curve, the whole series, nothing masked: Eq. A6 itself
+    for mag in (False, True):
+        sf2, pairs, offs = orc.ensemble_sf(x[:1], N, 1.0, 7, 0, lags, mag)
+        ref, rp = orc.structure_function(x[0], lags, mag)
+        assert offs[0] == 0 and (pairs == rp).all() and np.allclose(sf2, ref, rtol=1e-14)
+    # general case rebuilt by hand from the raw Philox words (pinned by the published known-answer vectors)
+    n_sub, keep, seed, curve0 = 120, 0.3, 11, 4
+    sf2, pairs, offs = orc.ensemble_sf(x, n_sub, keep, seed, curve0, lags[:4])
+    acc, cnt = np.zeros(4), np.zeros(4, dtype=np.int64)
+    for b in range(B):
+        w = orc.philox_stream(seed, 0, curve0 + b, 3)
+        off = int(np.floor(orc.u53(w[0], w[1]) * (N - n_sub + 1)))
+        assert off == offs[b] and 0 <= off <= N - n_sub
+        kept = np.zeros(n_sub, dtype=bool)
+        for j in range(n_sub):
+            w = orc.philox_stream(seed, j >> 1, curve0 + b, 4)
+            kept[j] = (orc.u53(w[2], w[3]) if j & 1 else orc.u53(w[0], w[1])) < keep
+        seg = x[b, off:off + n_sub]
+        for q, l in enumerate(lags[:4]):
+            use = kept[:-l] & kept[l:]
+            acc[q] += np.sum((seg[:-l] - seg[l:])[use] ** 2)
+            cnt[q] += use.sum()
+    assert (pairs == cnt).all() and cnt[0] > 0
+    assert np.allclose(sf2, acc / np.maximum(cnt, 1), rtol=1e-13)
+    # a different curve0 draws different positions and masks
+    assert not np.array_equal(orc.ensemble_sf(x, n_sub, keep, seed, curve0 + 1, lags[:4])[2], offs)
+
+
+def test_ensemble_sf_is_unbiased_and_pair_counts_scale(orc):
+    """Fig. 8's statement: "the ensemble SF always scatters around the representative SF"; for a random walk
+    E[SF^2(l)] = l whatever the mask, and the pooled number of pairs is ~ keep^2 (n_sub - l) B."""
+    rng = np.random.default_rng(6)
+    B, N, n_sub = 400, 5000, 1000
+    x = np.cumsum(rng.standard_normal((B, N)), axis=1)
+    lags = np.array([1, 3, 10, 30, 100])
+    for keep in (0.1, 0.5):
+        sf2, pairs, offs = orc.ensemble_sf(x, n_sub, keep, 3, 0, lags)
+        expect = keep ** 2 * (n_sub - lags) * B
+        assert np.all(np.abs(pairs - expect) < 6 * np.sqrt(expect) + 0.02 * expect)
+        # relative scatter of the pooled mean: var of a squared Gaussian difference is 2 l^2, pairs are correlated -> loose
+        assert np.all(np.abs(sf2 / lags - 1.0) < 0.25)
+        assert offs.min() >= 0 and offs.max() <= N - n_sub and len(set(offs.tolist())) > B // 2
+
+
+def test_moments(orc):
+    scipy_stats = pytest.importorskip("scipy.stats")
+    rng = np.random.default_rng(7)
+    x = rng.gamma(2.0, 1.5, 20000)
+    m = orc.moments(x)
+    assert m[0] == pytest.approx(x.mean(), rel=1e-13) and m[1] == pytest.approx(x.var(), rel=1e-12)
+    assert m[2] == pytest.approx(scipy_stats.skew(x), rel=1e-11) and m[3] == pytest.approx(scipy_stats.kurtosis(x), rel=1e-11)
+    # closed forms: two-point distribution {0 with prob 3/4, 1 with prob 1/4}: skew = (1 - 2p)/sqrt(pq), kurt = (1 - 6pq)/(pq)
+    y = np.array([0.0] * 750 + [1.0] * 250)
+    p, q = 0.25, 0.75
+    m = orc.moments(y)
+    assert m[0] == pytest.approx(p) and m[1] == pytest.approx(p * q)
+    assert m[2] == pytest.approx((1 - 2 * p) / np.sqrt(p * q)) and m[3] == pytest.approx((1 - 6 * p * q) / (p * q))
+    # a Gaussian series has skewness and excess kurtosis ~ 0 (what Fig. 2 tests the TK95 output against)
+    g = orc.moments(rng.standard_normal(200000))
+    assert abs(g[2]) < 0.03 and abs(g[3]) < 0.06
