@@ -48,7 +48,8 @@ typedef enum {
     AGNVAR_OP_E13_ITERATE = 3,
     AGNVAR_OP_PERIODOGRAM = 4,
     AGNVAR_OP_STRUCTURE_FUNCTION = 5,
-    AGNVAR_OP_DELTA_M_PROB = 6
+    AGNVAR_OP_DELTA_M_PROB = 6,
+    AGNVAR_OP_ENSEMBLE_SF = 7
 } agnvar_op;
 
 /* Eq. 3: PSD(f) = A [ (f/f_b)^alpha_low + (f/f_b)^alpha_high ]^-1.
@@ -72,7 +73,8 @@ typedef struct {
 
 /* Bytes of scratch the given op needs.  `oversample` matters for AGNVAR_OP_TK_GENERATE only
  * (pass 1 otherwise); `aux` = grid_points for ERDF_SAMPLE_SORTED, nbins for PERIODOGRAM, 1 for E13_ITERATE
- * with the delta_i rule / history (see agnvar_e13_opts), nlags for STRUCTURE_FUNCTION and DELTA_M_PROB, else 0.
+ * with the delta_i rule / history (see agnvar_e13_opts), nlags for STRUCTURE_FUNCTION, DELTA_M_PROB and
+ * ENSEMBLE_SF (pass n_sub as N for ENSEMBLE_SF), else 0.
  * Returns 0 for invalid arguments. */
 size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int oversample, int64_t aux);
 
@@ -205,6 +207,24 @@ int agnvar_structure_function(int64_t B, int64_t N, int dtype, const void* d_x, 
 int agnvar_delta_m_prob(int64_t B, int64_t N, int dtype, const void* d_x, const int64_t* h_lags, int nlags,
                         const double* h_dm_ref, int nref, double m_zero, int use_cut, double m_cut, double* d_prob,
                         int64_t* d_considered, void* d_ws, size_t ws_bytes, void* stream);
+
+/* eSF -- ensemble structure function of sparsely sampled sub-segments (PAPER.md:253-259 sec. 3.2.5-3.2.6, :276, Fig. 7-8):
+ * from every curve a CONSECUTIVE sub-sample of n_sub points at a random position, masked so that a random fraction
+ * `keep` of its points survives; SF(tau)^2 at lag l = Eq. A6 over all pairs of kept points separated by l, pooled over
+ * all B curves.  The paper does not say how positions and masks are drawn (Q23): Philox tag 3, call 0 of curve
+ * curve0 + b: offset_b = floor(u (N - n_sub + 1)); tag 4: point j is kept iff u_j < keep, u_j from call j >> 1, words
+ * (0, 1) if j is even, (2, 3) if odd.  mag as in agnvar_structure_function.
+ *   d_sf2      out [nlags] fp64 (0 where no pair survives);  d_pairs  out [nlags] i64 or NULL (pooled pair counts)
+ *   d_offsets  out [B] i64 or NULL
+ * EINVAL: bad B/N/dtype, n_sub < 2 or > N, keep not in (0, 1], bad lags, NULL d_x/d_sf2. */
+int agnvar_ensemble_sf(int64_t B, int64_t N, int dtype, const void* d_x, int64_t n_sub, double keep, uint64_t seed,
+                       uint32_t curve0, const int64_t* h_lags, int nlags, int mag, double* d_sf2, int64_t* d_pairs,
+                       int64_t* d_offsets, void* d_ws, size_t ws_bytes, void* stream);
+
+/* Moments of each curve's value distribution (the TK95 output-PDF check of sec. 3.2.1 / Fig. 2):
+ * d_out [B][4] fp64 = mean, variance (1/N), skewness m3 / m2^1.5, excess kurtosis m4 / m2^2 - 3.  No workspace.
+ * EINVAL: bad B/N/dtype, B > 2^31 - 1, NULL pointer. */
+int agnvar_moments(int64_t B, int64_t N, int dtype, const void* d_x, double* d_out, void* stream);
 
 /* O1 -- the raw random words every other call consumes (for bit-exact checks of the generator):
  * d_out[4 i + w] = word w of Philox4x32-10 with counter (lo(i0+i), hi(i0+i), curve, tag) and key

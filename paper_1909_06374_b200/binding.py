@@ -14,13 +14,14 @@ from . import _build
 
 AGNVAR_F32, AGNVAR_F64 = 0, 1
 AGNVAR_ERDF_BPL, AGNVAR_ERDF_LOGNORMAL = 0, 1
-OP_ERDF_SAMPLE_SORTED, OP_TK_GENERATE, OP_E13_ITERATE, OP_PERIODOGRAM, OP_STRUCTURE_FUNCTION, OP_DELTA_M_PROB = 1, 2, 3, 4, 5, 6
+(OP_ERDF_SAMPLE_SORTED, OP_TK_GENERATE, OP_E13_ITERATE, OP_PERIODOGRAM, OP_STRUCTURE_FUNCTION, OP_DELTA_M_PROB,
+ OP_ENSEMBLE_SF) = 1, 2, 3, 4, 5, 6, 7
 
 EXPORTS = (
     "agnvar_workspace_bytes", "agnvar_psd_bpl", "agnvar_erdf_sample_sorted", "agnvar_erdf_table", "agnvar_tk_generate",
     "agnvar_e13_iterate", "agnvar_periodogram", "agnvar_philox_u32", "agnvar_strerror", "agnvar_version",
     "agnvar_launch_count", "agnvar_trace_begin", "agnvar_trace_end", "agnvar_kernel_name",
-    "agnvar_structure_function", "agnvar_delta_m_prob",
+    "agnvar_structure_function", "agnvar_delta_m_prob", "agnvar_ensemble_sf", "agnvar_moments",
 )
 
 
@@ -85,6 +86,10 @@ def lib():
     L.agnvar_delta_m_prob.restype = i32
     L.agnvar_delta_m_prob.argtypes = [i64, i64, i32, vp, C.POINTER(i64), i32, C.POINTER(dbl), i32, dbl, i32, dbl, vp, vp,
                                       vp, sz, vp]
+    L.agnvar_ensemble_sf.restype = i32
+    L.agnvar_ensemble_sf.argtypes = [i64, i64, i32, vp, i64, dbl, u64, u32, C.POINTER(i64), i32, i32, vp, vp, vp, vp, sz, vp]
+    L.agnvar_moments.restype = i32
+    L.agnvar_moments.argtypes = [i64, i64, i32, vp, vp, vp]
     L.agnvar_philox_u32.restype = i32
     L.agnvar_philox_u32.argtypes = [u64, u64, i64, u32, u32, vp, vp]
     L.agnvar_strerror.restype = C.c_char_p
@@ -361,3 +366,32 @@ def agnvar_delta_m_prob(x, lags, dm_ref, m_zero=0.0, m_cut=None):
                                          0.0 if m_cut is None else float(m_cut), _ptr(prob), _ptr(cons), _ptr(ws),
                                          ws.numel(), _stream()), "agnvar_delta_m_prob")
     return prob, cons
+
+
+def agnvar_ensemble_sf(x, n_sub, keep, seed, lags, curve0=0, mag=False):
+    """NEXT-4 (Fig. 7-8): ensemble SF over masked consecutive sub-samples of every curve.
+    Returns dict(sf2 [nlags] fp64, pairs [nlags] i64, offsets [B] i64)."""
+    B, N = x.shape
+    code, _ = _dt(x.dtype)
+    dev = x.device
+    nl = len(lags)
+    arr = (C.c_int64 * nl)(*[int(l) for l in lags])
+    with _on(dev):
+        sf2 = torch.empty((nl,), dtype=torch.float64, device=dev)
+        pairs = torch.empty((nl,), dtype=torch.int64, device=dev)
+        offs = torch.empty((B,), dtype=torch.int64, device=dev)
+        ws = workspace(workspace_bytes(OP_ENSEMBLE_SF, B, n_sub, code, 1, nl), dev)
+        _check(lib().agnvar_ensemble_sf(B, N, code, _ptr(x), int(n_sub), float(keep), int(seed), int(curve0), arr, nl,
+                                        1 if mag else 0, _ptr(sf2), _ptr(pairs), _ptr(offs), _ptr(ws), ws.numel(), _stream()),
+               "agnvar_ensemble_sf")
+    return {"sf2": sf2, "pairs": pairs, "offsets": offs}
+
+
+def agnvar_moments(x):
+    """Per-curve mean, variance, skewness, excess kurtosis: [B][4] fp64 (Fig. 2's check of the TK95 output PDF)."""
+    B, N = x.shape
+    code, _ = _dt(x.dtype)
+    with _on(x.device):
+        out = torch.empty((B, 4), dtype=torch.float64, device=x.device)
+        _check(lib().agnvar_moments(B, N, code, _ptr(x), _ptr(out), _stream()), "agnvar_moments")
+    return out

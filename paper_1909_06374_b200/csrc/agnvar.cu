@@ -507,6 +507,37 @@ int dm_impl(int64_t B, int64_t N, const void* d_x, const int64_t* h_lags, int nl
     return cuda_status(cudaGetLastError());
 }
 
+// ---- NEXT-4: ensemble SF of masked sub-segments ---------------------------------------------------------------
+inline size_t ws_ens(int64_t B, int64_t n_sub, int64_t nlags) {
+    Carver c(nullptr);
+    c.take<long long>((size_t)nlags);
+    c.take<double>((size_t)B * n_sub);
+    c.take<unsigned char>((size_t)B * n_sub);
+    c.take<unsigned long long>((size_t)nlags);
+    c.take<double>((size_t)B * nlags * sf_chunks(n_sub));
+    return c.off;
+}
+template <typename T>
+int ens_impl(int64_t B, int64_t N, const void* d_x, int64_t n_sub, double keep, uint64_t seed, uint32_t curve0,
+             const int64_t* h_lags, int nlags, int mag, double* d_sf2, int64_t* d_pairs, int64_t* d_offsets, void* d_ws,
+             size_t ws_bytes, cudaStream_t st) {
+    if (ws_bytes < ws_ens(B, n_sub, nlags) || !d_ws || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
+    Carver c(d_ws);
+    long long* lags = c.take<long long>((size_t)nlags);
+    double* v = c.take<double>((size_t)B * n_sub);
+    unsigned char* kept = c.take<unsigned char>((size_t)B * n_sub);
+    unsigned long long* count = c.take<unsigned long long>((size_t)nlags);
+    const int nch = sf_chunks(n_sub);
+    double* partial = c.take<double>((size_t)B * nlags * nch);
+    CK(cudaMemcpyAsync(lags, h_lags, (size_t)nlags * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    CK(cudaMemsetAsync(count, 0, (size_t)nlags * sizeof(unsigned long long), st));
+    AGN_LAUNCH(K_SF, st, (ens_prepare_kernel<T><<<bgrid(cdiv(n_sub, 256), B), 256, 0, st>>>((const T*)d_x, N, n_sub, keep, seed, curve0, mag, v, kept,
+                                                                                        (long long*)d_offsets, (int)B)));
+    AGN_LAUNCH(K_SF, st, (ens_partial_kernel<<<dim3((unsigned)nch, (unsigned)nlags, (unsigned)B), 256, 0, st>>>(v, kept, n_sub, lags, nlags, partial, count, nch, (int)B)));
+    AGN_LAUNCH(K_SF, st, (ens_final_kernel<<<(unsigned)nlags, 256, 0, st>>>(partial, count, nch, nlags, (int)B, d_sf2, (long long*)d_pairs)));
+    return cuda_status(cudaGetLastError());
+}
+
 }  // namespace
 
 // =====================================================================================================
@@ -583,6 +614,9 @@ size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int overs
         case AGNVAR_OP_DELTA_M_PROB:
             if (aux < 1 || aux > 4096 || B > 65535) return 0;
             return ws_sf(B, N, aux, true);
+        case AGNVAR_OP_ENSEMBLE_SF:
+            if (aux < 1 || aux > 4096 || B > 65535) return 0;
+            return ws_ens(B, N, aux);
         default: return 0;
     }
 }
@@ -731,6 +765,26 @@ int agnvar_delta_m_prob(int64_t B, int64_t N, int dtype, const void* d_x, const 
                               ws_bytes, (cudaStream_t)stream);
     return dm_impl<double>(B, N, d_x, h_lags, nlags, h_dm_ref, nref, m_zero, use_cut, m_cut, d_prob, d_considered, d_ws,
                            ws_bytes, (cudaStream_t)stream);
+}
+
+int agnvar_ensemble_sf(int64_t B, int64_t N, int dtype, const void* d_x, int64_t n_sub, double keep, uint64_t seed,
+                       uint32_t curve0, const int64_t* h_lags, int nlags, int mag, double* d_sf2, int64_t* d_pairs,
+                       int64_t* d_offsets, void* d_ws, size_t ws_bytes, void* stream) {
+    if (!valid_BN(B, N) || B > 65535 || !valid_dtype(dtype) || !d_x || !d_sf2 || !valid_lags(h_lags, nlags)) return AGNVAR_EINVAL;
+    if (n_sub < 2 || n_sub > N || !(keep > 0.0) || !(keep <= 1.0)) return AGNVAR_EINVAL;
+    if (dtype == AGNVAR_F32)
+        return ens_impl<float>(B, N, d_x, n_sub, keep, seed, curve0, h_lags, nlags, mag, d_sf2, d_pairs, d_offsets, d_ws,
+                               ws_bytes, (cudaStream_t)stream);
+    return ens_impl<double>(B, N, d_x, n_sub, keep, seed, curve0, h_lags, nlags, mag, d_sf2, d_pairs, d_offsets, d_ws,
+                            ws_bytes, (cudaStream_t)stream);
+}
+
+int agnvar_moments(int64_t B, int64_t N, int dtype, const void* d_x, double* d_out, void* stream) {
+    if (!valid_BN(B, N) || B > 0x7fffffffll || !valid_dtype(dtype) || !d_x || !d_out) return AGNVAR_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == AGNVAR_F32) AGN_LAUNCH(K_SF, st, (moments_kernel<float><<<(unsigned)B, 256, 0, st>>>((const float*)d_x, N, d_out)));
+    else AGN_LAUNCH(K_SF, st, (moments_kernel<double><<<(unsigned)B, 256, 0, st>>>((const double*)d_x, N, d_out)));
+    return cuda_status(cudaGetLastError());
 }
 
 int agnvar_periodogram(int64_t B, int64_t N, int dtype, const void* d_x, double dt, int norm, int nbins,

@@ -134,4 +134,100 @@ __global__ void dm_final_kernel(const unsigned long long* __restrict__ counts, c
     if (considered_out && i % nref == 0) considered_out[bq] = (long long)P;
 }
 
+// ------------------------------------------------------------------------------------------------
+// NEXT-4: ensemble SF of masked sub-segments (Fig. 7-8; Q23) and moments (Fig. 2)
+// ------------------------------------------------------------------------------------------------
+// one thread per (curve, point j of the sub-sample): offset from Philox tag 3, keep flag from tag 4, value (or magnitude)
+template <typename T>
+__global__ void __launch_bounds__(256) ens_prepare_kernel(const T* __restrict__ x, long long N, long long n_sub, double keep,
+                                                          uint64_t seed, uint32_t curve0, int mag, double* __restrict__ v,
+                                                          unsigned char* __restrict__ kept, long long* __restrict__ offsets, int B) {
+    const long long b = bidx();
+    const long long j = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (b >= B || j >= n_sub) return;
+    const uint4 w3 = philox_stream(seed, 0ull, curve0 + (uint32_t)b, 3u);
+    const long long off = (long long)floor(u53(w3.x, w3.y) * (double)(N - n_sub + 1));
+    if (j == 0 && offsets) offsets[b] = off;
+    const uint4 w4 = philox_stream(seed, (uint64_t)(j >> 1), curve0 + (uint32_t)b, 4u);
+    const double u = (j & 1) ? u53(w4.z, w4.w) : u53(w4.x, w4.y);
+    kept[b * n_sub + j] = (u < keep) ? 1 : 0;
+    const double xv = (double)x[b * N + off + j];
+    v[b * n_sub + j] = mag ? -2.5 * log10(xv) : xv;
+}
+
+// partial[b][q][chunk] = sum over the chunk's kept pairs of (v_j - v_{j+l})^2; count[q] += number of kept pairs
+__global__ void __launch_bounds__(256) ens_partial_kernel(const double* __restrict__ v, const unsigned char* __restrict__ kept,
+                                                          long long n_sub, const long long* __restrict__ lags, int nlags,
+                                                          double* __restrict__ partial, unsigned long long* __restrict__ count,
+                                                          int nchunks, int B) {
+    __shared__ double sh[256];
+    const long long b = blockIdx.z;
+    const int q = blockIdx.y;
+    const long long l = lags[q];
+    const long long P = n_sub - l;
+    const long long beg = (long long)blockIdx.x * kSfChunk;
+    const long long end = beg + kSfChunk < P ? beg + kSfChunk : P;
+    const double* vb = v + b * n_sub;
+    const unsigned char* kb = kept + b * n_sub;
+    double acc = 0.0;
+    unsigned int np = 0;
+    for (long long i = beg + threadIdx.x; i < end; i += 256) {
+        if (kb[i] & kb[i + l]) {
+            const double d = vb[i] - vb[i + l];
+            acc += d * d;
+            ++np;
+        }
+    }
+    const double tot = block_sum<256>(acc, sh);
+    if (threadIdx.x == 0) partial[(b * nlags + q) * nchunks + blockIdx.x] = tot;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) np += __shfl_xor_sync(0xffffffffu, np, o);
+    if ((threadIdx.x & 31) == 0 && np) atomicAdd(&count[q], (unsigned long long)np);
+}
+
+// pooled over the curves, fixed order: sf2[q] = (sum_b sum_chunk partial) / count[q]
+__global__ void __launch_bounds__(256) ens_final_kernel(const double* __restrict__ partial, const unsigned long long* __restrict__ count,
+                                                        int nchunks, int nlags, int B, double* __restrict__ sf2,
+                                                        long long* __restrict__ pairs) {
+    __shared__ double sh[256];
+    const int q = blockIdx.x;
+    double acc = 0.0;
+    const long long per = nchunks;
+    for (long long i = threadIdx.x; i < (long long)B * per; i += 256) {
+        const long long b = i / per, c = i - b * per;
+        acc += partial[(b * nlags + q) * nchunks + c];
+    }
+    const double tot = block_sum<256>(acc, sh);
+    if (threadIdx.x == 0) {
+        const unsigned long long n = count[q];
+        sf2[q] = n ? tot / (double)n : 0.0;
+        if (pairs) pairs[q] = (long long)n;
+    }
+}
+
+// per curve: mean, variance (1/N), skewness, excess kurtosis (two passes, fixed-order fp64 sums)
+template <typename T>
+__global__ void __launch_bounds__(256) moments_kernel(const T* __restrict__ x, long long N, double* __restrict__ out) {
+    __shared__ double sh[256];
+    const long long b = blockIdx.x;
+    const T* xb = x + b * N;
+    double s1 = 0.0;
+    for (long long i = threadIdx.x; i < N; i += 256) s1 += (double)xb[i];
+    const double mu = block_sum<256>(s1, sh) / (double)N;
+    double a2 = 0.0, a3 = 0.0, a4 = 0.0;
+    for (long long i = threadIdx.x; i < N; i += 256) {
+        const double d = (double)xb[i] - mu, d2 = d * d;
+        a2 += d2; a3 += d2 * d; a4 += d2 * d2;
+    }
+    const double m2 = block_sum<256>(a2, sh) / (double)N;
+    const double m3 = block_sum<256>(a3, sh) / (double)N;
+    const double m4 = block_sum<256>(a4, sh) / (double)N;
+    if (threadIdx.x == 0) {
+        out[b * 4 + 0] = mu;
+        out[b * 4 + 1] = m2;
+        out[b * 4 + 2] = m2 > 0.0 ? m3 / (m2 * sqrt(m2)) : 0.0;
+        out[b * 4 + 3] = m2 > 0.0 ? m4 / (m2 * m2) - 3.0 : 0.0;
+    }
+}
+
 }  // namespace agn

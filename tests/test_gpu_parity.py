@@ -513,3 +513,37 @@ def test_onchip_loop_early_exit_is_a_fixed_point(ag, orc, N):
     xadj = again["x_adj"].cpu().numpy()
     for b in np.flatnonzero(conv)[:6]:
         assert (u32(p)[b] == orc.stable_argsort(xadj[b].astype(np.float64))).all()
+
+
+# ---- NEXT-4: ensemble SF of masked sub-segments (Fig. 7-8), output-PDF moments of TK95 series (Fig. 2) ------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("keep", [1.0, 0.1, 0.01])
+def test_ensemble_sf(ag, orc, dtype, keep):
+    """Offsets and masks come from Philox (integers: exact); the pooled pair counts are exact and the pooled sums are
+    fp64 on both sides (<= 1e-12 relative)."""
+    B, N, n_sub, seed, curve0 = 40, 2 ** 14, 1000, 17, 3
+    srt, perm0, an = _inputs(ag, BPL, PSD, B, N, 1, dtype, 14)
+    x = ag.agnvar_e13_iterate(an, srt, perm0, 3)["x"]
+    xh = x.cpu().numpy().astype(np.float64)
+    lags = [1, 2, 5, 10, 30, 100, 300, 999, 1000]
+    for mag in (False, True):
+        out = ag.agnvar_ensemble_sf(x, n_sub, keep, seed, lags, curve0=curve0, mag=mag)
+        sf2, pairs, offs = orc.ensemble_sf(xh, n_sub, keep, seed, curve0, lags, mag)
+        assert (out["offsets"].cpu().numpy() == offs).all()
+        assert (out["pairs"].cpu().numpy() == pairs).all()
+        assert np.allclose(out["sf2"].cpu().numpy(), sf2, rtol=1e-12, atol=0)
+    if keep == 1.0:
+        assert pairs[0] == B * (n_sub - 1) and pairs[-1] == 0
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_moments_of_tk_series(ag, orc, dtype):
+    """TK95-only ensemble (sec. 3.2.1 / Fig. 2): moments of the generated series against the oracle's on the same values."""
+    B, N = 6, 2 ** 15
+    xn, _ = ag.agnvar_tk_generate(dict(A=0.0, f_b=1.0, alpha_low=2.5, alpha_high=2.5), B, N, 1.0, 1, dtype, 23, 0)
+    got = ag.agnvar_moments(xn).cpu().numpy()
+    xh = xn.cpu().numpy().astype(np.float64)
+    for b in range(B):
+        ref = orc.moments(xh[b])
+        assert got[b][0] == pytest.approx(ref[0], rel=1e-9, abs=1e-12 * np.sqrt(ref[1]))
+        assert np.allclose(got[b][1:], ref[1:], rtol=1e-10, atol=1e-12)
