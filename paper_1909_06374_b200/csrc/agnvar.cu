@@ -82,6 +82,7 @@ template <typename T> size_t ws_e13(int64_t B, int64_t N, bool delta) {
         c.take<uint32_t>((size_t)B * N);      // second working permutation (d_perm is output only)
         c.take<double>((size_t)B * delta_chunks(N));
     }
+    if (bucket1_wb_applicable(sizeof(T), N)) c.take<unsigned char>(bucket1_wb_bytes(B, N));   // write-back records of the sort
     return c.off + sort_ws_any<T>(B, N);
 }
 template <typename T> size_t ws_tk(int64_t B, int64_t N, int os) {
@@ -167,6 +168,11 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
         P0 = c.take<uint32_t>((size_t)B * N);
         dpartial = c.take<double>((size_t)B * nch);
     }
+    // long fp32 curves: the sort also carries the values home (L4 + L5 in three kernels, bucket1.cuh write-back mode)
+    const bool wb_mode = bucket1_wb_applicable(sizeof(T), N);
+    B1Wb wb;
+    memset(&wb, 0, sizeof(wb));
+    if (wb_mode) bucket1_wb_carve(c.take<unsigned char>(bucket1_wb_bytes(B, N)), B, N, &wb);
     void* sort_ws = (unsigned char*)d_ws + c.off;
     const bool two_level = N >= (1ll << kTwoLevelScatterLog);
     // the binned (value, dst) pairs live in the sort's ping-pong buffers, which are idle after the sort
@@ -222,10 +228,12 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
         CK(cudaMemcpyAsync(P0, d_perm, (size_t)B * N * 4, cudaMemcpyDeviceToDevice, st));
         cur = P0; x = XA; xn = XB;
     }
-    auto rank_scatter = [&](const uint32_t* inew, const uint32_t* iold, T* xout, void* spare, bool count) -> int {
+    // gate != null: only the curves with gate[b] != 0 (those the write-back sort gave up on)
+    auto rank_scatter = [&](const uint32_t* inew, const uint32_t* iold, T* xout, void* spare, bool count,
+                            const uint32_t* gate) -> int {
         if constexpr (sizeof(T) == 4) {
             if (two_level && sort32_applicable(sizeof(T), N)) {
-                if (rank_scatter_two_level32(inew, iold, sorted, xout, B, N, (uint2*)spare, cursor, changed, st) != cudaSuccess)
+                if (rank_scatter_two_level32(inew, iold, sorted, xout, B, N, (uint2*)spare, cursor, changed, st, gate) != cudaSuccess)
                     return AGNVAR_ECUDA;
                 return AGNVAR_OK;
             }
@@ -234,14 +242,14 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
             if (rank_scatter_two_level<T>(inew, iold, sorted, xout, B, N, pv, pd, cursor, changed, st) != cudaSuccess)
                 return AGNVAR_ECUDA;
         } else if (count) {
-            AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(inew, iold, sorted, xout, N, changed, (int)B)));
+            AGN_LAUNCH(gate ? K_SORT_FALLBACK : K_SCATTER, st, (scatter_count_kernel<T, true><<<bgrid(sg, B), 256, 0, st>>>(inew, iold, sorted, xout, N, changed, (int)B, gate)));
         } else {
             AGN_LAUNCH(K_SCATTER, st, (scatter_count_kernel<T, false><<<bgrid(sg, B), 256, 0, st>>>(inew, nullptr, sorted, xout, N, nullptr, (int)B)));
         }
         return AGNVAR_OK;
     };
     // first x_sim: the draw in draw order (Q15); idx_old = idx_new, so the change count stays 0
-    if (int rc = rank_scatter(cur, cur, x, sort_ws, false)) return rc;
+    if (int rc = rank_scatter(cur, cur, x, sort_ws, false, nullptr)) return rc;
     int k_done = 0;
     for (int k = 1; k <= max_iter; ++k) {
         if constexpr (sizeof(T) == 4) if (use2) {
@@ -267,14 +275,16 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
         if constexpr (sizeof(T) == 4) {
             if (sort32_applicable(sizeof(T), N)) {
                 uint2* sp = nullptr;
-                if (seg_argsort32(Z, nxt, nullptr, B, N, sort_ws, &sp, st, &sort_gate) != cudaSuccess) return AGNVAR_ECUDA;
+                if (wb_mode) { wb.sorted = (const float*)sorted; wb.idx_old = cur; wb.changed = changed; wb.x_out = (float*)xn; }
+                if (seg_argsort32((const float*)Z, nxt, nullptr, B, N, sort_ws, &sp, st, &sort_gate, wb_mode ? &wb : nullptr) != cudaSuccess)
+                    return AGNVAR_ECUDA;
                 spare = sp;
                 sorted_here = true;
             }
         }
         if (!sorted_here && seg_argsort<T>(Z, nxt, nullptr, B, N, sort_ws, st) != cudaSuccess) return AGNVAR_ECUDA;
-        // L5 rank scatter + change count
-        if (int rc = rank_scatter(nxt, cur, xn, spare, true)) return rc;
+        // L5 rank scatter + change count (write-back mode: already done by the sort, except for curves on the fallback)
+        if (int rc = rank_scatter(nxt, cur, xn, spare, true, wb_mode ? sort_gate : nullptr)) return rc;
         // delta_k (Eq. 4) between x_sim,k (x) and x_sim,k+1 (xn)
         if (dmode)
             AGN_LAUNCH(K_DELTA, st, (delta_partial_kernel<T><<<bgrid((unsigned)nch, B), 256, 0, st>>>(x, xn, N, dpartial, nch, (int)B)));

@@ -49,6 +49,8 @@ struct Part1Args {
     uint32_t* cursor;           // [B][nb] zero on entry
     uint32_t* overflow;         // [B]
     const uint2* tab;           // [B][65536]
+    uint32_t* loc;              // write-back mode (else null): [B][N] slab position (bucket * kB1Cap + offset) of the pair
+    unsigned short* jrec;       //   at stage position s of the tile, and its sample number inside the tile, in STAGE order
     uint32_t N, nb, M;
     long long B;
 };
@@ -178,6 +180,22 @@ __global__ void __launch_bounds__(kB1PartThreads, 2) part1_kernel(Part1Args a) {
     }
     __syncthreads();
     uint2* out = a.out + (size_t)b * nb * kB1Cap;
+    if (a.loc) {
+        // write-back mode: remember, in stage order (coalesced), where every pair went and which sample it was
+        uint32_t* lo = a.loc + (size_t)b * a.N + tile0;
+        unsigned short* jo = a.jrec + (size_t)b * a.N + tile0;
+#pragma unroll 4
+        for (int s = t; s < kB1Tile; s += kB1PartThreads) {
+            const uint2 e = stage[s];
+            const uint32_t d = e.y >> 13;
+            const uint32_t off = cnt[d] + (uint32_t)s;
+            const uint32_t l = d * (uint32_t)kB1Cap + off;
+            if (off < (uint32_t)kB1Cap) out[l] = make_uint2(e.x, tile0 + (e.y & 0x1fffu));
+            lo[s] = l;
+            jo[s] = (unsigned short)(e.y & 0x1fffu);
+        }
+        return;
+    }
 #pragma unroll 4
     for (int s = t; s < kB1Tile; s += kB1PartThreads) {
         const uint2 e = stage[s];
@@ -192,10 +210,27 @@ __global__ void __launch_bounds__(kB1PartThreads, 2) part1_kernel(Part1Args a) {
 // ------------------------------------------------------------------------------------------------
 struct B1Smem {
     unsigned long long pair[kB1Cap];      // (key << 32) | index, grouped by slot
+    uint32_t cwpad[4];                    // cwpad[3] stays 0: the "end of slot -1" of the 16-bit view of cw
     uint32_t cw[kB1Slots / 2];            // two 16-bit counters per word: populations, then starts, then ends of the slots
     uint32_t wsum[kB1SortThreads / 32];
 };
+static_assert(sizeof(B1Smem) <= 115712, "two finish CTAs per SM");
 
+// Write-back mode (the E13 loop, L4 + L5 in one go): the finish kernel does not only emit idx_new[r]; it also counts the
+// rank changes against idx_old[r] and writes the VALUE that belongs to the pair, sorted[r] (L5: x[idx_new[r]] =
+// sorted[r]), to the pair's own slab position in `valslab`.  gather_back_kernel then brings the values home along
+// the records part1_kernel kept (loc, jrec), replacing the two-level rank scatter (bin + place).
+struct B1Wb {
+    const float* sorted;            // [B][N] the ERDF draw in rank order
+    const uint32_t* idx_old;        // [B][N] permutation of the previous iteration
+    unsigned long long* changed;    // [B]
+    float* valslab;                 // [B][nb][kB1Cap]
+    uint32_t* loc;                  // [B][N]
+    unsigned short* jrec;           // [B][N]
+    float* x_out;                   // [B][N]
+};
+
+template <bool WB>
 __global__ void __launch_bounds__(kB1SortThreads, 2) bucket1_sort_kernel(const uint2* __restrict__ slabs,
                                                                          const uint32_t* __restrict__ cursor,
                                                                          const uint32_t* __restrict__ base,
@@ -203,7 +238,7 @@ __global__ void __launch_bounds__(kB1SortThreads, 2) bucket1_sort_kernel(const u
                                                                          const uint32_t* __restrict__ klos,
                                                                          uint32_t* __restrict__ idx_out,
                                                                          float* __restrict__ sorted_out, uint32_t N,
-                                                                         uint32_t nb, long long B) {
+                                                                         uint32_t nb, long long B, B1Wb wb) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     B1Smem& sm = *reinterpret_cast<B1Smem*>(smem_raw);
     const long long b = bidx();
@@ -233,6 +268,8 @@ __global__ void __launch_bounds__(kB1SortThreads, 2) bucket1_sort_kernel(const u
     constexpr int WPT = kB1Slots / 2 / kB1SortThreads;      // counter words per thread in the scan (4 = one uint4)
     static_assert(WPT == 4, "one uint4 of packed counters per thread");
     reinterpret_cast<uint4*>(sm.cw)[t] = make_uint4(0u, 0u, 0u, 0u);
+    if (t == 0) sm.cwpad[3] = 0u;
+    const unsigned short* send = reinterpret_cast<const unsigned short*>(sm.cw);       // after step 3: send[s] = end of slot s
     __syncthreads();
     // 1. slot populations (the slab stays in L2 for step 3).  (Two pairs per 128-bit load measured slower: 1.85 vs 1.69 ms.)
 #pragma unroll 4
@@ -256,9 +293,19 @@ __global__ void __launch_bounds__(kB1SortThreads, 2) bucket1_sort_kernel(const u
         }
         if (lane == 31) sm.wsum[warp] = inc;
         __syncthreads();
-        uint32_t run = inc - sum;
+        if (warp == 0) {
+            // exclusive scan of the 32 warp totals
+            const uint32_t wt = sm.wsum[lane];
+            uint32_t wi = wt;
 #pragma unroll
-        for (int wv = 0; wv < kB1SortThreads / 32; ++wv) run += (wv < warp) ? sm.wsum[wv] : 0u;
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t m = __shfl_up_sync(0xffffffffu, wi, o);
+                if (lane >= o) wi += m;
+            }
+            sm.wsum[lane] = wi - wt;
+        }
+        __syncthreads();
+        uint32_t run = inc - sum + sm.wsum[warp];
         uint32_t o[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -277,21 +324,103 @@ __global__ void __launch_bounds__(kB1SortThreads, 2) bucket1_sort_kernel(const u
         const uint32_t sh = (s & 1u) << 4;
         const uint32_t q = (atomicAdd(&sm.cw[s >> 1], 1u << sh) >> sh) & 0xffffu;
         sm.pair[q] = ((unsigned long long)kv.x << 32) | kv.y;
+        if (WB) reinterpret_cast<uint32_t*>(wb.valslab)[((size_t)b * nb + bk) * kB1Cap + e] = q;   // read back in step 4C
     }
     __syncthreads();
     // 4. exact rank of every pair among its slot mates (they are contiguous; the 64-bit (key, index) words are all
     //    distinct), one pair per thread at a time, and the index goes to that rank
     uint32_t* io = idx_out + (size_t)b * N + r0;
+    if (WB) {
+        // L4 + L5 for this bucket.  Nothing below touches global memory at a scattered address: the ranks of a bucket
+        // are contiguous (r0 .. r0 + n), so idx_new, idx_old and sorted[] are accessed in RANK order (coalesced), the
+        // value slab in SLAB order (coalesced), and the two orders meet in shared memory.  An index needs 26 bits
+        // (N <= 2^26): the 6 spare bits of the low word at position r say where the pair of rank r sits, as a signed
+        // offset inside the slot (slots of <= 31 pairs; a larger slot -- massive ties -- is marked and takes a slow,
+        // still exact, path).
+        constexpr uint32_t IDXM = 0x03ffffffu;
+        constexpr unsigned long long CMPM = 0xffffffff03ffffffull;
+        constexpr uint32_t BIG = 0x80000000u;                           // offset field = -32: "this slot is big"
+        uint32_t* plo = reinterpret_cast<uint32_t*>(sm.pair);           // little endian: word 2 q = index, 2 q + 1 = key
+        const uint32_t* iold = wb.idx_old + (size_t)b * N + r0;
+        const float* srt = wb.sorted + (size_t)b * N + r0;
+        uint32_t* vs = reinterpret_cast<uint32_t*>(wb.valslab) + ((size_t)b * nb + bk) * kB1Cap;
+        uint32_t diff = 0;
+        // (sorted[] and idx_old of this bucket's ranks are first touched in 4B: have them in L2 by then)
+        if ((uint32_t)t * 32u < n) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(srt + t * 32));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(iold + t * 32));
+        }
+        // 4A. rank of every pair inside its slot; position r learns where its pair is
+#pragma unroll 2
+        for (uint32_t q = t; q < n; q += kB1SortThreads) {
+            const unsigned long long v = sm.pair[q] & CMPM;             // (another pair's offset may already sit here)
+            const int s = (int)slot_of((uint32_t)(v >> 32));
+            const uint32_t a = send[s - 1], z = send[s];
+            const uint32_t k = z - a;
+            if (k == 1u) continue;
+            uint32_t c;
+            if (k == 2u) {
+                c = ((sm.pair[q == a ? a + 1u : a] & CMPM) < v);
+            } else {
+                c = 0;
+                uint32_t h = a;
+                for (; h + 1u < z; h += 2u) {
+                    const unsigned long long m0 = sm.pair[h] & CMPM, m1 = sm.pair[h + 1u] & CMPM;
+                    c += (m0 < v);
+                    c += (m1 < v);
+                }
+                if (h < z) c += ((sm.pair[h] & CMPM) < v);
+            }
+            const uint32_t r = a + c;
+            if (k <= 31u) {
+                plo[2 * r] = (plo[2 * r] & IDXM) | ((q - r) << 26);     // the index bits of position r never change
+            } else {
+                plo[2 * q] = (uint32_t)v | BIG;
+                io[r] = (uint32_t)v;
+                diff += (__ldg(iold + r) != (uint32_t)v);
+            }
+        }
+        __syncthreads();
+        // 4B. rank order: the pair of rank p gives its index and takes sorted[r0 + p] (into the key half of its word:
+        //     keys are not needed any more)
+#pragma unroll 2
+        for (uint32_t p = t; p < n; p += kB1SortThreads) {
+            const uint32_t lo = plo[2 * p];
+            if ((lo & 0xfc000000u) == BIG) continue;                    // big slot: done in 4A / 4C
+            const uint32_t h = p + (uint32_t)((int32_t)lo >> 26);
+            const uint32_t idx = plo[2 * h] & IDXM;
+            io[p] = idx;
+            diff += (__ldcs(iold + p) != idx);
+            plo[2 * h + 1] = __float_as_uint(__ldcs(srt + p));
+        }
+        __syncthreads();
+        // 4C. slab order: the value of the pair that came from slab position e goes back to position e
+        for (uint32_t e = t; e < n; e += kB1SortThreads) {
+            const uint32_t q = vs[e];
+            const uint32_t lo = plo[2 * q], hi = plo[2 * q + 1];
+            uint32_t val = hi;
+            if ((lo & 0xfc000000u) == BIG) {
+                const int s = (int)slot_of(hi);
+                const uint32_t a = send[s - 1], z = send[s];
+                const unsigned long long v = ((unsigned long long)hi << 32) | (lo & IDXM);
+                uint32_t r = a;
+                for (uint32_t h = a; h < z; ++h) r += ((sm.pair[h] & CMPM) < v);
+                val = __float_as_uint(__ldg(srt + r));
+            }
+            vs[e] = val;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) diff += __shfl_xor_sync(0xffffffffu, diff, o);
+        if (lane == 0 && diff) atomicAdd(&wb.changed[b], (unsigned long long)diff);
+        return;
+    }
     float* so = sorted_out ? sorted_out + (size_t)b * N + r0 : nullptr;
 #pragma unroll 2
     for (uint32_t q = t; q < n; q += kB1SortThreads) {
         const unsigned long long v = sm.pair[q];
         const uint32_t key = (uint32_t)(v >> 32);
-        const uint32_t s = slot_of(key);
-        const uint32_t w = sm.cw[s >> 1];
-        uint32_t z, a;
-        if (s & 1u) { z = w >> 16; a = w & 0xffffu; }
-        else { z = w & 0xffffu; a = s ? (sm.cw[(s >> 1) - 1] >> 16) : 0u; }
+        const int s = (int)slot_of(key);
+        const uint32_t a = send[s - 1], z = send[s];
         uint32_t r = q;
         if (z - a > 1u) {
             r = a;
@@ -302,19 +431,73 @@ __global__ void __launch_bounds__(kB1SortThreads, 2) bucket1_sort_kernel(const u
     }
 }
 
+// L5 of the write-back mode: x[tile0 + jrec[s]] = valslab[loc[s]] for the stage positions s of one partition tile.
+// loc / jrec are read in stage order (coalesced), the slab values along the runs part1_kernel wrote (consecutive s of
+// a run are consecutive slab positions), and the tile is put into time order in shared memory before it is stored.
+constexpr int kB1GatherThreads = 512;
+__global__ void __launch_bounds__(kB1GatherThreads, 4) gather_back_kernel(const uint32_t* __restrict__ loc,
+                                                                          const unsigned short* __restrict__ jrec,
+                                                                          const float* __restrict__ valslab,
+                                                                          const uint32_t* __restrict__ overflow,
+                                                                          float* __restrict__ x, uint32_t N, uint32_t nb,
+                                                                          long long B) {
+    __shared__ __align__(16) float xs[kB1Tile];
+    const long long b = bidx();
+    if (b >= B) return;
+    if (overflow[b]) return;                       // this curve takes the LSD sort and the plain rank scatter
+    const int t = threadIdx.x;
+    const size_t g0 = (size_t)b * N + (size_t)blockIdx.x * kB1Tile;
+    const float* vs = valslab + (size_t)b * nb * kB1Cap;
+    const uint4* l4 = reinterpret_cast<const uint4*>(loc + g0);
+    const uint2* j4 = reinterpret_cast<const uint2*>(jrec + g0);
+    constexpr int NV = kB1Tile / 4 / kB1GatherThreads;      // 4 vectors of 4 records per thread
+    uint4 l[NV];
+    uint2 j[NV];
+#pragma unroll
+    for (int k = 0; k < NV; ++k) { l[k] = __ldcs(l4 + k * kB1GatherThreads + t); j[k] = __ldcs(j4 + k * kB1GatherThreads + t); }
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        const float v0 = __ldcs(vs + l[k].x), v1 = __ldcs(vs + l[k].y), v2 = __ldcs(vs + l[k].z), v3 = __ldcs(vs + l[k].w);
+        xs[j[k].x & 0xffffu] = v0; xs[j[k].x >> 16] = v1; xs[j[k].y & 0xffffu] = v2; xs[j[k].y >> 16] = v3;
+    }
+    __syncthreads();
+    float4* xo = reinterpret_cast<float4*>(x + g0);
+#pragma unroll
+    for (int k = 0; k < NV; ++k) __stcs(xo + k * kB1GatherThreads + t, reinterpret_cast<const float4*>(xs)[k * kB1GatherThreads + t]);
+}
+
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
 inline cudaError_t bucket1_set_attrs() {
     cudaFuncSetAttribute(part1_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    cudaFuncSetAttribute(bucket1_sort_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaFuncSetAttribute(bucket1_sort_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaFuncSetAttribute(bucket1_sort_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     cudaError_t e = cudaFuncSetAttribute(part1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)part1_smem(kB1MaxBuckets));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket1_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(B1Smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket1_sort_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(B1Smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket1_sort_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(B1Smem));
     return e;
 }
 
 // pair scratch (uint2 units): slabs [B][nb][kB1Cap]
 inline size_t bucket1_pair_elems(long long B, long long N) { return (size_t)B * (size_t)(N >> kB1MeanLog) * kB1Cap; }
+
+// The write-back mode pays where the plain rank scatter needs two levels (N >= 2^22: bin + place, 2.5 ms per C4
+// iteration, against 0.94 for gather_back + 1.05 more in the finish kernel + 0.23 in part1: C4 470 -> 464 ms per step);
+// for shorter curves the one-kernel scatter inside an L2-resident window is cheaper (C3: 750 vs 835 ms per step).
+inline bool bucket1_wb_applicable(size_t elem_size, long long N) { return bucket1_applicable(elem_size, N) && N >= (1ll << 22); }
+
+// write-back scratch of the E13 loop: loc u32 [B][N] | jrec u16 [B][N] | valslab f32 [B][nb][kB1Cap]
+inline size_t bucket1_wb_bytes(long long B, long long N) {
+    return align_up((size_t)B * N * 4, 256) + align_up((size_t)B * N * 2, 256) + align_up(bucket1_pair_elems(B, N) * 4, 256);
+}
+inline void bucket1_wb_carve(void* p, long long B, long long N, B1Wb* wb) {
+    unsigned char* w = (unsigned char*)p;
+    wb->loc = (uint32_t*)w; w += align_up((size_t)B * N * 4, 256);
+    wb->jrec = (unsigned short*)w; w += align_up((size_t)B * N * 2, 256);
+    wb->valslab = (float*)w;
+}
+
 
 // control words: hist [B][65536] u32 | cursor [B][nb] | overflow [B] (zeroed per call) | tab [B][65536] uint2 |
 //                base [B][nb] | klo [B][nb+1]
@@ -330,8 +513,11 @@ inline size_t bucket1_ctl_bytes(long long B, long long N) {
 
 // vals [B][N] -> idx_out (and optionally the sorted values) for the curves whose buckets all fit; *overflow_out points
 // at the per-curve flags (1 = not sorted here).  pairs: bucket1_pair_elems(B, N) (key, index) pairs of scratch.
+// wb != null: write-back mode (see B1Wb): also x_out[idx_out[r]] = sorted[r] and the rank-change count, for the curves
+// whose buckets all fit.
 inline cudaError_t bucket1_sort(const float* vals, uint32_t* idx_out, float* sorted_out, long long B, long long N,
-                                uint2* pairs, void* ctl, const uint32_t** overflow_out, cudaStream_t st) {
+                                uint2* pairs, void* ctl, const uint32_t** overflow_out, cudaStream_t st,
+                                const B1Wb* wb = nullptr) {
     const uint32_t nb = (uint32_t)(N >> kB1MeanLog);
     unsigned char* w = (unsigned char*)ctl;
     uint32_t* hist = (uint32_t*)w;
@@ -352,11 +538,19 @@ inline cudaError_t bucket1_sort(const float* vals, uint32_t* idx_out, float* sor
     Part1Args a;
     a.vals = vals; a.out = pairs; a.cursor = cursor; a.overflow = overflow; a.tab = tab;
     a.N = (uint32_t)N; a.nb = nb; a.M = M; a.B = B;
-    AGN_LAUNCH(K_SORT_PART_ONE, st, (part1_kernel<<<bgrid((unsigned)(N / kB1Tile), B), kB1PartThreads, part1_smem(nb), st>>>(a)));
+    a.loc = wb ? wb->loc : nullptr; a.jrec = wb ? wb->jrec : nullptr;
+    AGN_LAUNCH(wb ? K_SORT_PART_ONE_WB : K_SORT_PART_ONE, st, (part1_kernel<<<bgrid((unsigned)(N / kB1Tile), B), kB1PartThreads, part1_smem(nb), st>>>(a)));
     const uint32_t bchunks = nb >= 1024 ? nb / 1024 : 1u;
     AGN_LAUNCH(K_SORT_CDF, st, (bucket_base_kernel<<<(unsigned)(B * bchunks), 1024, 0, st>>>(cursor, base, nb, bchunks, (uint32_t)kB1Cap)));
-    AGN_LAUNCH(K_SORT_BUCKET, st, (bucket1_sort_kernel<<<bgrid(nb, B), kB1SortThreads, sizeof(B1Smem), st>>>(
-        pairs, cursor, base, overflow, klo, idx_out, sorted_out, (uint32_t)N, nb, B)));
+    if (wb) {
+        AGN_LAUNCH(K_SORT_BUCKET_WB, st, (bucket1_sort_kernel<true><<<bgrid(nb, B), kB1SortThreads, sizeof(B1Smem), st>>>(
+            pairs, cursor, base, overflow, klo, idx_out, sorted_out, (uint32_t)N, nb, B, *wb)));
+        AGN_LAUNCH(K_GATHER_BACK, st, (gather_back_kernel<<<bgrid((unsigned)(N / kB1Tile), B), kB1GatherThreads, 0, st>>>(
+            wb->loc, wb->jrec, wb->valslab, overflow, wb->x_out, (uint32_t)N, nb, B)));
+    } else {
+        AGN_LAUNCH(K_SORT_BUCKET, st, (bucket1_sort_kernel<false><<<bgrid(nb, B), kB1SortThreads, sizeof(B1Smem), st>>>(
+            pairs, cursor, base, overflow, klo, idx_out, sorted_out, (uint32_t)N, nb, B, B1Wb())));
+    }
     *overflow_out = overflow;
     return cudaGetLastError();
 }

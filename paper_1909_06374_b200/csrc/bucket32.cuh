@@ -164,6 +164,7 @@ struct PartArgs {
     uint32_t nc;                // coarse slabs per curve
     uint32_t cap_in, cap_out;
     uint32_t tiles_in;          // LEVEL 1: tiles per coarse slab
+    const uint32_t* gate;       // LEVEL 2: if not null, only the curves with gate[b] != 0 are processed
     long long B;
 };
 
@@ -174,6 +175,7 @@ __global__ void __launch_bounds__(kBkPartThreads, (LEVEL == 2 ? 4 : 6)) bucket_p
     PartSmem<LEVEL>& sm = *reinterpret_cast<PartSmem<LEVEL>*>(smem_raw);
     const long long b = bidx();
     if (b >= a.B) return;
+    if (LEVEL == 2 && a.gate && a.gate[b] == 0u) return;
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     const uint2* tab = a.tab + (size_t)b * kBkBins;
     uint32_t coarse = 0, tile = blockIdx.x, n_in = a.N;
@@ -523,6 +525,7 @@ inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* so
     AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)(B * kCdfChunks), 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
     AGN_LAUNCH(K_SORT_CDF, st, (bucket_bounds_kernel<<<bgrid((g.nb + 256) / 256, B), 256, 0, st>>>(tab, klo, g.nb, bucket32_magic(g.nb), kBkSlotLog, B)));
     PartArgs a;
+    memset(&a, 0, sizeof(a));
     a.vals = vals; a.in = slabs1; a.in_count = cursor1; a.overflow = overflow; a.tab = tab;
     a.N = (uint32_t)N; a.nb = g.nb; a.M = bucket32_magic(g.nb); a.lb = g.lb; a.nc = g.nc; a.cap_in = g.cap1; a.tiles_in = g.tiles1; a.B = B;
     a.out = slabs1; a.cursor = cursor1; a.cap_out = g.cap1;

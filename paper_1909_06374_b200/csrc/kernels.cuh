@@ -302,9 +302,10 @@ __global__ void __launch_bounds__(256) scatter_count_kernel(const uint32_t* __re
                                                             const uint32_t* __restrict__ idx_old,
                                                             const T* __restrict__ sorted, T* __restrict__ x,
                                                             long long N, unsigned long long* __restrict__ changed,
-                                                            int B) {
+                                                            int B, const uint32_t* __restrict__ gate = nullptr) {
     const long long b = bidx();
     if (b >= B) return;
+    if (gate && gate[b] == 0u) return;          // fallback of the write-back sort: only the curves it gave up on
     const long long off = b * N;
     unsigned int local = 0;
     for (long long r = ((long long)blockIdx.x * 256 + threadIdx.x) * 4; r < N; r += (long long)gridDim.x * 1024) {

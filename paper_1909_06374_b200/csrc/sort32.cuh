@@ -253,9 +253,11 @@ __global__ void __launch_bounds__(kS32Threads, 4) sweep32_kernel(Sweep32Args a) 
 // L5 two-level: place step (the bin step is bucket_part_kernel<2> of bucket32.cuh)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) scatter_place32_kernel(const uint4* __restrict__ pairs2, float* __restrict__ x,
-                                                              uint32_t N, uint32_t* __restrict__ cursor, long long B) {
+                                                              uint32_t N, uint32_t* __restrict__ cursor, long long B,
+                                                              const uint32_t* __restrict__ gate) {
     const long long b = bidx();
     if (b >= B) return;
+    if (gate && gate[b] == 0u) return;
     if (blockIdx.x == 0) cursor[b * kRadix + threadIdx.x] = 0u;      // ready for the next iteration's bin pass
     const size_t seg = (size_t)b * N;
     float* xs = x + seg;
@@ -319,8 +321,10 @@ __global__ void __launch_bounds__(kRadix) lsd_clear_kernel(uint32_t* __restrict_
 }
 
 // vals [B][N] -> idx_out [B][N]; optionally the sorted values.  Returns the free pair buffer (for the scatter) in *spare.
+// wb (one-level distribution sort only): write-back mode, see B1Wb in bucket1.cuh.
 inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* sorted_out, long long B, long long N,
-                                 void* ws, uint2** spare, cudaStream_t st, const uint32_t** gate_out = nullptr) {
+                                 void* ws, uint2** spare, cudaStream_t st, const uint32_t** gate_out = nullptr,
+                                 const B1Wb* wb = nullptr) {
     constexpr int NP = 4;
     unsigned char* w = (unsigned char*)ws;
     uint2* pa = (uint2*)w; w += align_up((size_t)B * N * sizeof(uint2), 256);
@@ -338,7 +342,7 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
     // LSD passes below then only run for curves it gave up on
     const uint32_t* gate = nullptr;
     if (one_level) {
-        e = bucket1_sort(vals, idx_out, sorted_out, B, N, pa, w + align_up(ctl, 256), &gate, st);
+        e = bucket1_sort(vals, idx_out, sorted_out, B, N, pa, w + align_up(ctl, 256), &gate, st, wb);
         if (e != cudaSuccess) return e;
     } else if (bucket32_applicable(4, N)) {
         e = bucket32_sort(vals, idx_out, sorted_out, B, N, pa, w + align_up(ctl, 256), &gate, st);
@@ -381,17 +385,18 @@ inline cudaError_t seg_argsort32(const float* vals, uint32_t* idx_out, float* so
 // L5 two-level for fp32 (N >= 2^kTwoLevelScatterLog).  cursor: [B][256] u32, zero on entry (left zero again).
 inline cudaError_t rank_scatter_two_level32(const uint32_t* idx_new, const uint32_t* idx_old, const float* sorted, float* x,
                                             long long B, long long N, uint2* pairs, uint32_t* cursor,
-                                            unsigned long long* changed, cudaStream_t st) {
+                                            unsigned long long* changed, cudaStream_t st, const uint32_t* gate = nullptr) {
     const int shift = ilog2_u64((uint64_t)N) - kRadixBits;
     // bin step: the tile kernel of bucket32.cuh in its LEVEL 2 form (no order is needed inside a window)
     PartArgs a;
     memset(&a, 0, sizeof(a));
     a.vals = sorted; a.idx_new = idx_new; a.idx_old = idx_old; a.changed = changed;
     a.out = pairs; a.cursor = cursor; a.N = (uint32_t)N; a.lb = (uint32_t)shift; a.nc = kRadix; a.nb = kRadix;
-    a.cap_out = (uint32_t)(N >> kRadixBits); a.B = B;
-    AGN_LAUNCH(K_SCATTER_BIN, st, (bucket_part_kernel<2><<<bgrid((unsigned)(N / bk_part_tile(2)), B), kBkPartThreads, sizeof(PartSmem<2>), st>>>(a)));
-    AGN_LAUNCH(K_SCATTER_PLACE, st, (scatter_place32_kernel<<<bgrid((unsigned)(N / 2048), B), 256, 0, st>>>(
-        (const uint4*)pairs, x, (uint32_t)N, cursor, B)));
+    a.cap_out = (uint32_t)(N >> kRadixBits); a.B = B; a.gate = gate;
+    // with a gate these two launches are the fallback of the write-back sort: they exit at once for every other curve
+    AGN_LAUNCH(gate ? K_SORT_FALLBACK : K_SCATTER_BIN, st, (bucket_part_kernel<2><<<bgrid((unsigned)(N / bk_part_tile(2)), B), kBkPartThreads, sizeof(PartSmem<2>), st>>>(a)));
+    AGN_LAUNCH(gate ? K_SORT_FALLBACK : K_SCATTER_PLACE, st, (scatter_place32_kernel<<<bgrid((unsigned)(N / 2048), B), 256, 0, st>>>(
+        (const uint4*)pairs, x, (uint32_t)N, cursor, B, gate)));
     return cudaGetLastError();
 }
 

@@ -321,8 +321,9 @@ def test_e13_ties_and_zero_amplitude(ag, orc):
         assert out["changed_hist"][b, 0].item() == np.count_nonzero(pnew[b] != perm0[b])
 
 
-@pytest.mark.parametrize("N", [2 ** 18, 2 ** 21])
-@pytest.mark.parametrize("case", ["red_noise", "quantised", "all_equal", "one_outlier"])
+@pytest.mark.parametrize("N", [2 ** 18, 2 ** 22])
+@pytest.mark.parametrize("case", ["red_noise", "quantised", "all_equal", "one_outlier", "mixed", "tone64", "tone4096",
+                                  "red_plus_tone"])
 def test_long_curve_argsort_paths(ag, orc, N, case):
     """fp32 curves of N >= 2^18 go through the distribution sort (bucket32.cuh); inputs it cannot bucket (massive
     ties -> slab overflow) must fall back to the LSD passes on the device.  Either way the permutation is THE stable
@@ -339,12 +340,25 @@ def test_long_curve_argsort_paths(ag, orc, N, case):
         an[:, N // 8] = 1.0                                # period-8 tone: at most 8 distinct values, N/8 copies each
     elif case == "all_equal":
         pass                                               # zero amplitudes: x_adj == 0 everywhere
+    elif case == "tone64":
+        an[:, N // 64] = 1.0                               # 64 values x N/64 copies: crowded interpolation slots
+    elif case == "tone4096":
+        an[:, N // 4096] = 1.0                             # period 4096: (near-)ties in groups of N/4096 -> slots of
+        an[:, N // 64] = 0.5                               # more than 63 pairs (the finish kernel's big-slot path)
+    elif case == "red_plus_tone":
+        j = np.arange(1, N // 2 + 1)
+        an[:, 1:] = (1e-4 / j).astype(np.float32)          # a strong tone on weak red noise: key density far from
+        an[:, N // 256] = 1.0                              # what the sampled CDF resolves
+    elif case == "mixed":
+        j = np.arange(1, N // 2 + 1)                       # curve 0 takes the write-back sort, curve 1 (quantised) the
+        an[0, 1:] = (1.0 / j).astype(np.float32)           # gated LSD fallback and the gated plain scatter, in ONE batch
+        an[1, N // 8] = 1.0
     else:
         an[:, 0] = 1e-3                                    # constant + one huge spike bin pair -> extreme key range
         an[:, 1] = 1e30
     d = lambda a: torch.tensor(a.view(np.int32) if a.dtype == np.uint32 else a, device="cuda")
     perm = d(perm0)
-    out = ag.agnvar_e13_iterate(d(an), d(srt), perm, 1, want_hist=True, want_xadj=True)
+    out = ag.agnvar_e13_iterate(d(an), d(srt), perm, 1, want_hist=True, want_xadj=True, want_fallbacks=True)
     xadj = out["x_adj"].cpu().numpy()
     pnew, x = u32(out["perm"]), out["x"].cpu().numpy()
     for b in range(B):
@@ -354,6 +368,10 @@ def test_long_curve_argsort_paths(ag, orc, N, case):
         xs[pnew[b]] = srt[b]
         assert (x[b] == xs).all()
         assert out["changed_hist"][b, 0].item() == np.count_nonzero(pnew[b] != perm0[b])
+    if case in ("red_noise", "mixed", "quantised"):
+        fb = out["sort_fallbacks"].cpu().numpy()
+        assert fb[0] == (1 if case == "quantised" else 0)
+        assert fb[1] == (0 if case == "red_noise" else 1)
 
 
 # ---- boundary behaviour ---------------------------------------------------------------------------
