@@ -294,3 +294,17 @@ def moments(x):
     out = np.empty(4)
     lib().orc_moments(_p(x), C.c_int64(x.size), _p(out))
     return out
+
+
+# ---- NEXT-3: slice sampling (Neal 2003) -----------------------------------------
+def slice_sample(erdf, N, chains, seed, b, dtype, burn_in=50, thin=1, w=1.0, m=8, table=None):
+    """erdf: dict as for erdf_draw (kind 0 / 1), or kind 2 with `table` = un-normalised density on a uniform grid
+    over [log10 lam_min, log10 lam_max].  Returns (lambda [N] in draw order, u = log10 lambda before rounding)."""
+    lam, u = np.empty(N), np.empty(N)
+    tab = _d(table) if table is not None else None
+    G = len(tab) if tab is not None else 0
+    assert N % chains == 0
+    lib().orc_slice_sample(*_erdf_args(erdf), _p(tab) if tab is not None else None, C.c_int64(G), C.c_int64(N),
+                           C.c_int64(chains), C.c_int(burn_in), C.c_int(thin), C.c_double(w), C.c_int(m),
+                           C.c_uint64(seed), C.c_uint32(b), C.c_int(dtype), _p(lam), _p(u))
+    return lam, u

@@ -36,6 +36,12 @@
 //                                  brute force with the mask rebuilt from the (KAT-pinned) Philox words; pooled pair
 //                                  count ~ p^2 (n_sub - l) B; unbiased for a random-walk ensemble
 //   orc_moments            pinned: closed forms (two-point and uniform distributions), scipy.stats on random data
+//   orc_slice_sample       pinned: one kept draw per chain (independent draws) KS-tested against the closed-form CDF
+//                                  (delta2 = 2 delta1), erf (log-normal) and closed forms of tabulated densities
+//                                  (triangle, two boxes with a zero-density gap), for step widths from 0.02 to 50 dex
+//                                  and 1 to 64 stepping-out steps (the stationary law must not depend on them); the
+//                                  paper's ~10% / ~1.7% fractions; support; a long single chain's
+//                                  mean / variance against quadrature; prefix property of the chain layout
 //
 // Build: g++ -O2 -std=c++17 -shared -fPIC -o liboracle.so agnvar_oracle.cpp   (oracle/build.py)
 
@@ -646,6 +652,88 @@ void orc_moments(const double* x, int64_t N, double out[4]) {
     out[1] = m2;
     out[2] = m2 > 0.0 ? m3 / (m2 * std::sqrt(m2)) : 0.0;
     out[3] = m2 > 0.0 ? m4 / (m2 * m2) - 3.0 : 0.0;
+}
+
+// ----------------------------------------------------------------------------------------------
+// NEXT-3. Slice sampling (Neal 2003, Ann. Statist. 31, 705), the paper's sampler for the random draw
+// ("for the random draw step we apply slice sampling (Neal 2003) from a normalised ERDF ...
+// additional functional forms can be added if needed"; PAPER.md:164 names it as what limits the running time).
+// The paper gives no detail beyond the citation; this is Neal's univariate update with the "stepping out"
+// procedure (his Fig. 3) followed by the "shrinkage" procedure (his Fig. 5), applied to u = log10(lambda), whose
+// density g(u) is proportional to xi(10^u) on [log10 lam_min, log10 lam_max] and 0 outside (reading Q10).
+//
+// density kinds: 0 / 1 = Eq. 1 / Eq. 2 (erdf_xi above); 2 = an arbitrary un-normalised density given as a table
+// gtab[0..G-1] >= 0 on the uniform grid u_k = u_lo + k D, linearly interpolated ("additional functional forms").
+//
+// Reading Q24 for what the paper leaves open:
+//   chains   `chains` independent Markov chains per curve; chain c starts at x = u_lo + U (u_hi - u_lo), makes
+//            burn_in + (N / chains) * thin updates and keeps every thin-th state after the burn-in; the j-th kept
+//            state of chain c is sample n = j * chains + c (N must be a multiple of chains).
+//   uniforms Philox stream tag 5, counter (call, chain c, curve b, 5): the chain's uniform number q is u53 of words
+//            (0,1) of call q >> 1 if q is even, of words (2,3) if odd; a chain uses its uniforms in order.
+//   update   y = g(x) U;  U: L = x - w U, R = L + w;  V: J = floor(m V), K = (m - 1) - J;
+//            while J > 0 and y < g(L): L -= w, J -= 1;   while K > 0 and y < g(R): R += w, K -= 1;
+//            repeat: U: x1 = L + U (R - L); accept if y < g(x1), else L = x1 if x1 < x, else R = x1.
+//            (At most 1000 shrinkage draws, then the chain stays at x: only reachable where g = 0 around x.)
+//   output   lambda = 10^x rounded to the output type.
+// Plain arithmetic, one rounding per operation, in the order written (built with -ffp-contract=off).
+// ----------------------------------------------------------------------------------------------
+static double slice_density(int kind, double u, double lam_star, double d1, double d2, double mu, double sigma,
+                            double u_lo, double u_hi, const double* gtab, int64_t G) {
+    if (u < u_lo || u > u_hi) return 0.0;
+    if (kind == 2) {
+        double D = (u_hi - u_lo) / (double)(G - 1);
+        double t = (u - u_lo) / D;
+        int64_t k = (int64_t)t;
+        if (k > G - 2) k = G - 2;
+        double f = t - (double)k;
+        return gtab[k] + f * (gtab[k + 1] - gtab[k]);
+    }
+    return erdf_xi(kind, u, lam_star, d1, d2, mu, sigma);
+}
+
+void orc_slice_sample(int kind, double lam_star, double d1, double d2, double mu, double sigma, double lam_min,
+                      double lam_max, const double* gtab, int64_t G, int64_t N, int64_t chains, int burn_in, int thin,
+                      double w, int m, uint64_t seed, uint32_t b, int dtype, double* lam, double* u_out) {
+    const double u_lo = std::log10(lam_min), u_hi = std::log10(lam_max);
+    const int64_t n_keep = N / chains;
+    auto g = [&](double u) { return slice_density(kind, u, lam_star, d1, d2, mu, sigma, u_lo, u_hi, gtab, G); };
+    for (int64_t c = 0; c < chains; ++c) {
+        uint64_t q = 0;                                   // uniforms used by this chain so far
+        auto next_uniform = [&]() {
+            uint32_t wd[4];
+            orc_philox_stream(seed, ((uint64_t)c << 32) | (q >> 1), b, 5u, wd);
+            double U = (q & 1) ? orc_u53(wd[2], wd[3]) : orc_u53(wd[0], wd[1]);
+            ++q;
+            return U;
+        };
+        double x = u_lo + next_uniform() * (u_hi - u_lo);
+        const int64_t total = (int64_t)burn_in + n_keep * (int64_t)thin;
+        for (int64_t t = 1; t <= total; ++t) {
+            // the slice
+            double y = g(x) * next_uniform();
+            // stepping out (Neal 2003, Fig. 3)
+            double L = x - w * next_uniform();
+            double R = L + w;
+            int J = (int)std::floor((double)m * next_uniform());
+            int K = (m - 1) - J;
+            while (J > 0 && y < g(L)) { L -= w; --J; }
+            while (K > 0 && y < g(R)) { R += w; --K; }
+            // shrinkage (Neal 2003, Fig. 5)
+            for (int it = 0; it < 1000; ++it) {
+                double x1 = L + next_uniform() * (R - L);
+                if (y < g(x1)) { x = x1; break; }
+                if (x1 < x) L = x1; else R = x1;
+            }
+            if (t > burn_in && (t - burn_in) % thin == 0) {
+                int64_t n = ((t - burn_in) / thin - 1) * chains + c;
+                double l = std::pow(10.0, x);
+                if (dtype == 0) l = (double)(float)l;
+                lam[n] = l;
+                if (u_out) u_out[n] = x;
+            }
+        }
+    }
 }
 
 }  // extern "C"
