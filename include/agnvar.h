@@ -19,7 +19,8 @@
  *   - dtype selects the arithmetic AND storage type of series, spectra and sort keys (float or
  *     double).  PSD values, the ERDF table and the inverse-CDF arithmetic are always fp64.
  *   - Random numbers: Philox4x32-10, key = (seed lo, seed hi), counter = (i lo, i hi, curve b, tag);
- *     tag 0 = TK normals (i = frequency index j), tag 1 = ERDF uniforms (i = n >> 1).  A curve's
+ *     tag 0 = TK normals (i = frequency index j), tag 1 = ERDF uniforms (i = n >> 1), tag 3 / 4 = sub-sample offsets /
+ *     masks (agnvar_ensemble_sf), tag 5 = slice-sampler uniforms (agnvar_slice_sample_sorted).  A curve's
  *     numbers depend on (seed, b0 + row) only, never on B or on the launch shape (b0 = `curve0`).
  */
 #ifndef AGNVAR_H
@@ -41,7 +42,7 @@ typedef enum {
 } agnvar_status;
 
 typedef enum { AGNVAR_F32 = 0, AGNVAR_F64 = 1 } agnvar_dtype;
-typedef enum { AGNVAR_ERDF_BPL = 0, AGNVAR_ERDF_LOGNORMAL = 1 } agnvar_erdf_kind;
+typedef enum { AGNVAR_ERDF_BPL = 0, AGNVAR_ERDF_LOGNORMAL = 1, AGNVAR_ERDF_TABLE = 2 /* agnvar_slice_sample_sorted only */ } agnvar_erdf_kind;
 typedef enum {
     AGNVAR_OP_ERDF_SAMPLE_SORTED = 1,
     AGNVAR_OP_TK_GENERATE = 2,
@@ -49,7 +50,8 @@ typedef enum {
     AGNVAR_OP_PERIODOGRAM = 4,
     AGNVAR_OP_STRUCTURE_FUNCTION = 5,
     AGNVAR_OP_DELTA_M_PROB = 6,
-    AGNVAR_OP_ENSEMBLE_SF = 7
+    AGNVAR_OP_ENSEMBLE_SF = 7,
+    AGNVAR_OP_SLICE_SAMPLE_SORTED = 8
 } agnvar_op;
 
 /* Eq. 3: PSD(f) = A [ (f/f_b)^alpha_low + (f/f_b)^alpha_high ]^-1.
@@ -74,7 +76,7 @@ typedef struct {
 /* Bytes of scratch the given op needs.  `oversample` matters for AGNVAR_OP_TK_GENERATE only
  * (pass 1 otherwise); `aux` = grid_points for ERDF_SAMPLE_SORTED, nbins for PERIODOGRAM, 1 for E13_ITERATE
  * with the delta_i rule / history (see agnvar_e13_opts), nlags for STRUCTURE_FUNCTION, DELTA_M_PROB and
- * ENSEMBLE_SF (pass n_sub as N for ENSEMBLE_SF), else 0.
+ * ENSEMBLE_SF (pass n_sub as N for ENSEMBLE_SF), else 0 (SLICE_SAMPLE_SORTED: 0).
  * Returns 0 for invalid arguments. */
 size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int oversample, int64_t aux);
 
@@ -99,6 +101,39 @@ int agnvar_psd_bpl(const double* d_f, int64_t n, const agnvar_psd* h_p, double* 
 int agnvar_erdf_sample_sorted(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t B, int64_t N, int dtype,
                               uint64_t seed, uint32_t curve0, int grid_points, void* d_sorted,
                               uint32_t* d_perm0, void* d_draw, void* d_ws, size_t ws_bytes, void* stream);
+
+/* S1 by the paper's own sampler (NEXT-3) -- slice sampling (Neal 2003, Ann. Statist. 31, 705) from the ERDF or from
+ * any un-normalised density ("for the random draw step we apply slice sampling (Neal 2003) from a
+ * normalised ERDF ... additional functional forms can be added if needed"; the step that limits the
+ * paper's running time), then the same stable sort as agnvar_erdf_sample_sorted, same outputs.  Same distribution as
+ * the inverse-CDF sampler, different samples.  Reading Q24 for what the paper leaves open:
+ *   state     u = log10(lambda); density g(u) ~ xi(10^u) on [log10 lam_min, log10 lam_max], 0 outside (Q10); kind
+ *             AGNVAR_ERDF_TABLE: g = linear interpolation of d_density (density_points >= 2 values >= 0 on the
+ *             uniform grid over that interval; one row per h_erdf entry; lam_star .. sigma_log10 ignored)
+ *   chains    `chains` independent Markov chains per curve (N a multiple of chains); chain c starts at
+ *             u_lo + U (u_hi - u_lo), makes burn_in + (N / chains) thin updates and keeps every thin-th state after
+ *             the burn-in; kept state j of chain c is draw n = j * chains + c
+ *   uniforms  Philox tag 5, counter (call, chain c, curve b, 5): uniform number q of a chain = words (0,1) of call
+ *             q >> 1 if q is even, words (2,3) if odd
+ *   update    y = g(x) U;  stepping out (Neal's Fig. 3): U: L = x - width U, R = L + width; V: J = floor(max_steps V),
+ *             K = max_steps - 1 - J; while J > 0 and y < g(L): L -= width, J -= 1; while K > 0 and y < g(R):
+ *             R += width, K -= 1;  shrinkage (Fig. 5): U: x1 = L + U (R - L); accept if y < g(x1), else L = x1 if
+ *             x1 < x, else R = x1 (at most 1000 draws, then the chain stays: only where g = 0 around x)
+ *   output    lambda = 10^x rounded to dtype; d_u_dbg (or NULL): [B][N] fp64, the states x in draw order
+ * All arithmetic fp64, one rounding per written operation (no FMA contraction).
+ * EINVAL: as agnvar_erdf_sample_sorted, plus NULL h_opts, chains < 1 or not a divisor of N or > 2^32, burn_in < 0,
+ * thin < 1, max_steps < 1, width <= 0 or non-finite, kind TABLE without d_density or with density_points < 2. */
+typedef struct {
+    int64_t chains;
+    int32_t burn_in, thin, max_steps, reserved;
+    double width;                 /* w, in dex */
+    const double* d_density;      /* kind TABLE: [n_erdf][density_points] fp64, else NULL */
+    int64_t density_points;
+    double* d_u_dbg;
+} agnvar_slice_opts;
+int agnvar_slice_sample_sorted(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t B, int64_t N, int dtype,
+                               uint64_t seed, uint32_t curve0, const agnvar_slice_opts* h_opts, void* d_sorted,
+                               uint32_t* d_perm0, void* d_draw, void* d_ws, size_t ws_bytes, void* stream);
 
 /* S1 (table only) -- the normalised cumulative table C of agnvar_erdf_sample_sorted (O4), for checking the
  * sampler's premise against a reference: d_out [n_erdf][grid_points] fp64, C_0 = 0, C_{G-1} = 1.

@@ -15,13 +15,14 @@ from . import _build
 AGNVAR_F32, AGNVAR_F64 = 0, 1
 AGNVAR_ERDF_BPL, AGNVAR_ERDF_LOGNORMAL = 0, 1
 (OP_ERDF_SAMPLE_SORTED, OP_TK_GENERATE, OP_E13_ITERATE, OP_PERIODOGRAM, OP_STRUCTURE_FUNCTION, OP_DELTA_M_PROB,
- OP_ENSEMBLE_SF) = 1, 2, 3, 4, 5, 6, 7
+ OP_ENSEMBLE_SF, OP_SLICE_SAMPLE_SORTED) = 1, 2, 3, 4, 5, 6, 7, 8
 
 EXPORTS = (
     "agnvar_workspace_bytes", "agnvar_psd_bpl", "agnvar_erdf_sample_sorted", "agnvar_erdf_table", "agnvar_tk_generate",
     "agnvar_e13_iterate", "agnvar_periodogram", "agnvar_philox_u32", "agnvar_strerror", "agnvar_version",
     "agnvar_launch_count", "agnvar_trace_begin", "agnvar_trace_end", "agnvar_kernel_name",
     "agnvar_structure_function", "agnvar_delta_m_prob", "agnvar_ensemble_sf", "agnvar_moments",
+    "agnvar_slice_sample_sorted",
 )
 
 
@@ -44,6 +45,12 @@ class agnvar_erdf(C.Structure):
 class agnvar_e13_opts(C.Structure):
     _fields_ = [("delta_threshold", C.c_double), ("d_delta_hist", C.c_void_p), ("d_sort_fallbacks", C.c_void_p),
                 ("check_every", C.c_int32), ("reserved", C.c_int32)]
+
+
+class agnvar_slice_opts(C.Structure):
+    _fields_ = [("chains", C.c_int64), ("burn_in", C.c_int32), ("thin", C.c_int32), ("max_steps", C.c_int32),
+                ("reserved", C.c_int32), ("width", C.c_double), ("d_density", C.c_void_p),
+                ("density_points", C.c_int64), ("d_u_dbg", C.c_void_p)]
 
 
 _lib = None
@@ -77,6 +84,9 @@ def lib():
     L.agnvar_e13_iterate.restype = i32
     L.agnvar_e13_iterate.argtypes = [i64, i64, i32, vp, vp, vp, vp, i32, vp, vp, vp, C.POINTER(agnvar_e13_opts), vp, sz,
                                      vp]
+    L.agnvar_slice_sample_sorted.restype = i32
+    L.agnvar_slice_sample_sorted.argtypes = [C.POINTER(agnvar_erdf), i64, i64, i64, i32, u64, u32,
+                                             C.POINTER(agnvar_slice_opts), vp, vp, vp, vp, sz, vp]
     L.agnvar_erdf_table.restype = i32
     L.agnvar_erdf_table.argtypes = [C.POINTER(agnvar_erdf), i64, i32, vp, vp]
     L.agnvar_periodogram.restype = i32
@@ -267,6 +277,31 @@ def agnvar_erdf_sample_sorted(erdf, B, N, dtype, seed, curve0=0, grid_points=409
                                                _ptr(perm0), _ptr(draw), _ptr(ws), ws.numel(), _stream()),
                "agnvar_erdf_sample_sorted")
     return srt, perm0, draw
+
+
+def agnvar_slice_sample_sorted(erdf, B, N, dtype, seed, chains, curve0=0, burn_in=50, thin=1, width=1.0, max_steps=8,
+                               density=None, want_perm0=True, want_draw=False, want_u=False, device="cuda"):
+    """NEXT-3: S1 by slice sampling (Neal 2003).  erdf kind 2 takes `density` [n_erdf][G] fp64 (device).
+    Returns (sorted [B][N], perm0 | None, draw | None, u [B][N] fp64 | None)."""
+    code, tdt = _dt(dtype)
+    arr, n = _erdf_array(erdf)
+    with _on(device):
+        srt = torch.empty((B, N), dtype=tdt, device=device)
+        perm0 = torch.empty((B, N), dtype=torch.int32, device=device) if want_perm0 else None
+        draw = torch.empty((B, N), dtype=tdt, device=device) if want_draw else None
+        u = torch.empty((B, N), dtype=torch.float64, device=device) if want_u else None
+        if density is not None:
+            assert density.dtype == torch.float64 and density.is_contiguous() and density.dim() == 2
+        opts = agnvar_slice_opts(int(chains), int(burn_in), int(thin), int(max_steps), 0, float(width),
+                                 density.data_ptr() if density is not None else None,
+                                 int(density.shape[1]) if density is not None else 0,
+                                 u.data_ptr() if u is not None else None)
+        nb = workspace_bytes(OP_SLICE_SAMPLE_SORTED, B, N, code, 1, 0)
+        ws = workspace(nb, srt.device)
+        _check(lib().agnvar_slice_sample_sorted(arr, n, B, N, code, int(seed), int(curve0), C.byref(opts), _ptr(srt),
+                                                _ptr(perm0), _ptr(draw), _ptr(ws), ws.numel(), _stream()),
+               "agnvar_slice_sample_sorted")
+    return srt, perm0, draw, u
 
 
 def agnvar_tk_generate(psd, B, N, dt, oversample, dtype, seed, curve0=0, want_xnorm=True, want_anorm=True,

@@ -11,6 +11,7 @@
 #include "sort32.cuh"
 #include "sf.cuh"
 #include "onchip.cuh"
+#include "slice.cuh"
 
 #include <cmath>
 #include <cstring>
@@ -391,7 +392,8 @@ int tk_impl(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_t N, double
 // ---- ERDF ----------------------------------------------------------------------------------------------
 template <typename T>
 int erdf_impl(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t B, int64_t N, uint64_t seed, uint32_t curve0,
-              int G, void* d_sorted, uint32_t* d_perm0, void* d_draw, void* d_ws, size_t ws_bytes, cudaStream_t st) {
+              int G, void* d_sorted, uint32_t* d_perm0, void* d_draw, void* d_ws, size_t ws_bytes, cudaStream_t st,
+              const agnvar_slice_opts* slice = nullptr) {
     if (ws_bytes < ws_erdf<T>(B, N, G) || !d_ws || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
     if (ensure_attrs<T>() != cudaSuccess) return AGNVAR_ECUDA;
     Carver c(d_ws);
@@ -408,9 +410,18 @@ int erdf_impl(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t B, int64_t N, u
     }
     if (cudaMemcpyAsync(erdf, he.data(), (size_t)n_erdf * sizeof(ErdfDev), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return AGNVAR_ECUDA;
-    AGN_LAUNCH(K_ERDF_TABLE, st, (erdf_table_kernel<<<(unsigned)n_erdf, 256, 0, st>>>(erdf, G, Ctab)));
-    AGN_LAUNCH(K_ERDF_SAMPLE, st, (erdf_sample_kernel<T><<<bgrid(cdiv(N / 2, 256), B), 256, 0, st>>>(erdf, n_erdf == 1 ? 0 : 1, Ctab, G, N, seed,
-                                                                      curve0, draw, (int)B)));
+    if (slice) {
+        // NEXT-3: the paper's sampler (slice.cuh), one thread per chain
+        SliceArgs sa;
+        sa.erdf = erdf; sa.per_curve = n_erdf == 1 ? 0 : 1; sa.gtab = slice->d_density; sa.G = slice->density_points;
+        sa.N = N; sa.chains = slice->chains; sa.burn_in = slice->burn_in; sa.thin = slice->thin; sa.m = slice->max_steps;
+        sa.w = slice->width; sa.seed = seed; sa.curve0 = curve0; sa.B = (int)B;
+        AGN_LAUNCH(K_SLICE_SAMPLE, st, (slice_sample_kernel<T><<<bgrid(cdiv(slice->chains, 128), B), 128, 0, st>>>(sa, draw, slice->d_u_dbg)));
+    } else {
+        AGN_LAUNCH(K_ERDF_TABLE, st, (erdf_table_kernel<<<(unsigned)n_erdf, 256, 0, st>>>(erdf, G, Ctab)));
+        AGN_LAUNCH(K_ERDF_SAMPLE, st, (erdf_sample_kernel<T><<<bgrid(cdiv(N / 2, 256), B), 256, 0, st>>>(erdf, n_erdf == 1 ? 0 : 1, Ctab, G, N, seed,
+                                                                          curve0, draw, (int)B)));
+    }
     // stable ascending sort carrying the draw index; perm0 is needed internally even if the caller
     // does not want it -> use the tail of the sort workspace? no: sort straight into d_perm0 or a scratch
     uint32_t* perm = d_perm0;
@@ -615,6 +626,8 @@ size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int overs
             if (aux < 2 || aux > 65536) return 0;
             // + a scratch permutation for callers that pass d_perm0 = NULL
             return (f32 ? ws_erdf<float>(B, N, aux) : ws_erdf<double>(B, N, aux)) + align_up((size_t)B * N * 4, 256);
+        case AGNVAR_OP_SLICE_SAMPLE_SORTED:
+            return (f32 ? ws_erdf<float>(B, N, 2) : ws_erdf<double>(B, N, 2)) + align_up((size_t)B * N * 4, 256);
         case AGNVAR_OP_PERIODOGRAM:
             if (aux < 0 || aux > 4096) return 0;
             return f32 ? ws_pgram<float>(B, N, aux) : ws_pgram<double>(B, N, aux);
@@ -652,12 +665,14 @@ int agnvar_psd_bpl(const double* d_f, int64_t n, const agnvar_psd* h_p, double* 
     return cuda_status(cudaGetLastError());
 }
 
-static bool valid_erdf(const agnvar_erdf* h_erdf, int64_t n_erdf) {
+static bool valid_erdf(const agnvar_erdf* h_erdf, int64_t n_erdf, bool allow_table = false) {
     for (int64_t i = 0; i < n_erdf; ++i) {
         const agnvar_erdf& e = h_erdf[i];
-        if (e.kind != AGNVAR_ERDF_BPL && e.kind != AGNVAR_ERDF_LOGNORMAL) return false;
+        if (e.kind != AGNVAR_ERDF_BPL && e.kind != AGNVAR_ERDF_LOGNORMAL && !(allow_table && e.kind == AGNVAR_ERDF_TABLE))
+            return false;
         if (!std::isfinite(e.lam_min) || !std::isfinite(e.lam_max) || !(e.lam_min > 0.0) || !(e.lam_min < e.lam_max))
             return false;
+        if (e.kind == AGNVAR_ERDF_TABLE) continue;
         if (e.kind == AGNVAR_ERDF_BPL) {
             if (!std::isfinite(e.lam_star) || !(e.lam_star > 0.0) || !std::isfinite(e.delta1) || !std::isfinite(e.delta2))
                 return false;
@@ -702,6 +717,28 @@ int agnvar_erdf_sample_sorted(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t
                                 need - tail, (cudaStream_t)stream);
     return erdf_impl<double>(h_erdf, n_erdf, B, N, seed, curve0, grid_points, d_sorted, perm, d_draw, d_ws, need - tail,
                              (cudaStream_t)stream);
+}
+
+int agnvar_slice_sample_sorted(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t B, int64_t N, int dtype,
+                               uint64_t seed, uint32_t curve0, const agnvar_slice_opts* h_opts, void* d_sorted,
+                               uint32_t* d_perm0, void* d_draw, void* d_ws, size_t ws_bytes, void* stream) {
+    if (!valid_BN(B, N) || !valid_dtype(dtype) || !h_erdf || !d_sorted || !h_opts) return AGNVAR_EINVAL;
+    if (!(n_erdf == 1 || n_erdf == B) || !valid_erdf(h_erdf, n_erdf, true)) return AGNVAR_EINVAL;
+    const agnvar_slice_opts& o = *h_opts;
+    if (o.chains < 1 || o.chains > ((int64_t)1 << 32) || N % o.chains != 0 || o.burn_in < 0 || o.thin < 1 || o.max_steps < 1 ||
+        !(o.width > 0.0) || !std::isfinite(o.width))
+        return AGNVAR_EINVAL;
+    for (int64_t i = 0; i < n_erdf; ++i)
+        if (h_erdf[i].kind == AGNVAR_ERDF_TABLE && (!o.d_density || o.density_points < 2)) return AGNVAR_EINVAL;
+    size_t need = agnvar_workspace_bytes(AGNVAR_OP_SLICE_SAMPLE_SORTED, B, N, dtype, 1, 0);
+    if (!d_ws || ws_bytes < need || !aligned(d_ws, 256)) return AGNVAR_EWORKSPACE;
+    const size_t tail = align_up((size_t)B * N * 4, 256);
+    uint32_t* perm = d_perm0 ? d_perm0 : (uint32_t*)((unsigned char*)d_ws + (need - tail));
+    if (dtype == AGNVAR_F32)
+        return erdf_impl<float>(h_erdf, n_erdf, B, N, seed, curve0, 2, d_sorted, perm, d_draw, d_ws, need - tail,
+                                (cudaStream_t)stream, h_opts);
+    return erdf_impl<double>(h_erdf, n_erdf, B, N, seed, curve0, 2, d_sorted, perm, d_draw, d_ws, need - tail,
+                             (cudaStream_t)stream, h_opts);
 }
 
 int agnvar_tk_generate(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_t N, double dt, int oversample,

@@ -149,7 +149,7 @@ inline DevCache& dev_cache() {
 enum KernelId {
     K_FFT_STRIDED = 0, K_FFT_CONTIG, K_REPLACE, K_SORT_CTA, K_SORT_HIST, K_SORT_SWEEP, K_SCATTER, K_ITER_POST,
     K_PERM_ANORM, K_TK_FILL, K_TK_COMBINE, K_UNTANGLE_OUT, K_PSD, K_ERDF_TABLE, K_ERDF_SAMPLE, K_PGRAM, K_TABLES,
-    K_COPY, K_PHILOX, K_SCATTER_BIN, K_SCATTER_PLACE, K_FFT_COL, K_FFT_MID, K_SORT_CDF, K_SORT_PART0, K_SORT_BUCKET, K_DELTA, K_SORT_PART1, K_SORT_PART_ONE, K_E13_ONCHIP, K_SF, K_SORT_FALLBACK, K_SORT_PART_ONE_WB, K_SORT_BUCKET_WB, K_GATHER_BACK, K_NIDS
+    K_COPY, K_PHILOX, K_SCATTER_BIN, K_SCATTER_PLACE, K_FFT_COL, K_FFT_MID, K_SORT_CDF, K_SORT_PART0, K_SORT_BUCKET, K_DELTA, K_SORT_PART1, K_SORT_PART_ONE, K_E13_ONCHIP, K_SF, K_SORT_FALLBACK, K_SORT_PART_ONE_WB, K_SORT_BUCKET_WB, K_GATHER_BACK, K_SLICE_SAMPLE, K_NIDS
 };
 static const char* const kKernelNames[K_NIDS] = {
     "fft_pass_strided", "fft_pass_contiguous", "amplitude_replace", "cta_argsort", "sort_digit_hist",
@@ -157,7 +157,7 @@ static const char* const kKernelNames[K_NIDS] = {
     "untangle_out", "psd", "erdf_table", "erdf_sample", "periodogram_scale_bin", "twiddle_tables", "copy", "philox",
     "scatter_bin", "scatter_place", "fft_columns", "fft_mid_fused", "sort_cdf_tables", "sort_part_level0",
     "sort_bucket_finish", "delta_rms", "sort_part_level1", "sort_part_onelevel", "e13_onchip_loop", "structure_function", "sort_lsd_fallback_gated",
-    "sort_part_onelevel_rec", "sort_finish_writeback", "scatter_gather_back"};
+    "sort_part_onelevel_rec", "sort_finish_writeback", "scatter_gather_back", "slice_sample"};
 
 struct TraceRec { int id; cudaEvent_t e0, e1; };
 struct TraceState {

@@ -565,3 +565,66 @@ def test_moments_of_tk_series(ag, orc, dtype):
         ref = orc.moments(xh[b])
         assert got[b][0] == pytest.approx(ref[0], rel=1e-9, abs=1e-12 * np.sqrt(ref[1]))
         assert np.allclose(got[b][1:], ref[1:], rtol=1e-10, atol=1e-12)
+
+
+# ---- NEXT-3: slice sampling (Neal 2003) -----------------------------------------------
+SLICE_CASES = [
+    ("bpl", BPL, None, dict(chains=64, burn_in=20, thin=1, width=1.0, max_steps=8)),
+    ("lognormal", LOGN, None, dict(chains=256, burn_in=5, thin=3, width=0.3, max_steps=4)),
+    ("bpl_nostepout", BPL, None, dict(chains=32, burn_in=0, thin=1, width=50.0, max_steps=1)),
+    ("table_gap", dict(kind=2, lam_min=1e-3, lam_max=10.0), "gap", dict(chains=128, burn_in=10, thin=1, width=6.0, max_steps=2)),
+    ("table_ramp", dict(kind=2, lam_min=1e-3, lam_max=10.0), "ramp", dict(chains=128, burn_in=10, thin=2, width=0.7, max_steps=4)),
+]
+
+
+def _slice_table(which):
+    if which is None:
+        return None
+    uu = np.linspace(-3, 1, 33)
+    if which == "ramp":
+        return np.linspace(0.0, 4.0, 33)
+    g = np.zeros(33)
+    g[(uu >= -3) & (uu <= -2)] = 1.0
+    g[(uu >= 0) & (uu <= 1)] = 3.0
+    return g
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("name,erdf,table,opt", SLICE_CASES, ids=[c[0] for c in SLICE_CASES])
+def test_slice_sample_sorted(ag, orc, dtype, name, erdf, table, opt):
+    """Every chain follows the oracle's chain: the states u (fp64) agree to rounding of pow / exp in the density
+    (they are bit-identical unless an accept decision sits within that rounding), lambda = 10^u to 2 ulp of fp64 /
+    1 ulp of fp32, and the sorted draw + permutation are the stable argsort of the GPU's own draw."""
+    B, N, seed, curve0 = 3, 2048, 21, 5
+    tab = _slice_table(table)
+    dens = torch.tensor(np.tile(tab, (1, 1)), device="cuda") if tab is not None else None
+    srt, perm0, draw, u = ag.agnvar_slice_sample_sorted(erdf, B, N, dtype, seed, curve0=curve0, density=dens,
+                                                        want_draw=True, want_u=True, **opt)
+    draw_h, u_h, srt_h, perm_h = draw.cpu().numpy(), u.cpu().numpy(), srt.cpu().numpy(), u32(perm0)
+    n_exact = 0
+    for b in range(B):
+        lam_ref, u_ref = orc.slice_sample(erdf, N, opt["chains"], seed, curve0 + b, 1 if dtype == "f64" else 0,
+                                          burn_in=opt["burn_in"], thin=opt["thin"], w=opt["width"], m=opt["max_steps"],
+                                          table=tab)
+        assert np.abs(u_h[b] - u_ref).max() <= 1e-12
+        n_exact += int((u_h[b] == u_ref).sum())
+        rel = np.abs(draw_h[b].astype(np.float64) - lam_ref) / lam_ref
+        assert rel.max() <= (1e-14 if dtype == "f64" else 1.2e-7)
+        order = orc.stable_argsort(draw_h[b].astype(np.float64))
+        assert (perm_h[b] == order).all()
+        assert (srt_h[b] == draw_h[b][order]).all()
+    if tab is not None:
+        assert n_exact == B * N          # tabulated densities: the same roundings on both sides, bit-identical chains
+    print(f"slice {name} {dtype}: {n_exact}/{B * N} states bit-identical")
+
+
+def test_slice_sample_validation(ag):
+    import paper_1909_06374_b200.binding as bd
+    for kw in (dict(chains=3), dict(chains=0), dict(chains=64, thin=0), dict(chains=64, width=0.0),
+               dict(chains=64, max_steps=0), dict(chains=64, burn_in=-1)):
+        with pytest.raises(bd.AgnvarError):
+            ag.agnvar_slice_sample_sorted(BPL, 1, 1024, "f32", 1, **kw)
+    with pytest.raises(bd.AgnvarError):        # a tabulated density without its table
+        ag.agnvar_slice_sample_sorted(dict(kind=2, lam_min=1e-3, lam_max=1.0), 1, 1024, "f32", 1, chains=64)
+    with pytest.raises(bd.AgnvarError):        # the inverse-CDF sampler does not take tables
+        ag.agnvar_erdf_sample_sorted(dict(kind=2, lam_min=1e-3, lam_max=1.0), 1, 1024, "f32", 1)
