@@ -181,21 +181,20 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
     uint32_t* pd = (uint32_t*)((unsigned char*)sort_ws + 2 * align_up((size_t)B * N * sizeof(T), 256));
     const T* sorted = (const T*)d_sorted;
 
-    // short fp32 curves: the whole loop inside one CTA per curve (onchip.cuh); per-curve early exit at changed = 0.
+    // short curves (fp32 to 2^14, fp64 to 2^13): the whole loop inside one CTA per curve (onchip.cuh); per-curve early exit
+    // at changed = 0.
     // (The delta_i rule keeps the generic path: it needs x_sim,k and x_sim,k+1 side by side.)
-    if constexpr (sizeof(T) == 4) {
-        if (onchip_applicable(sizeof(T), N) && !dmode) {
-            AGN_LAUNCH(K_TABLES, st, (tw_init_kernel<T><<<(1 << kLogTw) / 256, 256, 0, st>>>(tables, 1 << kLogTw, kLogTw)));
-            CK(cudaMemsetAsync(counters, 0, sizeof(unsigned int), st));
-            if (d_changed_hist) CK(cudaMemsetAsync(d_changed_hist, 0, (size_t)B * max_iter * sizeof(int64_t), st));
-            if (opt.d_sort_fallbacks) CK(cudaMemsetAsync(opt.d_sort_fallbacks, 0, (size_t)B * sizeof(int32_t), st));
-            OnchipArgs oa;
-            oa.anorm = (const float*)d_anorm; oa.sorted = (const float*)d_sorted; oa.perm = d_perm; oa.x = (float*)d_x;
-            oa.xadj_dbg = (float*)d_xadj_dbg; oa.iters_used = d_iters_used; oa.hist = (long long*)d_changed_hist;
-            oa.tw14 = (const float2*)tables; oa.ticket = counters; oa.max_iter = max_iter; oa.B = B;
-            if (onchip_run(ilog2_u64((uint64_t)N), oa, st) != cudaSuccess) return AGNVAR_ECUDA;
-            return cuda_status(cudaGetLastError());
-        }
+    if (onchip_applicable(sizeof(T), N) && !dmode) {
+        AGN_LAUNCH(K_TABLES, st, (tw_init_kernel<T><<<(1 << kLogTw) / 256, 256, 0, st>>>(tables, 1 << kLogTw, kLogTw)));
+        CK(cudaMemsetAsync(counters, 0, sizeof(unsigned int), st));
+        if (d_changed_hist) CK(cudaMemsetAsync(d_changed_hist, 0, (size_t)B * max_iter * sizeof(int64_t), st));
+        if (opt.d_sort_fallbacks) CK(cudaMemsetAsync(opt.d_sort_fallbacks, 0, (size_t)B * sizeof(int32_t), st));
+        OnchipArgs<T> oa;
+        oa.anorm = (const T*)d_anorm; oa.sorted = (const T*)d_sorted; oa.perm = d_perm; oa.x = (T*)d_x;
+        oa.xadj_dbg = (T*)d_xadj_dbg; oa.iters_used = d_iters_used; oa.hist = (long long*)d_changed_hist;
+        oa.tw14 = (const C*)tables; oa.ticket = counters; oa.max_iter = max_iter; oa.B = B;
+        if (onchip_run<T>(ilog2_u64((uint64_t)N), oa, st) != cudaSuccess) return AGNVAR_ECUDA;
+        return cuda_status(cudaGetLastError());
     }
     // long fp32 curves: column sub-passes in registers + fused mid kernel (fft2.cuh); otherwise the generic passes
     const bool use2 = fft2_applicable(sizeof(T), logL);

@@ -1,7 +1,8 @@
-// onchip.cuh -- the whole E13 loop (L1-L6) of one short fp32 light curve inside ONE CTA (256 <= N <= 2^14):
-// x_sim, the spectrum, the sort's (key, index) pairs, the slot counters and the previous permutation all live in shared
-// memory (12 N bytes: 12 KB at N = 1024, 192 KB at N = 2^14); HBM sees perm0 and the result once per call, and per
-// iteration only A_norm (2 B per sample) and sorted[] (4 B per sample), both re-read through L1/L2.  A curve leaves the
+// onchip.cuh -- the whole E13 loop (L1-L6) of one short light curve inside ONE CTA (fp32: 256 <= N <= 2^14; fp64:
+// 256 <= N <= 2^13): x_sim, the spectrum, the sort's (key, index) pairs, the slot counters and the previous permutation
+// all live in shared memory (fp32: 12 N bytes, 12 KB at N = 1024, 192 KB at N = 2^14; fp64: 20 N bytes, 80 KB at
+// N = 4096); HBM sees perm0 and the result once per call, and per iteration only A_norm (half a value per sample) and
+// sorted[] (one value per sample), both re-read through L1/L2.  A curve leaves the
 // loop at its own first k with changed = 0 (L6 decided on chip; no other curve waits for it), CTAs take curves from a
 // ticket counter.  This is SURVEY section 7 steps 4-5 / 8(d): "one curve per CTA: on-chip loop".
 //
@@ -24,28 +25,46 @@
 
 namespace agn {
 
-template <int LOGN> struct OnchipCfg {
+// (key, time index) of the in-CTA sort: fp32 packs both into one 64-bit word; fp64 keys are 64 bits wide themselves
+template <typename T> struct OcPair;
+template <> struct OcPair<float> {
+    typedef unsigned long long type;
+    static __device__ __forceinline__ type make(float v, uint32_t idx) { return ((unsigned long long)key_of(v) << 32) | idx; }
+    static __device__ __forceinline__ bool less(const type& a, const type& b) { return a < b; }
+    static __device__ __forceinline__ uint32_t idx(const type& a) { return (uint32_t)a; }
+    static __device__ __forceinline__ float val(const type& a) { return val_of((uint32_t)(a >> 32)); }
+};
+template <> struct OcPair<double> {
+    typedef ulonglong2 type;            // x = key, y = index
+    static __device__ __forceinline__ type make(double v, uint32_t idx) { return make_ulonglong2(key_of(v), (unsigned long long)idx); }
+    static __device__ __forceinline__ bool less(const type& a, const type& b) { return a.x < b.x || (a.x == b.x && a.y < b.y); }
+    static __device__ __forceinline__ uint32_t idx(const type& a) { return (uint32_t)a.y; }
+    static __device__ __forceinline__ double val(const type& a) { return val_of((uint64_t)a.x); }
+};
+
+template <typename T, int LOGN> struct OnchipCfg {
     static constexpr int N = 1 << LOGN, L = N / 2;
     static constexpr int THREADS = (N / 8 > 1024) ? 1024 : N / 8;
     static constexpr int KPT = N / THREADS;             // keys per thread (8 or 16)
     static constexpr int EPT = L / THREADS;             // complex points per thread in an FFT stage (4 or 8)
     static constexpr int RP = L + (L >> 4);             // padded row
     static constexpr int WARPS = THREADS / 32;
-    // region A: spectrum / x_sim (complex RP) in the FFT half of an iteration, (key, index) pairs (u64 N) in the sort half
-    static constexpr size_t bytesA = (size_t)N * 8;
+    // region A: spectrum / x_sim (complex RP) in the FFT half of an iteration, (key, index) pairs in the sort half
+    static constexpr size_t bytesA = (size_t)N * sizeof(typename OcPair<T>::type) > (size_t)RP * 2 * sizeof(T)
+                                         ? (size_t)N * sizeof(typename OcPair<T>::type) : (size_t)RP * 2 * sizeof(T);
     static constexpr size_t smem = bytesA + (size_t)N * 2 /* packed slot counters */ + (size_t)N * 2 /* idx_old u16 */ +
                                    (size_t)(2 * 32 + 32) * 8 /* reduction scratch */;
 };
 
-struct OnchipArgs {
-    const float* anorm;         // [B][L+1] natural order
-    const float* sorted;        // [B][N]
+template <typename T> struct OnchipArgs {
+    const T* anorm;             // [B][L+1] natural order
+    const T* sorted;            // [B][N]
     uint32_t* perm;             // [B][N] in: perm0, out: final permutation
-    float* x;                   // [B][N] out
-    float* xadj_dbg;            // [B][N] or NULL: x_adj of the last executed iteration
+    T* x;                       // [B][N] out
+    T* xadj_dbg;                // [B][N] or NULL: x_adj of the last executed iteration
     int32_t* iters_used;        // [B] or NULL
     long long* hist;            // [B][max_iter] or NULL (zeroed by the host)
-    const float2* tw14;         // exp(-2 pi i m / 2^14)
+    const typename Cx<T>::type* tw14;   // exp(-2 pi i m / 2^14)
     unsigned int* ticket;       // zero on entry
     int max_iter;
     long long B;
@@ -55,32 +74,35 @@ struct OnchipArgs {
 __device__ __forceinline__ int xpos(int j) { const int n = j >> 1; return 2 * (n + (n >> 4)) + (j & 1); }
 
 // all Stockham stages of one row of L = 2^logL points (natural in -> natural out, forward sign)
-template <int THREADS, int EPT>
-__device__ __forceinline__ void onchip_fft(float2* s, int logL, int Rp, const float2* __restrict__ tw14) {
+template <typename T, int THREADS, int EPT>
+__device__ __forceinline__ void onchip_fft(typename Cx<T>::type* s, int logL, int Rp, const typename Cx<T>::type* __restrict__ tw14) {
     constexpr int RAD = EPT >= 8 ? 8 : EPT;
     constexpr int LOGRAD = RAD == 8 ? 3 : (RAD == 4 ? 2 : 1);
     int logNs = 0;
     while (logL - logNs >= LOGRAD) {
-        fft_stage<float, RAD, THREADS, EPT, true>(s, logL, logNs, 0, Rp, tw14);
+        fft_stage<T, RAD, THREADS, EPT, true>(s, logL, logNs, 0, Rp, tw14);
         logNs += LOGRAD;
     }
-    if (logL - logNs == 2) fft_stage<float, 4, THREADS, EPT, true>(s, logL, logNs, 0, Rp, tw14);
-    else if (logL - logNs == 1) fft_stage<float, 2, THREADS, EPT, true>(s, logL, logNs, 0, Rp, tw14);
+    if (logL - logNs == 2) fft_stage<T, 4, THREADS, EPT, true>(s, logL, logNs, 0, Rp, tw14);
+    else if (logL - logNs == 1) fft_stage<T, 2, THREADS, EPT, true>(s, logL, logNs, 0, Rp, tw14);
 }
 
-template <int LOGN>
-__global__ void __launch_bounds__(OnchipCfg<LOGN>::THREADS) e13_onchip_kernel(OnchipArgs a) {
-    typedef OnchipCfg<LOGN> Cfg;
+template <typename T, int LOGN>
+__global__ void __launch_bounds__(OnchipCfg<T, LOGN>::THREADS) e13_onchip_kernel(OnchipArgs<T> a) {
+    typedef OnchipCfg<T, LOGN> Cfg;
+    typedef typename Cx<T>::type C;
+    typedef OcPair<T> PR;
+    typedef typename PR::type Pair;
     constexpr int N = Cfg::N, L = Cfg::L, THREADS = Cfg::THREADS, KPT = Cfg::KPT, RP = Cfg::RP, WARPS = Cfg::WARPS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2* Z = reinterpret_cast<float2*>(smem_raw);
-    float* Zf = reinterpret_cast<float*>(smem_raw);
-    unsigned long long* pair = reinterpret_cast<unsigned long long*>(smem_raw);
+    C* Z = reinterpret_cast<C*>(smem_raw);
+    T* Zf = reinterpret_cast<T*>(smem_raw);
+    Pair* pair = reinterpret_cast<Pair*>(smem_raw);
     uint32_t* cw = reinterpret_cast<uint32_t*>(smem_raw + Cfg::bytesA);                  // [N/2]
     unsigned short* perm_s = reinterpret_cast<unsigned short*>(smem_raw + Cfg::bytesA + (size_t)N * 2);      // [N]
     double* red = reinterpret_cast<double*>(smem_raw + Cfg::bytesA + (size_t)N * 4);     // [64] + [32]
     __shared__ unsigned int s_curve;
-    __shared__ float s_lo, s_scale;
+    __shared__ T s_lo, s_scale;
     __shared__ unsigned int s_changed;
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
 
@@ -90,8 +112,8 @@ __global__ void __launch_bounds__(OnchipCfg<LOGN>::THREADS) e13_onchip_kernel(On
     __syncthreads();
     const long long b = s_curve;
     if (b >= a.B) break;
-    const float* An = a.anorm + b * (L + 1);
-    const float* srt = a.sorted + b * N;
+    const T* An = a.anorm + b * (L + 1);
+    const T* srt = a.sorted + b * N;
     uint32_t* pg = a.perm + b * N;
     // x_sim,1: the draw in draw order (Q15); idx_old = perm0
     for (int r = t; r < N; r += THREADS) {
@@ -103,21 +125,21 @@ __global__ void __launch_bounds__(OnchipCfg<LOGN>::THREADS) e13_onchip_kernel(On
     for (int k = 1; k <= a.max_iter; ++k) {
         __syncthreads();
         // ---- L1 forward FFT
-        onchip_fft<THREADS, Cfg::EPT>(Z, LOGN - 1, RP, a.tw14);
+        onchip_fft<T, THREADS, Cfg::EPT>(Z, LOGN - 1, RP, a.tw14);
         // ---- L2 untangle + amplitude replace + re-tangle (the stage's trailing barrier has been passed)
         for (int kk = t; kk <= L / 2; kk += THREADS) {
             if (kk == 0) {
-                const float2 z0 = Z[0];
-                const float x0 = z0.x + z0.y, xl = z0.x - z0.y;
-                const float a0 = An[0], al = An[L];
-                const float y0 = (x0 != 0.f) ? (x0 > 0.f ? a0 : -a0) : a0;
-                const float yl = (xl != 0.f) ? (xl > 0.f ? al : -al) : al;
-                Z[0] = make_float2(0.5f * (y0 + yl), 0.5f * (y0 - yl));
+                const C z0 = Z[0];
+                const T x0 = z0.x + z0.y, xl = z0.x - z0.y;
+                const T a0 = An[0], al = An[L];
+                const T y0 = (x0 != (T)0) ? (x0 > (T)0 ? a0 : -a0) : a0;
+                const T yl = (xl != (T)0) ? (xl > (T)0 ? al : -al) : al;
+                Z[0] = mk<T>((T)0.5 * (y0 + yl), (T)0.5 * (y0 - yl));
             } else {
                 const int k2 = L - kk;
                 const int p1 = kk + (kk >> 4), p2 = k2 + (k2 >> 4);
-                float2 z1 = Z[p1], z2 = Z[p2];
-                replace_pair<float>(z1, z2, a.tw14[kk << (kLogTw - LOGN)], An[kk], An[k2]);      // w_N^k
+                C z1 = Z[p1], z2 = Z[p2];
+                replace_pair<T>(z1, z2, a.tw14[kk << (kLogTw - LOGN)], An[kk], An[k2]);      // w_N^k
                 Z[p1] = z1;
                 if (k2 != kk) Z[p2] = z2;
             }
@@ -126,19 +148,19 @@ __global__ void __launch_bounds__(OnchipCfg<LOGN>::THREADS) e13_onchip_kernel(On
         // ---- L3 inverse FFT: swap, forward stages, swap and 1/L (folded into the key read below)
         for (int n = t; n < L; n += THREADS) { const int p = n + (n >> 4); Z[p] = cswap(Z[p]); }
         __syncthreads();
-        onchip_fft<THREADS, Cfg::EPT>(Z, LOGN - 1, RP, a.tw14);
+        onchip_fft<T, THREADS, Cfg::EPT>(Z, LOGN - 1, RP, a.tw14);
         // ---- L4 keys into registers: x_adj[j] = (1/L) * swapped component, + 0.0 (Q13)
-        float v[KPT];
-        const float invL = 1.0f / (float)L;
-        float sum = 0.f, sq = 0.f;
+        T v[KPT];
+        const T invL = (T)1 / (T)L;
+        T sum = 0, sq = 0;
 #pragma unroll
         for (int i = 0; i < KPT; ++i) {
             const int j = i * THREADS + t;
             const int n = j >> 1;
             // element j of the real series is the (j & 1) component of the UNSWAPPED result = the other one of Z
-            v[i] = Zf[2 * (n + (n >> 4)) + ((j & 1) ^ 1)] * invL + 0.0f;
+            v[i] = Zf[2 * (n + (n >> 4)) + ((j & 1) ^ 1)] * invL + (T)0;
             sum += v[i];
-            sq = fmaf(v[i], v[i], sq);
+            sq += v[i] * v[i];
         }
         if (a.xadj_dbg) {
 #pragma unroll
@@ -161,17 +183,17 @@ __global__ void __launch_bounds__(OnchipCfg<LOGN>::THREADS) e13_onchip_kernel(On
                     if (!(var > 0.0)) var = 0.0;
                     const double sg = sqrt(var);
                     const double lo = mu - 4.0 * sg, width = 8.0 * sg;
-                    s_lo = (float)lo;
-                    s_scale = (width > 0.0 && isfinite(width)) ? (float)((double)N / width) : 0.f;
+                    s_lo = (T)lo;
+                    s_scale = (width > 0.0 && isfinite(width)) ? (T)((double)N / width) : (T)0;
                 }
             }
             for (int i = t; i < N / 2; i += THREADS) cw[i] = 0u;
             __syncthreads();
         }
-        const float lo = s_lo, scale = s_scale;
-        auto slot_of = [&](float x) -> uint32_t {
-            const float f = (x - lo) * scale;                      // monotone in x; NaN / negative -> slot 0
-            return (f >= 1.0f) ? min((uint32_t)f, (uint32_t)(N - 1)) : 0u;
+        const T lo = s_lo, scale = s_scale;
+        auto slot_of = [&](T x) -> uint32_t {
+            const T f = (x - lo) * scale;                          // monotone in x; NaN / negative -> slot 0
+            return (f >= (T)1) ? (f < (T)N ? (uint32_t)f : (uint32_t)(N - 1)) : 0u;
         };
         // slot populations
 #pragma unroll
@@ -220,18 +242,18 @@ __global__ void __launch_bounds__(OnchipCfg<LOGN>::THREADS) e13_onchip_kernel(On
         for (int i = 0; i < KPT; ++i) {
             const uint32_t s = slot_of(v[i]), sh = (s & 1u) << 4;
             const uint32_t q = (atomicAdd(&cw[s >> 1], 1u << sh) >> sh) & 0xffffu;
-            pair[q] = ((unsigned long long)key_of(v[i]) << 32) | (uint32_t)(i * THREADS + t);
+            pair[q] = PR::make(v[i], (uint32_t)(i * THREADS + t));
         }
         __syncthreads();
         // exact rank among the slot mates; L5 on the fly: change count, idx_old <- idx_new, value for x_sim
         uint32_t oidx[KPT];
-        float oval[KPT];
+        T oval[KPT];
         uint32_t diff = 0;
 #pragma unroll
         for (int i = 0; i < KPT; ++i) {
             const int q = i * THREADS + t;
-            const unsigned long long pv = pair[q];
-            const uint32_t s = slot_of(val_of((uint32_t)(pv >> 32)));
+            const Pair pv = pair[q];
+            const uint32_t s = slot_of(PR::val(pv));
             const uint32_t w = cw[s >> 1];
             uint32_t z, st0;
             if (s & 1u) { z = w >> 16; st0 = w & 0xffffu; }
@@ -239,9 +261,9 @@ __global__ void __launch_bounds__(OnchipCfg<LOGN>::THREADS) e13_onchip_kernel(On
             uint32_t r = (uint32_t)q;
             if (z - st0 > 1u) {
                 r = st0;
-                for (uint32_t h = st0; h < z; ++h) r += (pair[h] < pv);
+                for (uint32_t h = st0; h < z; ++h) r += PR::less(pair[h], pv);
             }
-            const uint32_t idx = (uint32_t)pv;
+            const uint32_t idx = PR::idx(pv);
             diff += ((uint32_t)perm_s[r] != idx);
             perm_s[r] = (unsigned short)idx;
             oidx[i] = idx;
@@ -268,35 +290,38 @@ __global__ void __launch_bounds__(OnchipCfg<LOGN>::THREADS) e13_onchip_kernel(On
     }   // curve loop
 }
 
-inline bool onchip_applicable(size_t elem_size, long long N) { return elem_size == 4 && N >= 256 && N <= 16384; }
+inline bool onchip_applicable(size_t elem_size, long long N) {
+    return N >= 256 && ((elem_size == 4 && N <= 16384) || (elem_size == 8 && N <= 8192));
+}
 
-template <int LOGN> inline cudaError_t onchip_launch(const OnchipArgs& a, int slot, cudaStream_t st) {
-    typedef OnchipCfg<LOGN> Cfg;
+template <typename T, int LOGN> inline cudaError_t onchip_launch(const OnchipArgs<T>& a, int slot, cudaStream_t st) {
+    typedef OnchipCfg<T, LOGN> Cfg;
     int& grid = dev_cache().grid[slot];
     if (!grid) {
-        cudaError_t e = cudaFuncSetAttribute(e13_onchip_kernel<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem);
+        cudaError_t e = cudaFuncSetAttribute(e13_onchip_kernel<T, LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem);
         if (e != cudaSuccess) return e;
-        cudaFuncSetAttribute(e13_onchip_kernel<LOGN>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        cudaFuncSetAttribute(e13_onchip_kernel<T, LOGN>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
         int per = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, e13_onchip_kernel<LOGN>, Cfg::THREADS, Cfg::smem);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, e13_onchip_kernel<T, LOGN>, Cfg::THREADS, Cfg::smem);
         if (e != cudaSuccess) return e;
         if (per < 1) return cudaErrorInvalidConfiguration;
         grid = dev_cache().sms * per;
     }
     const unsigned g = (unsigned)std::min<long long>(a.B, grid);
-    AGN_LAUNCH(K_E13_ONCHIP, st, (e13_onchip_kernel<LOGN><<<g, Cfg::THREADS, Cfg::smem, st>>>(a)));
+    AGN_LAUNCH(K_E13_ONCHIP, st, (e13_onchip_kernel<T, LOGN><<<g, Cfg::THREADS, Cfg::smem, st>>>(a)));
     return cudaGetLastError();
 }
 
-inline cudaError_t onchip_run(int logN, const OnchipArgs& a, cudaStream_t st) {
+template <typename T> inline cudaError_t onchip_run(int logN, const OnchipArgs<T>& a, cudaStream_t st) {
+    constexpr int s0 = sizeof(T) == 4 ? 3 : 10;         // dev_cache().grid slots 3..9 (fp32), 10..15 (fp64)
     switch (logN) {
-        case 8: return onchip_launch<8>(a, 3, st);
-        case 9: return onchip_launch<9>(a, 3 + 1, st);
-        case 10: return onchip_launch<10>(a, 3 + 2, st);
-        case 11: return onchip_launch<11>(a, 3 + 3, st);
-        case 12: return onchip_launch<12>(a, 3 + 4, st);
-        case 13: return onchip_launch<13>(a, 3 + 5, st);
-        case 14: return onchip_launch<14>(a, 3 + 6, st);
+        case 8: return onchip_launch<T, 8>(a, s0, st);
+        case 9: return onchip_launch<T, 9>(a, s0 + 1, st);
+        case 10: return onchip_launch<T, 10>(a, s0 + 2, st);
+        case 11: return onchip_launch<T, 11>(a, s0 + 3, st);
+        case 12: return onchip_launch<T, 12>(a, s0 + 4, st);
+        case 13: return onchip_launch<T, 13>(a, s0 + 5, st);
+        case 14: if constexpr (sizeof(T) == 4) return onchip_launch<T, 14>(a, s0 + 6, st); else return cudaErrorInvalidValue;
         default: return cudaErrorInvalidValue;
     }
 }
