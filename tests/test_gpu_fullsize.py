@@ -117,3 +117,47 @@ def test_c4_full_size_lockstep(orc):
               f"fraction {eq:.4f}, changed {hist[:, 0].tolist()}")
         del xadj, x, out, x_prev, perm_prev, xadj64, xnext64, xg
     ag.free_workspace()
+
+
+def test_maximum_size_2p27(orc):
+    """The largest series the ABI accepts (N = 2^27, the paper's own cap), one curve, fp32: S1, S2 and two
+    E13 iterations through the paths only this size takes (two-level distribution sort, three column sub-passes of the
+    FFT, two-level rank scatter).  Properties that pin the result at any size, plus one whole oracle step from the GPU's
+    own x_sim (x_adj relative L2, eps-sortedness)."""
+    import paper_1909_06374_b200 as ag
+    from paper_1909_06374_b200 import workloads
+    cfg = workloads.config("C4", B=1)
+    N = 2 ** 27
+    srt, perm, _ = ag.agnvar_erdf_sample_sorted(cfg["erdf"], 1, N, "f32", cfg["seed"], 0, cfg["grid_points"])
+    assert bool((srt[:, 1:] >= srt[:, :-1]).all())
+    _, an = ag.agnvar_tk_generate(cfg["psd"], 1, N, cfg["dt"], 1, "f32", cfg["seed"], 0, want_xnorm=False)
+    assert bool(torch.isfinite(an).all())
+    o = ag.agnvar_e13_iterate(an, srt, perm, 1, want_fallbacks=True)
+    perm_prev, x_prev = perm.clone(), o["x"].clone()
+    del o
+    out = ag.agnvar_e13_iterate(an, srt, perm, 1, want_hist=True, want_xadj=True, want_fallbacks=True)
+    torch.cuda.synchronize()
+    xadj, x, hist = out["x_adj"], out["x"], out["changed_hist"]
+    p = perm[0].long()
+    seen = torch.zeros(N, dtype=torch.uint8, device="cuda")
+    seen[p] = 1
+    assert bool(seen.all()), "not a permutation"
+    del seen
+    xa = (xadj[0] + 0.0)[p]
+    assert bool((xa[1:] >= xa[:-1]).all()), "x_adj is not sorted along the permutation"
+    tie = xa[1:] == xa[:-1]
+    assert bool((p[1:][tie] > p[:-1][tie]).all()), "equal keys are not in time-index order"
+    del xa, tie
+    assert torch.equal(x[0][p], srt[0]), "rank scatter"
+    assert int(hist[0, 0]) == int((perm[0] != perm_prev[0]).sum()), "change count"
+    del p
+    xadj64, _, xnext64, _ = orc.e13_step(an[0].cpu().numpy(), srt[0].cpu().numpy(), u32(perm_prev[0]).copy(),
+                                         x_prev[0].cpu().numpy())
+    xg = xadj[0].cpu().numpy().astype(np.float64)
+    rel = np.linalg.norm(xg - xadj64) / np.linalg.norm(xadj64)
+    eps = np.max(np.abs(xg - xadj64))
+    print(f"N=2^27: x_adj rel L2 {rel:.2e}, eps {eps:.2e}, changed {hist[:, 0].tolist()}, "
+          f"sort fallbacks {out['sort_fallbacks'].tolist()}")
+    assert rel <= 1e-5, rel
+    assert (np.diff(xadj64[u32(perm[0])]) >= -2.0 * eps).all()
+    ag.free_workspace()
