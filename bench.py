@@ -137,8 +137,11 @@ class ClockSampler:
 
 
 def workload_label(cfg):
-    return (f"{cfg['name']}: B={cfg['B']} curves x N=2^{cfg['N'].bit_length() - 1} samples, {cfg['dtype']}, "
-            f"max_iter={cfg['max_iter']}, oversample={cfg['oversample']}")
+    s = (f"{cfg['name']}: B={cfg['B']} curves x N=2^{cfg['N'].bit_length() - 1} samples, {cfg['dtype']}, "
+         f"max_iter={cfg['max_iter']}, oversample={cfg['oversample']}")
+    if cfg.get("sampler") == "slice":
+        s += f", S1 by slice sampling {cfg['slice']} (NOT the headline configuration)"
+    return s
 
 
 # ------------------------------------------------------------------------------------------------------
@@ -274,6 +277,8 @@ def main():
     ap.add_argument("--workload", default="C4")
     ap.add_argument("--batch", type=int, default=None, help="override B (subset of the configuration)")
     ap.add_argument("--max-iter", type=int, default=None, help="override max_iter (NOT the headline configuration)")
+    ap.add_argument("--sampler", default="inverse_cdf", choices=["inverse_cdf", "slice"],
+                    help="S1 by the inverse-CDF table (north_star, the headline) or by the paper's slice sampler (NEXT-3)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-context", action="store_true", help="skip the fp32 free-running context numbers")
@@ -287,6 +292,9 @@ def main():
     cfg = workloads.config(args.workload, B=args.batch)
     if args.max_iter is not None:
         cfg["max_iter"] = args.max_iter
+    if args.sampler == "slice":
+        cfg["sampler"] = "slice"
+        cfg["slice"] = dict(chains=min(cfg["N"], 65536), burn_in=50, thin=1, width=1.0, max_steps=8)
     if args.impl == "reference":
         run_reference(args, cfg)
         return 0

@@ -23,8 +23,16 @@ def generate_light_curves(cfg, device="cuda", host_out=None, want_hist=False, cu
     B, N = cfg["B"], cfg["N"]
     psd_c, erdf_c = _b.marshal_params(cfg)
     hook("S1")
-    srt, perm, _ = _b.agnvar_erdf_sample_sorted(erdf_c, B, N, cfg["dtype"], cfg["seed"], curve0,
-                                                cfg["grid_points"], device=device)
+    if cfg.get("sampler", "inverse_cdf") == "slice":
+        # the paper's own sampler for the random draw (NEXT-3): cfg["slice"] = dict(chains, burn_in, thin,
+        # width, max_steps); same distribution as the inverse-CDF sampler, different samples
+        so = dict(chains=min(N, 4096), burn_in=50, thin=1, width=1.0, max_steps=8)
+        so.update(cfg.get("slice", {}))
+        srt, perm, _, _ = _b.agnvar_slice_sample_sorted(erdf_c, B, N, cfg["dtype"], cfg["seed"], curve0=curve0,
+                                                        device=device, **so)
+    else:
+        srt, perm, _ = _b.agnvar_erdf_sample_sorted(erdf_c, B, N, cfg["dtype"], cfg["seed"], curve0,
+                                                    cfg["grid_points"], device=device)
     hook("S2")
     _, anorm = _b.agnvar_tk_generate(psd_c, B, N, cfg["dt"], cfg["oversample"], cfg["dtype"], cfg["seed"],
                                      curve0, want_xnorm=False, device=device)

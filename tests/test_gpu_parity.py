@@ -628,3 +628,24 @@ def test_slice_sample_validation(ag):
         ag.agnvar_slice_sample_sorted(dict(kind=2, lam_min=1e-3, lam_max=1.0), 1, 1024, "f32", 1, chains=64)
     with pytest.raises(bd.AgnvarError):        # the inverse-CDF sampler does not take tables
         ag.agnvar_erdf_sample_sorted(dict(kind=2, lam_min=1e-3, lam_max=1.0), 1, 1024, "f32", 1)
+
+
+def test_pipeline_with_slice_sampler(ag, orc):
+    """The whole path with the paper's sampler for the draw (cfg['sampler'] = 'slice'): S1 is the oracle's
+    slice-sampled draw, and the E13 loop on it is the oracle's (fp64: identical trajectory from the same inputs)."""
+    from paper_1909_06374_b200 import workloads
+    cfg = workloads.config("C1", B=2)
+    so = dict(chains=64, burn_in=10, thin=1, width=1.0, max_steps=4)
+    cfg.update(N=1024, max_iter=20, sampler="slice", slice=so)
+    out = ag.generate_light_curves(cfg, want_hist=True)
+    srt, perm0, _, _ = ag.agnvar_slice_sample_sorted(cfg["erdf"], 2, 1024, "f64", cfg["seed"], **so)
+    _, an = ag.agnvar_tk_generate(cfg["psd"], 2, 1024, cfg["dt"], cfg["oversample"], "f64", cfg["seed"], 0,
+                                  want_xnorm=False)
+    for b in range(2):
+        lam, _ = orc.slice_sample(cfg["erdf"][0], 1024, 64, cfg["seed"], b, 1, burn_in=10, thin=1, w=1.0, m=4)
+        srt_h = srt[b].cpu().numpy()
+        assert np.allclose(srt_h, np.sort(lam), rtol=1e-14, atol=0)
+        ref = orc.e13_iterate(an[b].cpu().numpy(), srt_h, u32(perm0[b]).copy(), 20)
+        assert int(out["iters_used"][b]) == ref["iters_used"]
+        assert (u32(out["perm"][b]) == ref["perm"]).all()
+        assert (out["x"][b].cpu().numpy() == ref["x"]).all()
