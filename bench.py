@@ -63,6 +63,8 @@ ALGO_BYTES_PER_SAMPLE = {
 }
 # SURVEY.md 8(d) two-level model, bytes per sample per iteration, per stage (fp32)
 STAGE_MODEL_BYTES = {"fft": 26.0, "argsort": 28.0, "scatter": 32.0}
+# SURVEY.md 8(d) "floor": what the method must move with unlimited on-chip capacity (reported alongside)
+STAGE_FLOOR_BYTES = {"fft": 10.0, "argsort": 8.0, "scatter": 16.0}
 STAGE_OF = {
     "fft_pass_strided": "fft", "fft_pass_contiguous": "fft", "amplitude_replace": "fft", "fft_mid_fused": "fft", "fft_columns": "fft",
     "sort_digit_hist": "argsort", "sort_onesweep": "argsort", "cta_argsort": "argsort",
@@ -443,7 +445,9 @@ def main():
                       "moved_bytes_per_sample": st_bytes[s],        # what this build's kernels move (algorithmic, summed)
                       "moved_over_model": st_bytes[s] / STAGE_MODEL_BYTES[s],
                       "achieved_GBps": STAGE_MODEL_BYTES[s] * B * N / (t / iters * 1e-3) / 1e9,
-                      "frac_of_peak": STAGE_MODEL_BYTES[s] * B * N / (t / iters * 1e-3) / 1e9 / peak}
+                      "frac_of_peak": STAGE_MODEL_BYTES[s] * B * N / (t / iters * 1e-3) / 1e9 / peak,
+                      "floor_bytes_per_sample": STAGE_FLOOR_BYTES[s],
+                      "frac_of_peak_floor_model": STAGE_FLOOR_BYTES[s] * B * N / (t / iters * 1e-3) / 1e9 / peak}
                   for s, t in st_ms.items()}
         if "argsort" in st_ms and "scatter" in st_ms:
             # the write-back sort does part of L5 inside the sort's finish kernel (values go home along the partition
