@@ -368,7 +368,7 @@ int tk_impl(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_t N, double
         const int logLM = ilog2_u64((uint64_t)M) - 1;
         const long long LM = M / 2;
         FftPlan<T> pm = fft_plan_init<T>(logLM, tabM, st);
-        AGN_LAUNCH(K_TK_FILL, st, (tk_fill_kernel<T><<<bgrid(cdiv(LM, 256), B), 256, 0, st>>>((C*)ZM, psd, pm.dg, dt, seed, curve0, (int)B)));
+        AGN_LAUNCH(K_TK_FILL, st, (tk_fill_kernel<T><<<bgrid(cdiv(LM / 2 + 1, 256), B), 256, 0, st>>>((C*)ZM, psd, pm.dg, dt, seed, curve0, (int)B)));
         fft_inverse<T>(pm, (const C*)ZM, (C*)ZM, LM, LM, (int)B, (T)(1.0 / (double)LM), st);
         if (os == 1) xsrc = ZM;
         else {

@@ -18,9 +18,11 @@ __global__ void philox_words_kernel(uint64_t seed, uint64_t i0, long long n, uin
 }
 
 // Eq. 3 bracket: [ (f/f_b)^a_lo + (f/f_b)^a_hi ]^-1
+// (r^a as exp2(a log2 r): one logarithm for both powers; the exponent a log2 r stays below ~100 in magnitude, so the
+//  result is within ~1e-14 relative of pow(): PSD values are gated at 1e-13 against the oracle)
 __device__ __forceinline__ double psd_shape(double f, double f_b, double a_lo, double a_hi) {
-    double r = f / f_b;
-    return 1.0 / (pow(r, a_lo) + pow(r, a_hi));
+    const double l = log2(f / f_b);
+    return 1.0 / (exp2(a_lo * l) + exp2(a_hi * l));
 }
 
 __global__ void psd_bpl_kernel(const double* __restrict__ f, long long n, PsdDev p, double* __restrict__ out) {
@@ -90,23 +92,35 @@ __device__ __forceinline__ double2 tk_X(const PsdDev& p, long long j, long long 
 // Power-of-two M: fill Z (position order, L = M/2 complex) such that the inverse complex FFT of length L
 // (unnormalised, then scale 1/L) yields z[n] = x[2n] + i x[2n+1] with x = irfft_M(X).
 // a = (X_k + conj X_{L-k})/2, b = (X_k - conj X_{L-k})/2, O = b conj(w_M^k), Z_k = a + i O.
+// One thread per PAIR of bins (k, L - k), 0 <= k <= L/2: both spectrum values are evaluated once (Philox, Box-Muller, Eq. 3)
+// and give both Z_k and Z_{L-k} (the second one goes to a scattered position: a plain 8-byte store).
 template <typename T>
 __global__ void tk_fill_kernel(typename Cx<T>::type* __restrict__ Z, const PsdDev* __restrict__ psd, Digits dg,
                                double dt, uint64_t seed, uint32_t curve0, int B) {
     const long long L = 1ll << dg.logL, M = 2 * L;
-    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int b = (int)bidx();
-    if (p >= L || b >= B) return;
+    if (2 * k > L || b >= B) return;
     PsdDev ps = psd[b];
-    uint32_t k = pos2k(dg, (uint32_t)p);
-    double2 X1 = tk_X(ps, k, M, dt, seed, curve0 + b);
-    double2 X2 = tk_X(ps, L - k, M, dt, seed, curve0 + b);     // k = 0 pairs with the Nyquist bin L
-    double2 a = make_double2(0.5 * (X1.x + X2.x), 0.5 * (X1.y - X2.y));
-    double2 bb = make_double2(0.5 * (X1.x - X2.x), 0.5 * (X1.y + X2.y));
+    const long long k2 = L - k;                                 // k = 0 pairs with the Nyquist bin L
+    const double2 X1 = tk_X(ps, k, M, dt, seed, curve0 + b);
+    const double2 X2 = tk_X(ps, k2, M, dt, seed, curve0 + b);
     double sn, cs;
     sincos_2pi_frac((uint64_t)k, dg.logL + 1, &sn, &cs);        // conj(w_M^k) = cos + i sin
-    double2 O = make_double2(bb.x * cs - bb.y * sn, bb.x * sn + bb.y * cs);
-    Z[(long long)b * L + p] = mk<T>((T)(a.x - O.y), (T)(a.y + O.x));
+    {
+        const double2 a = make_double2(0.5 * (X1.x + X2.x), 0.5 * (X1.y - X2.y));
+        const double2 bb = make_double2(0.5 * (X1.x - X2.x), 0.5 * (X1.y + X2.y));
+        const double2 O = make_double2(bb.x * cs - bb.y * sn, bb.x * sn + bb.y * cs);
+        Z[(long long)b * L + k2pos(dg, (uint32_t)k)] = mk<T>((T)(a.x - O.y), (T)(a.y + O.x));
+    }
+    if (k > 0 && k2 != k) {
+        // the same formula with the roles of the two bins exchanged; conj(w_M^{L-k}) = -cos + i sin
+        const double2 a = make_double2(0.5 * (X2.x + X1.x), 0.5 * (X2.y - X1.y));
+        const double2 bb = make_double2(0.5 * (X2.x - X1.x), 0.5 * (X2.y + X1.y));
+        const double c2 = -cs, s2 = sn;
+        const double2 O = make_double2(bb.x * c2 - bb.y * s2, bb.x * s2 + bb.y * c2);
+        Z[(long long)b * L + k2pos(dg, (uint32_t)k2)] = mk<T>((T)(a.x - O.y), (T)(a.y + O.x));
+    }
 }
 
 // M = 5 * Mp (oversample 10 or 20): three decimated spectra X_r[q] = Xfull[5q + r], r = 0,1,2, each a

@@ -160,7 +160,7 @@ __global__ void __launch_bounds__(OnchipCfg<T, LOGN>::THREADS) e13_onchip_kernel
             // element j of the real series is the (j & 1) component of the UNSWAPPED result = the other one of Z
             v[i] = Zf[2 * (n + (n >> 4)) + ((j & 1) ^ 1)] * invL + (T)0;
             sum += v[i];
-            sq += v[i] * v[i];
+            sq = fma(v[i], v[i], sq);
         }
         if (a.xadj_dbg) {
 #pragma unroll
@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(OnchipCfg<T, LOGN>::THREADS) e13_onchip_kernel
         const T lo = s_lo, scale = s_scale;
         auto slot_of = [&](T x) -> uint32_t {
             const T f = (x - lo) * scale;                          // monotone in x; NaN / negative -> slot 0
-            return (f >= (T)1) ? (f < (T)N ? (uint32_t)f : (uint32_t)(N - 1)) : 0u;
+            return (f >= (T)1) ? min((uint32_t)f, (uint32_t)(N - 1)) : 0u;     // (the conversion saturates)
         };
         // slot populations
 #pragma unroll
