@@ -447,7 +447,7 @@ template <typename T> __global__ void copy_canon_kernel(const T* __restrict__ sr
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double erdf_xi(const ErdfDev& e, double u) {
     if (e.kind == 0) {
-        double r = pow(10.0, u) / e.lam_star;
+        double r = exp10(u) / e.lam_star;         // (exp10: same 1-ulp class as pow(10, u), a third of its cost)
         return 1.0 / (pow(r, e.d1) + pow(r, e.d2));
     }
     double z = (u - e.mu) / e.sigma;
@@ -524,7 +524,7 @@ __global__ void erdf_sample_kernel(const ErdfDev* __restrict__ erdf, int per_cur
         }
         double c0 = Cc[lo], c1 = Cc[lo + 1];
         double uu = (e.u_lo + (double)lo * D) + (U[q] - c0) / (c1 - c0) * D;
-        out[(long long)b * N + 2 * i + q] = (T)pow(10.0, uu);
+        out[(long long)b * N + 2 * i + q] = (T)exp10(uu);
     }
 }
 

@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(128) slice_sample_kernel(SliceArgs a, T* __res
         if (--until_keep == 0) {
             until_keep = a.thin;
             const long long n = j * a.chains + c;
-            out[(long long)b * a.N + n] = (T)pow(10.0, x);
+            out[(long long)b * a.N + n] = (T)exp10(x);
             if (u_out) u_out[(long long)b * a.N + n] = x;
             ++j;
         }
