@@ -34,7 +34,7 @@ struct Carver {
 
 inline bool is_pow2(int64_t n) { return n > 0 && (n & (n - 1)) == 0; }
 inline bool valid_BN(int64_t B, int64_t N) {
-    return B >= 1 && B <= (int64_t)1 << 30 && is_pow2(N) && N >= 4 && N <= ((int64_t)1 << 27);
+    return B >= 1 && B <= (int64_t)1 << 30 && is_pow2(N) && N >= 4 && N <= ((int64_t)1 << 28);
 }
 inline bool valid_dtype(int d) { return d == AGNVAR_F32 || d == AGNVAR_F64; }
 inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }

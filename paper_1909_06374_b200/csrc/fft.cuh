@@ -17,7 +17,7 @@
 namespace agn {
 
 constexpr int kLogTw = 14;        // fine table: exp(-2 pi i m / 2^14)
-constexpr int kLogLo = 13;        // per-level low table: exp(-2 pi i l / D), l < 2^13
+constexpr int kLogLo = 14;        // per-level low table: exp(-2 pi i l / D), l < 2^14 (levels up to D = 2^28: the real-FFT level of N = 2^28)
 constexpr int kMaxPass = 3;
 constexpr int kFftThreads = 512;
 
@@ -55,7 +55,7 @@ __host__ __device__ __forceinline__ uint32_t k2pos(const Digits& d, uint32_t k) 
 // Twiddle level: w_D^idx = exp(-2 pi i idx / D), D = 2^logD <= 2^27, idx < D/2... (any idx < D).
 template <typename T> struct TwLevel {
     const typename Cx<T>::type* tw14;   // exp(-2 pi i m / 2^14)
-    const typename Cx<T>::type* lo;     // exp(-2 pi i l / D), l < 2^13 (only if logD > 14)
+    const typename Cx<T>::type* lo;     // exp(-2 pi i l / D), l < 2^kLogLo (only if logD > kLogTw)
     int logD;
 };
 
@@ -63,7 +63,7 @@ template <typename T>
 __device__ __forceinline__ typename Cx<T>::type tw_lookup(const TwLevel<T>& lv, uint32_t idx) {
     if (lv.logD <= kLogTw) return lv.tw14[idx << (kLogTw - lv.logD)];
     uint32_t h = idx >> kLogLo, l = idx & ((1u << kLogLo) - 1u);
-    // exp(-2 pi i h 2^13 / D) = tw14[h * 2^14 * 2^13 / D]
+    // exp(-2 pi i h 2^kLogLo / D) = tw14[h * 2^kLogTw * 2^kLogLo / D]
     return cmul(lv.tw14[h << (kLogTw + kLogLo - lv.logD)], lv.lo[l]);
 }
 

@@ -37,7 +37,8 @@ def test_workspace_query_and_validation(L):
     assert b.workspace_bytes(b.OP_E13_ITERATE, 4, 2 ** 26, "f32") > 4 * 2 ** 26 * 4
     assert b.workspace_bytes(b.OP_E13_ITERATE, 4, 2 ** 26 + 2, "f32") == 0
     assert b.workspace_bytes(b.OP_E13_ITERATE, 4, 2, "f32") == 0
-    assert b.workspace_bytes(b.OP_E13_ITERATE, 4, 2 ** 28, "f32") == 0
+    assert b.workspace_bytes(b.OP_E13_ITERATE, 1, 2 ** 28, "f32") > 2 ** 28 * 4 * 4     # the largest series accepted
+    assert b.workspace_bytes(b.OP_E13_ITERATE, 4, 2 ** 29, "f32") == 0
     assert b.workspace_bytes(b.OP_TK_GENERATE, 4, 4096, "f64", 3) == 0
     assert b.workspace_bytes(b.OP_TK_GENERATE, 4, 4096, "f64", 10) > 0
     assert b.workspace_bytes(b.OP_ERDF_SAMPLE_SORTED, 4, 4096, "f64", 1, 1) == 0
