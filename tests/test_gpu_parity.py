@@ -649,3 +649,20 @@ def test_pipeline_with_slice_sampler(ag, orc):
         assert int(out["iters_used"][b]) == ref["iters_used"]
         assert (u32(out["perm"][b]) == ref["perm"]).all()
         assert (out["x"][b].cpu().numpy() == ref["x"]).all()
+
+
+def test_slice_sample_per_curve_parameters(ag, orc):
+    """n_erdf = B: every curve its own density (C5's per-curve ERDF slopes; per-curve tables for kind 2)."""
+    from paper_1909_06374_b200 import workloads
+    cfg = workloads.config("C5", B=6)
+    opt = dict(chains=32, burn_in=5, thin=1, width=1.0, max_steps=4)
+    _, _, draw, u = ag.agnvar_slice_sample_sorted(cfg["erdf"], 6, 512, "f64", 9, want_draw=True, want_u=True, **opt)
+    for b in range(6):
+        _, u_ref = orc.slice_sample(cfg["erdf"][b], 512, 32, 9, b, 1, burn_in=5, thin=1, w=1.0, m=4)
+        assert np.abs(u[b].cpu().numpy() - u_ref).max() <= 1e-12
+    tabs = np.stack([np.linspace(0.0, 4.0, 17), np.linspace(4.0, 0.0, 17) ** 2, np.ones(17)])
+    erdfs = [dict(kind=2, lam_min=1e-3, lam_max=10.0)] * 3
+    _, _, _, u = ag.agnvar_slice_sample_sorted(erdfs, 3, 512, "f32", 9, want_u=True, density=torch.tensor(tabs, device="cuda"), **opt)
+    for b in range(3):
+        _, u_ref = orc.slice_sample(erdfs[b], 512, 32, 9, b, 0, burn_in=5, thin=1, w=1.0, m=4, table=tabs[b])
+        assert (u[b].cpu().numpy() == u_ref).all()
