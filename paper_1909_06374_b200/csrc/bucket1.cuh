@@ -37,10 +37,10 @@ constexpr int kB1Tile = kB1PartThreads * kB1PartEpt;      // 8192 keys
 constexpr int kB1SortThreads = 1024;
 
 inline bool bucket1_applicable(size_t elem_size, long long N) {
-    return elem_size == 4 && N >= (1ll << 18) && N <= ((long long)kB1MaxBuckets << kB1MeanLog);
+    return elem_size == 4 && N >= (1ll << 15) && N <= ((long long)kB1MaxBuckets << kB1MeanLog);
 }
-inline uint32_t bucket1_magic(uint32_t nb) {
-    return (uint32_t)((((unsigned __int128)nb) << (32 + kB1SlotLog + 9)) / (kBkTotalW << 16));
+inline uint32_t bucket1_magic(uint32_t nb, int bl) {
+    return (uint32_t)((((unsigned __int128)nb) << (32 + kB1SlotLog + 25 - bl)) / (bk_total_w(bl) << (32 - bl)));
 }
 
 struct Part1Args {
@@ -52,6 +52,7 @@ struct Part1Args {
     uint32_t* loc;              // write-back mode (else null): [B][N] slab position (bucket * kB1Cap + offset) of the pair
     unsigned short* jrec;       //   at stage position s of the tile, and its sample number inside the tile, in STAGE order
     uint32_t N, nb, M;
+    int bl;                     // log2 of the CDF table's bins per curve
     long long B;
 };
 
@@ -71,7 +72,7 @@ __global__ void __launch_bounds__(kB1PartThreads, 2) part1_kernel(Part1Args a) {
     if (b >= a.B) return;
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     constexpr int NW = kB1PartThreads / 32;
-    const uint2* tab = a.tab + (size_t)b * kBkBins;
+    const uint2* tab = a.tab + ((size_t)b << a.bl);
     const uint32_t nb = a.nb;
     const uint32_t nv = nb >> 2;                          // uint4 words of counters (nb is a multiple of 32)
     const uint32_t nchunk = (nb + kB1Chunk - 1) / kB1Chunk;      // <= 64
@@ -89,7 +90,7 @@ __global__ void __launch_bounds__(kB1PartThreads, 2) part1_kernel(Part1Args a) {
         // few, wide buckets: neighbouring samples of a smooth series mostly share theirs -- one atomic for lane 0's group
 #pragma unroll
         for (int j = 0; j < kB1PartEpt; ++j) {
-            const uint32_t d = min(bs_of(key[j], tab, a.M) >> kB1SlotLog, nb - 1u);
+            const uint32_t d = min(bs_of(key[j], tab, a.M, a.bl) >> kB1SlotLog, nb - 1u);
             const uint32_t dl = __shfl_sync(0xffffffffu, d, 0);
             const uint32_t same = __ballot_sync(0xffffffffu, d == dl);
             uint32_t r = 0;
@@ -101,7 +102,7 @@ __global__ void __launch_bounds__(kB1PartThreads, 2) part1_kernel(Part1Args a) {
     } else {
 #pragma unroll
         for (int j = 0; j < kB1PartEpt; ++j) {
-            const uint32_t d = min(bs_of(key[j], tab, a.M) >> kB1SlotLog, nb - 1u);
+            const uint32_t d = min(bs_of(key[j], tab, a.M, a.bl) >> kB1SlotLog, nb - 1u);
             dr[j] = (d << 14) | atomicAdd(&cnt[d], 1u);
         }
     }
@@ -230,7 +231,19 @@ struct B1Wb {
     float* x_out;                   // [B][N]
 };
 
-template <bool WB>
+// TAB: the slot of a key is its sub-bucket position on the sampled CDF (bs_of, the same table look-up part1_kernel
+// did) instead of a linear map of the key onto the bucket's key interval.  For the few, wide buckets of a short curve
+// (N < 2^20: a bucket is 1/4 .. 1/64 of the whole distribution, and float keys are logarithmic in the value) the
+// linear map crowds most pairs into a few slots -- the rank among slot mates costs the square of a slot's population:
+// 2.3 ms instead of 0.2 per 2^25 samples at N = 2^15 with C4's ERDF.  The table of such a curve is small (2^11 ..
+// 2^15 bins) and stays in L1 / L2.
+struct B1Tab {
+    const uint2* tab;               // [B][2^bl]
+    uint32_t M;
+    int bl;
+};
+
+template <bool WB, bool TAB>
 __global__ void __launch_bounds__(kB1SortThreads, 2) bucket1_sort_kernel(const uint2* __restrict__ slabs,
                                                                          const uint32_t* __restrict__ cursor,
                                                                          const uint32_t* __restrict__ base,
@@ -238,7 +251,7 @@ __global__ void __launch_bounds__(kB1SortThreads, 2) bucket1_sort_kernel(const u
                                                                          const uint32_t* __restrict__ klos,
                                                                          uint32_t* __restrict__ idx_out,
                                                                          float* __restrict__ sorted_out, uint32_t N,
-                                                                         uint32_t nb, long long B, B1Wb wb) {
+                                                                         uint32_t nb, long long B, B1Wb wb, B1Tab tb) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     B1Smem& sm = *reinterpret_cast<B1Smem*>(smem_raw);
     const long long b = bidx();
@@ -261,7 +274,13 @@ __global__ void __launch_bounds__(kB1SortThreads, 2) bucket1_sort_kernel(const u
         if (bk == 0 && nb > 2) { width = 2u * min(kb[2] - kb[1], 0x7fffffffu); klo = kb[1] > width ? kb[1] - width : 0u; width = kb[1] - klo; }
     }
     const float scale = (float)kB1Slots / ((float)width + 1.0f);
+    const uint2* ctab = TAB ? tb.tab + ((size_t)b << tb.bl) : nullptr;
+    const uint32_t bs0 = bk << kB1SlotLog;
     auto slot_of = [&](uint32_t key) -> uint32_t {
+        if (TAB) {
+            const uint32_t bs = bs_of(key, ctab, tb.M, tb.bl);          // monotone in the key; equal keys, equal slots
+            return bs > bs0 ? min(bs - bs0, (uint32_t)(kB1Slots - 1)) : 0u;
+        }
         const uint32_t d = key > klo ? key - klo : 0u;
         return min((uint32_t)(__uint2float_rz(d) * scale), (uint32_t)(kB1Slots - 1));
     };
@@ -471,11 +490,13 @@ __global__ void __launch_bounds__(kB1GatherThreads, 4) gather_back_kernel(const 
 // ------------------------------------------------------------------------------------------------
 inline cudaError_t bucket1_set_attrs() {
     cudaFuncSetAttribute(part1_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    cudaFuncSetAttribute(bucket1_sort_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    cudaFuncSetAttribute(bucket1_sort_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaFuncSetAttribute(bucket1_sort_kernel<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaFuncSetAttribute(bucket1_sort_kernel<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaFuncSetAttribute(bucket1_sort_kernel<true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     cudaError_t e = cudaFuncSetAttribute(part1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)part1_smem(kB1MaxBuckets));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket1_sort_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(B1Smem));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket1_sort_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(B1Smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket1_sort_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(B1Smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket1_sort_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(B1Smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bucket1_sort_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(B1Smem));
     return e;
 }
 
@@ -503,11 +524,11 @@ inline void bucket1_wb_carve(void* p, long long B, long long N, B1Wb* wb) {
 //                base [B][nb] | klo [B][nb+1]
 inline size_t bucket1_zero_bytes(long long B, long long N) {
     const size_t nb = (size_t)(N >> kB1MeanLog);
-    return (size_t)B * kBkBins * 4 + (size_t)B * nb * 4 + (size_t)B * 4;
+    return (((size_t)B * 4) << bk_binlog(N)) + (size_t)B * nb * 4 + (size_t)B * 4;
 }
 inline size_t bucket1_ctl_bytes(long long B, long long N) {
     const size_t nb = (size_t)(N >> kB1MeanLog);
-    return align_up(bucket1_zero_bytes(B, N), 256) + align_up((size_t)B * kBkBins * 8, 256) + align_up((size_t)B * nb * 4, 256) +
+    return align_up(bucket1_zero_bytes(B, N), 256) + align_up(((size_t)B * 8) << bk_binlog(N), 256) + align_up((size_t)B * nb * 4, 256) +
            align_up((size_t)B * (nb + 1) * 4, 256);
 }
 
@@ -521,35 +542,43 @@ inline cudaError_t bucket1_sort(const float* vals, uint32_t* idx_out, float* sor
     const uint32_t nb = (uint32_t)(N >> kB1MeanLog);
     unsigned char* w = (unsigned char*)ctl;
     uint32_t* hist = (uint32_t*)w;
-    uint32_t* cursor = hist + (size_t)B * kBkBins;
+    const int bl = bk_binlog(N);
+    uint32_t* cursor = hist + ((size_t)B << bl);
     uint32_t* overflow = cursor + (size_t)B * nb;
     const size_t zero_bytes = bucket1_zero_bytes(B, N);
     w += align_up(zero_bytes, 256);
-    uint2* tab = (uint2*)w; w += align_up((size_t)B * kBkBins * 8, 256);
+    uint2* tab = (uint2*)w; w += align_up(((size_t)B * 8) << bl, 256);
     uint32_t* base = (uint32_t*)w; w += align_up((size_t)B * nb * 4, 256);
     uint32_t* klo = (uint32_t*)w;
     cudaError_t e = cudaMemsetAsync(hist, 0, zero_bytes, st);
     if (e != cudaSuccess) return e;
     const uint32_t nsamp = (uint32_t)(N >> kBkSampleLog);
-    const uint32_t M = bucket1_magic(nb);
-    AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B)));
-    AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)(B * kCdfChunks), 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
-    AGN_LAUNCH(K_SORT_CDF, st, (bucket_bounds_kernel<<<bgrid((nb + 256) / 256, B), 256, 0, st>>>(tab, klo, nb, M, kB1SlotLog, B)));
+    const uint32_t M = bucket1_magic(nb, bl);
+    const unsigned chunks = cdf_chunks(bl);
+    AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B, bl)));
+    AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)(B * chunks), 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog), bl, chunks)));
+    AGN_LAUNCH(K_SORT_CDF, st, (bucket_bounds_kernel<<<bgrid((nb + 256) / 256, B), 256, 0, st>>>(tab, klo, nb, M, kB1SlotLog, B, bl)));
     Part1Args a;
     a.vals = vals; a.out = pairs; a.cursor = cursor; a.overflow = overflow; a.tab = tab;
-    a.N = (uint32_t)N; a.nb = nb; a.M = M; a.B = B;
+    a.N = (uint32_t)N; a.nb = nb; a.M = M; a.B = B; a.bl = bl;
     a.loc = wb ? wb->loc : nullptr; a.jrec = wb ? wb->jrec : nullptr;
     AGN_LAUNCH(wb ? K_SORT_PART_ONE_WB : K_SORT_PART_ONE, st, (part1_kernel<<<bgrid((unsigned)(N / kB1Tile), B), kB1PartThreads, part1_smem(nb), st>>>(a)));
     const uint32_t bchunks = nb >= 1024 ? nb / 1024 : 1u;
     AGN_LAUNCH(K_SORT_CDF, st, (bucket_base_kernel<<<(unsigned)(B * bchunks), 1024, 0, st>>>(cursor, base, nb, bchunks, (uint32_t)kB1Cap)));
     if (wb) {
-        AGN_LAUNCH(K_SORT_BUCKET_WB, st, (bucket1_sort_kernel<true><<<bgrid(nb, B), kB1SortThreads, sizeof(B1Smem), st>>>(
-            pairs, cursor, base, overflow, klo, idx_out, sorted_out, (uint32_t)N, nb, B, *wb)));
+        AGN_LAUNCH(K_SORT_BUCKET_WB, st, (bucket1_sort_kernel<true, false><<<bgrid(nb, B), kB1SortThreads, sizeof(B1Smem), st>>>(
+            pairs, cursor, base, overflow, klo, idx_out, sorted_out, (uint32_t)N, nb, B, *wb, B1Tab())));
         AGN_LAUNCH(K_GATHER_BACK, st, (gather_back_kernel<<<bgrid((unsigned)(N / kB1Tile), B), kB1GatherThreads, 0, st>>>(
             wb->loc, wb->jrec, wb->valslab, overflow, wb->x_out, (uint32_t)N, nb, B)));
     } else {
-        AGN_LAUNCH(K_SORT_BUCKET, st, (bucket1_sort_kernel<false><<<bgrid(nb, B), kB1SortThreads, sizeof(B1Smem), st>>>(
-            pairs, cursor, base, overflow, klo, idx_out, sorted_out, (uint32_t)N, nb, B, B1Wb())));
+        B1Tab tb;
+        tb.tab = tab; tb.M = M; tb.bl = bl;
+        if (N < (1ll << 20))
+            AGN_LAUNCH(K_SORT_BUCKET, st, (bucket1_sort_kernel<false, true><<<bgrid(nb, B), kB1SortThreads, sizeof(B1Smem), st>>>(
+                pairs, cursor, base, overflow, klo, idx_out, sorted_out, (uint32_t)N, nb, B, B1Wb(), tb)));
+        else
+            AGN_LAUNCH(K_SORT_BUCKET, st, (bucket1_sort_kernel<false, false><<<bgrid(nb, B), kB1SortThreads, sizeof(B1Smem), st>>>(
+                pairs, cursor, base, overflow, klo, idx_out, sorted_out, (uint32_t)N, nb, B, B1Wb(), tb)));
     }
     *overflow_out = overflow;
     return cudaGetLastError();

@@ -44,10 +44,18 @@ constexpr int kBkSlots = 1 << kBkSlotLog;         // interpolation slots of the 
 // The table holds (cumw << 7, w), so that pos >> 9 = tab.x + ((low16 * w) >> 9) fits 32 bits, and
 // bs = bucket << 11 | slot = floor((pos >> 9) * M / 2^32) with M = floor(2^32 * nb * 2048 * 512 / (total * 2^16)):
 // one multiply-high.  Every step is monotone in the key, and equal keys get equal bs.
-constexpr unsigned long long kBkTotalW = (1ull << 24) + (1ull << 16);
-__device__ __forceinline__ uint32_t bs_of(uint32_t key, const uint2* __restrict__ tab, uint32_t M) {
-    const uint2 e = __ldg(tab + (key >> (32 - kBkBinLog)));
-    const uint32_t pos = e.x + (uint32_t)(((unsigned long long)(key & (kBkBins - 1)) * e.y) >> 9);
+// The number of bins follows the curve length (bl = log2 of it, 11 .. 16: a short curve has few buckets to tell apart,
+// and a 65536-bin table per curve would cost more than its sort): bin = top bl key bits, the low 32 - bl bits
+// interpolate, add-one mass 2^bl, pos >> (25 - bl) = tab.x + ((low * w) >> (25 - bl)); tab.x = cumw << 7 for every bl.
+constexpr unsigned long long kBkTotalW = (1ull << 24) + (1ull << 16);       // bl = 16
+__host__ __device__ constexpr unsigned long long bk_total_w(int bl) { return (1ull << 24) + (1ull << bl); }
+inline int bk_binlog(long long N) {
+    const int l = ilog2_u64((uint64_t)N) - 4;
+    return l < 11 ? 11 : (l > kBkBinLog ? kBkBinLog : l);
+}
+__device__ __forceinline__ uint32_t bs_of(uint32_t key, const uint2* __restrict__ tab, uint32_t M, int bl = kBkBinLog) {
+    const uint2 e = __ldg(tab + (key >> (32 - bl)));
+    const uint32_t pos = e.x + (uint32_t)(((unsigned long long)(key & ((1u << (32 - bl)) - 1u)) * e.y) >> (25 - bl));
     return __umulhi(pos, M);
 }
 inline uint32_t bucket32_magic(uint32_t nb) {
@@ -55,18 +63,18 @@ inline uint32_t bucket32_magic(uint32_t nb) {
 }
 
 __global__ void __launch_bounds__(256) cdf_sample_kernel(const float* __restrict__ vals, uint32_t* __restrict__ hist,
-                                                         uint32_t N, long long B) {
+                                                         uint32_t N, long long B, int bl = kBkBinLog) {
     const long long b = bidx();
     if (b >= B) return;
     const uint32_t i = blockIdx.x * 256 + threadIdx.x;          // sample number
     const bool in = i < (N >> kBkSampleLog);
     // the sample of block i of 64 keys sits at a position that varies with i (no fixed phase)
     const uint32_t e = (i << kBkSampleLog) + ((i * 0x9E3779B1u) >> (32 - kBkSampleLog));
-    const uint32_t bin = in ? (key_of(vals[(size_t)b * N + e]) >> (32 - kBkBinLog)) : 0xffffffffu;
+    const uint32_t bin = in ? (key_of(vals[(size_t)b * N + e]) >> (32 - bl)) : 0xffffffffu;
     // neighbouring samples of a smooth series share their bin: one atomic per distinct bin and warp
     const uint32_t peers = __match_any_sync(0xffffffffu, bin);
     if (in && (threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1))
-        atomicAdd(&hist[(size_t)b * kBkBins + bin], (uint32_t)__popc(peers));
+        atomicAdd(&hist[((size_t)b << bl) + bin], (uint32_t)__popc(peers));
 }
 
 // tab[bin] = (exclusive cumulative weight << 7, weight), weight = (cnt << logK) + 1.  kCdfChunks CTAs per curve, each
@@ -107,12 +115,14 @@ __device__ __forceinline__ uint32_t block_excl_scan_1024(uint32_t v, uint32_t* w
     *total = __shfl_sync(0xffffffffu, wi, 31);
     return inc - v + __shfl_sync(0xffffffffu, wi - w, warp);
 }
-__global__ void __launch_bounds__(1024) cdf_table_kernel(const uint32_t* __restrict__ hist, uint2* __restrict__ tab, int logK) {
+inline unsigned cdf_chunks(int bl) { return (1u << bl) >= 1024u * kCdfChunks ? (unsigned)kCdfChunks : (1u << bl) / 1024u; }
+__global__ void __launch_bounds__(1024) cdf_table_kernel(const uint32_t* __restrict__ hist, uint2* __restrict__ tab, int logK,
+                                                         int bl = kBkBinLog, uint32_t chunks = kCdfChunks) {
     __shared__ uint32_t ws[32];
-    const uint32_t curve = blockIdx.x / kCdfChunks, chunk = blockIdx.x % kCdfChunks;
-    const uint32_t* h = hist + (size_t)curve * kBkBins;
-    uint2* t = tab + (size_t)curve * kBkBins;
-    constexpr uint32_t PER = kBkBins / kCdfChunks;          // bins per chunk
+    const uint32_t curve = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
+    const uint32_t* h = hist + ((size_t)curve << bl);
+    uint2* t = tab + ((size_t)curve << bl);
+    const uint32_t PER = (1u << bl) / chunks;               // bins per chunk (a multiple of 1024)
     uint32_t before = 0;
     for (uint32_t i = threadIdx.x; i < chunk * PER; i += 1024) before += (h[i] << logK) + 1u;
     uint32_t run = block_sum_1024(before, ws);
@@ -309,25 +319,26 @@ __global__ void __launch_bounds__(1024) bucket_base_kernel(const uint32_t* __res
 // [klo[k], klo[k+1]), so inside the finish kernel a slot is a plain linear map of the key onto that interval -- no
 // table look-up per key there.  One thread per bucket: invert umulhi(pos, M) >= k << kBkSlotLog, then the table.
 __global__ void __launch_bounds__(256) bucket_bounds_kernel(const uint2* __restrict__ tabs, uint32_t* __restrict__ klo,
-                                                            uint32_t nb, uint32_t M, int slot_log, long long B) {
+                                                            uint32_t nb, uint32_t M, int slot_log, long long B,
+                                                            int bl = kBkBinLog) {
     const long long b = bidx();
     if (b >= B) return;
     const uint32_t k = blockIdx.x * 256 + threadIdx.x;
     if (k > nb) return;
     uint32_t* out = klo + (size_t)b * (nb + 1);
     if (k == nb) { out[k] = 0xffffffffu; return; }
-    const uint2* tab = tabs + (size_t)b * kBkBins;
+    const uint2* tab = tabs + ((size_t)b << bl);
     const unsigned long long want = ((unsigned long long)k << slot_log) << 32;
     const unsigned long long P = (want + M - 1) / M;               // smallest pos32 with umulhi(pos32, M) >= k << slotlog
-    uint32_t lo = 0, hi = kBkBins - 1;                              // largest bin with tab[bin].x <= P
+    uint32_t lo = 0, hi = (1u << bl) - 1u;                          // largest bin with tab[bin].x <= P
     while (lo < hi) {
         const uint32_t mid = (lo + hi + 1) >> 1;
         if ((unsigned long long)tab[mid].x <= P) lo = mid; else hi = mid - 1;
     }
     const uint2 e = tab[lo];
-    const unsigned long long need = (P - e.x) << 9;                 // low16 * w >= need
-    const unsigned long long low = min((need + e.y - 1) / e.y, (unsigned long long)(kBkBins - 1));
-    out[k] = (lo << kBkBinLog) | (uint32_t)low;
+    const unsigned long long need = (P - e.x) << (25 - bl);         // low * w >= need
+    const unsigned long long low = min((need + e.y - 1) / e.y, (unsigned long long)((1u << (32 - bl)) - 1u));
+    out[k] = (lo << (32 - bl)) | (uint32_t)low;
 }
 
 struct BkSmem {
