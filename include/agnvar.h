@@ -15,9 +15,10 @@
  *   - Every call returns an agnvar_status; nothing throws or aborts.  AGNVAR_EINVAL is returned
  *     before any launch.  AGNVAR_ECUDA wraps a failed launch (sticky CUDA errors are not cleared).
  *   - Arrays are row-major [B][N], one light curve contiguous.  N is a power of two,
- *     4 <= N <= 2^28 (the paper's own cap is 2^27, "set by memory limitations"; a 180 GB B200 holds
- *     the loop's working set well beyond it, and 2^28 is what the generic three-pass FFT reaches).  The fastest
- *     paths cover fp32 up to 2^26 (one-level distribution sort) and 2^27 (register column FFT, two-level sort).
+ *     4 <= N <= 2^30 (the paper's own cap is 2^27, "set by memory limitations"; a 180 GB B200 holds
+ *     the loop's working set, ~45 bytes per sample, well beyond it).  The fastest paths cover fp32 up to 2^26
+ *     (one-level distribution sort) and 2^27 (register column FFT, two-level sort); longer series run through the
+ *     generic three-pass FFT and the LSD sort.
  *   - dtype selects the arithmetic AND storage type of series, spectra and sort keys (float or
  *     double).  PSD values, the ERDF table and the inverse-CDF arithmetic are always fp64.
  *   - Random numbers: Philox4x32-10, key = (seed lo, seed hi), counter = (i lo, i hi, curve b, tag);

@@ -34,7 +34,7 @@ struct Carver {
 
 inline bool is_pow2(int64_t n) { return n > 0 && (n & (n - 1)) == 0; }
 inline bool valid_BN(int64_t B, int64_t N) {
-    return B >= 1 && B <= (int64_t)1 << 30 && is_pow2(N) && N >= 4 && N <= ((int64_t)1 << 28);
+    return B >= 1 && B <= (int64_t)1 << 30 && is_pow2(N) && N >= 4 && N <= ((int64_t)1 << 30);
 }
 inline bool valid_dtype(int d) { return d == AGNVAR_F32 || d == AGNVAR_F64; }
 inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
@@ -619,7 +619,7 @@ size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int overs
     switch (op) {
         case AGNVAR_OP_E13_ITERATE: return f32 ? ws_e13<float>(B, N, aux != 0) : ws_e13<double>(B, N, aux != 0);
         case AGNVAR_OP_TK_GENERATE:
-            if (!valid_oversample(oversample) || N * (int64_t)oversample > ((int64_t)1 << 28)) return 0;
+            if (!valid_oversample(oversample) || N * (int64_t)oversample > ((int64_t)1 << 30)) return 0;
             return f32 ? ws_tk<float>(B, N, oversample) : ws_tk<double>(B, N, oversample);
         case AGNVAR_OP_ERDF_SAMPLE_SORTED:
             if (aux < 2 || aux > 65536) return 0;
@@ -752,7 +752,7 @@ int agnvar_tk_generate(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_
             !std::isfinite(p.alpha_high))
             return AGNVAR_EINVAL;
     }
-    if (N * (int64_t)oversample > ((int64_t)1 << 28)) return AGNVAR_EUNSUPPORTED;
+    if (N * (int64_t)oversample > ((int64_t)1 << 30)) return AGNVAR_EUNSUPPORTED;
     if (dtype == AGNVAR_F32)
         return tk_impl<float>(h_psd, n_psd, B, N, dt, oversample, seed, curve0, d_xnorm, d_anorm, d_ws, ws_bytes,
                               (cudaStream_t)stream);

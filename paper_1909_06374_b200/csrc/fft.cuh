@@ -17,7 +17,8 @@
 namespace agn {
 
 constexpr int kLogTw = 14;        // fine table: exp(-2 pi i m / 2^14)
-constexpr int kLogLo = 14;        // per-level low table: exp(-2 pi i l / D), l < 2^14 (levels up to D = 2^28: the real-FFT level of N = 2^28)
+constexpr int kLogLo = 16;        // per-level low table: room for exp(-2 pi i l / D), l < 2^16; a level uses its first 2^lo_bits(logD) entries
+__host__ __device__ __forceinline__ int lo_bits(int logD) { return logD - kLogTw > 13 ? logD - kLogTw : 13; }   // levels up to D = 2^30
 constexpr int kMaxPass = 3;
 constexpr int kFftThreads = 512;
 
@@ -52,19 +53,20 @@ __host__ __device__ __forceinline__ uint32_t k2pos(const Digits& d, uint32_t k) 
     return pos;
 }
 
-// Twiddle level: w_D^idx = exp(-2 pi i idx / D), D = 2^logD <= 2^27, idx < D/2... (any idx < D).
+// Twiddle level: w_D^idx = exp(-2 pi i idx / D), D = 2^logD <= 2^30, any idx < D.
 template <typename T> struct TwLevel {
     const typename Cx<T>::type* tw14;   // exp(-2 pi i m / 2^14)
-    const typename Cx<T>::type* lo;     // exp(-2 pi i l / D), l < 2^kLogLo (only if logD > kLogTw)
+    const typename Cx<T>::type* lo;     // exp(-2 pi i l / D), l < 2^lo_bits(logD) (only if logD > kLogTw)
     int logD;
 };
 
 template <typename T>
 __device__ __forceinline__ typename Cx<T>::type tw_lookup(const TwLevel<T>& lv, uint32_t idx) {
     if (lv.logD <= kLogTw) return lv.tw14[idx << (kLogTw - lv.logD)];
-    uint32_t h = idx >> kLogLo, l = idx & ((1u << kLogLo) - 1u);
-    // exp(-2 pi i h 2^kLogLo / D) = tw14[h * 2^kLogTw * 2^kLogLo / D]
-    return cmul(lv.tw14[h << (kLogTw + kLogLo - lv.logD)], lv.lo[l]);
+    const int lb = lo_bits(lv.logD);            // 13 up to D = 2^27 (64 KB of low table), logD - 14 above
+    uint32_t h = idx >> lb, l = idx & ((1u << lb) - 1u);
+    // exp(-2 pi i h 2^lb / D) = tw14[h * 2^kLogTw * 2^lb / D]
+    return cmul(lv.tw14[h << (kLogTw + lb - lv.logD)], lv.lo[l]);
 }
 
 // table init: out[m] = exp(-2 pi i m / 2^logD), m < n
