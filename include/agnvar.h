@@ -18,7 +18,7 @@
  *     4 <= N <= 2^30 (the paper's own cap is 2^27, "set by memory limitations"; a 180 GB B200 holds
  *     the loop's working set, ~45 bytes per sample, well beyond it).  The fastest paths cover fp32 up to 2^26
  *     (one-level distribution sort) and 2^27 (register column FFT, two-level sort); longer series run through the
- *     generic three-pass FFT and the LSD sort.
+ *     generic three-pass FFT and the LSD sort.  fp64: N (and oversample * N) <= 2^27; beyond that AGNVAR_EUNSUPPORTED.
  *   - dtype selects the arithmetic AND storage type of series, spectra and sort keys (float or
  *     double).  PSD values, the ERDF table and the inverse-CDF arithmetic are always fp64.
  *   - Random numbers: Philox4x32-10, key = (seed lo, seed hi), counter = (i lo, i hi, curve b, tag);
@@ -41,7 +41,7 @@ typedef enum {
     AGNVAR_EINVAL = 1,       /* bad argument (see each call) */
     AGNVAR_EWORKSPACE = 2,   /* ws_bytes too small or d_ws NULL / misaligned */
     AGNVAR_ECUDA = 3,        /* a CUDA launch or API call failed */
-    AGNVAR_EUNSUPPORTED = 4  /* valid request this build does not implement (e.g. oversample*N > 2^28) */
+    AGNVAR_EUNSUPPORTED = 4  /* valid request this build does not implement (oversample*N > 2^30; fp64 beyond 2^27) */
 } agnvar_status;
 
 typedef enum { AGNVAR_F32 = 0, AGNVAR_F64 = 1 } agnvar_dtype;
@@ -154,7 +154,7 @@ int agnvar_erdf_table(const agnvar_erdf* h_erdf, int64_t n_erdf, int grid_points
  *   d_xnorm     out [B][N] dtype or NULL
  *   d_anorm     out [B][N/2+1] dtype or NULL
  * EINVAL: bad B/N/dtype/oversample, n_psd not 1 or B, dt <= 0, f_b <= 0, non-finite parameter,
- * NULL h_psd, both outputs NULL.  EUNSUPPORTED: oversample * N > 2^28. */
+ * NULL h_psd, both outputs NULL.  EUNSUPPORTED: oversample * N > 2^30 (fp64: 2^27). */
 int agnvar_tk_generate(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_t N, double dt, int oversample,
                        int dtype, uint64_t seed, uint32_t curve0, void* d_xnorm, void* d_anorm, void* d_ws,
                        size_t ws_bytes, void* stream);

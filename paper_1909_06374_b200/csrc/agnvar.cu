@@ -37,6 +37,9 @@ inline bool valid_BN(int64_t B, int64_t N) {
     return B >= 1 && B <= (int64_t)1 << 30 && is_pow2(N) && N >= 4 && N <= ((int64_t)1 << 30);
 }
 inline bool valid_dtype(int d) { return d == AGNVAR_F32 || d == AGNVAR_F64; }
+// the generic FFT plan has three passes: 2^29 complex points in fp32 (8192-point tiles), 2^26 in fp64 (4096-point tiles);
+// sizes above that are refused (AGNVAR_EUNSUPPORTED), never silently wrong
+inline bool size_supported(int dtype, int64_t len) { return len <= (dtype == AGNVAR_F64 ? ((int64_t)1 << 27) : ((int64_t)1 << 30)); }
 inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
 inline bool valid_oversample(int o) { return o == 1 || o == 2 || o == 4 || o == 8 || o == 10 || o == 16 || o == 20; }
 
@@ -614,12 +617,12 @@ int agnvar_trace_end(int64_t cap, int32_t* h_ids, float* h_ms, int64_t* h_n) {
 const char* agnvar_kernel_name(int id) { return (id >= 0 && id < K_NIDS) ? kKernelNames[id] : nullptr; }
 
 size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int oversample, int64_t aux) {
-    if (!valid_BN(B, N) || !valid_dtype(dtype)) return 0;
+    if (!valid_BN(B, N) || !valid_dtype(dtype) || !size_supported(dtype, N)) return 0;
     const bool f32 = dtype == AGNVAR_F32;
     switch (op) {
         case AGNVAR_OP_E13_ITERATE: return f32 ? ws_e13<float>(B, N, aux != 0) : ws_e13<double>(B, N, aux != 0);
         case AGNVAR_OP_TK_GENERATE:
-            if (!valid_oversample(oversample) || N * (int64_t)oversample > ((int64_t)1 << 30)) return 0;
+            if (!valid_oversample(oversample) || !size_supported(dtype, N * (int64_t)oversample)) return 0;
             return f32 ? ws_tk<float>(B, N, oversample) : ws_tk<double>(B, N, oversample);
         case AGNVAR_OP_ERDF_SAMPLE_SORTED:
             if (aux < 2 || aux > 65536) return 0;
@@ -705,6 +708,7 @@ int agnvar_erdf_sample_sorted(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_t
                               uint64_t seed, uint32_t curve0, int grid_points, void* d_sorted, uint32_t* d_perm0,
                               void* d_draw, void* d_ws, size_t ws_bytes, void* stream) {
     if (!valid_BN(B, N) || !valid_dtype(dtype) || !h_erdf || !d_sorted) return AGNVAR_EINVAL;
+    if (!size_supported(dtype, N)) return AGNVAR_EUNSUPPORTED;
     if (!(n_erdf == 1 || n_erdf == B) || grid_points < 2 || grid_points > 65536) return AGNVAR_EINVAL;
     if (!valid_erdf(h_erdf, n_erdf)) return AGNVAR_EINVAL;
     size_t need = agnvar_workspace_bytes(AGNVAR_OP_ERDF_SAMPLE_SORTED, B, N, dtype, 1, grid_points);
@@ -722,6 +726,7 @@ int agnvar_slice_sample_sorted(const agnvar_erdf* h_erdf, int64_t n_erdf, int64_
                                uint64_t seed, uint32_t curve0, const agnvar_slice_opts* h_opts, void* d_sorted,
                                uint32_t* d_perm0, void* d_draw, void* d_ws, size_t ws_bytes, void* stream) {
     if (!valid_BN(B, N) || !valid_dtype(dtype) || !h_erdf || !d_sorted || !h_opts) return AGNVAR_EINVAL;
+    if (!size_supported(dtype, N)) return AGNVAR_EUNSUPPORTED;
     if (!(n_erdf == 1 || n_erdf == B) || !valid_erdf(h_erdf, n_erdf, true)) return AGNVAR_EINVAL;
     const agnvar_slice_opts& o = *h_opts;
     if (o.chains < 1 || o.chains > ((int64_t)1 << 32) || N % o.chains != 0 || o.burn_in < 0 || o.thin < 1 || o.max_steps < 1 ||
@@ -752,7 +757,7 @@ int agnvar_tk_generate(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_
             !std::isfinite(p.alpha_high))
             return AGNVAR_EINVAL;
     }
-    if (N * (int64_t)oversample > ((int64_t)1 << 30)) return AGNVAR_EUNSUPPORTED;
+    if (!size_supported(dtype, N * (int64_t)oversample)) return AGNVAR_EUNSUPPORTED;
     if (dtype == AGNVAR_F32)
         return tk_impl<float>(h_psd, n_psd, B, N, dt, oversample, seed, curve0, d_xnorm, d_anorm, d_ws, ws_bytes,
                               (cudaStream_t)stream);
@@ -764,6 +769,7 @@ int agnvar_e13_iterate(int64_t B, int64_t N, int dtype, const void* d_anorm, con
                        void* d_x, int max_iter, int32_t* d_iters_used, int64_t* d_changed_hist, void* d_xadj_dbg,
                        const agnvar_e13_opts* h_opts, void* d_ws, size_t ws_bytes, void* stream) {
     if (!valid_BN(B, N) || !valid_dtype(dtype) || max_iter < 1) return AGNVAR_EINVAL;
+    if (!size_supported(dtype, N)) return AGNVAR_EUNSUPPORTED;
     if (!d_anorm || !d_sorted || !d_perm || !d_x) return AGNVAR_EINVAL;
     if (!aligned(d_perm, 16) || !aligned(d_x, 16) || !aligned(d_sorted, 16)) return AGNVAR_EINVAL;
     E13Opts opt;
@@ -839,6 +845,7 @@ int agnvar_periodogram(int64_t B, int64_t N, int dtype, const void* d_x, double 
     if (!valid_BN(B, N) || !valid_dtype(dtype) || !d_x || !d_out) return AGNVAR_EINVAL;
     if (!(norm == 0 || norm == 1) || !(dt > 0.0) || !std::isfinite(dt) || nbins < 0 || nbins > 4096) return AGNVAR_EINVAL;
     if (!aligned(d_x, 16)) return AGNVAR_EINVAL;
+    if (!size_supported(dtype, N)) return AGNVAR_EUNSUPPORTED;
     if (nbins > 0) {
         if (!h_bin_edges_j) return AGNVAR_EINVAL;
         if (h_bin_edges_j[0] < 1 || h_bin_edges_j[nbins] > N / 2 + 1) return AGNVAR_EINVAL;

@@ -163,11 +163,12 @@ def test_maximum_size_2p27(orc):
     ag.free_workspace()
 
 
-@pytest.mark.parametrize("logn", [28, 30])
-def test_beyond_the_papers_cap(orc, logn):
+@pytest.mark.parametrize("logn,dtype", [(28, "f32"), (30, "f32"), (27, "f64")])
+def test_beyond_the_papers_cap(orc, logn, dtype):
     """N = 2^28 and 2^30 (the largest series the ABI accepts), 2x and 8x the paper's maximum (2^27, "set
     by memory limitations"), one curve, fp32, through the generic three-pass FFT (twiddle levels up to 2^30), the LSD
-    sort and the two-level scatter.  The oracle cannot redo a step of this size in test time, so the checks are: the properties that pin L4-L6 at any size (exact); the FFT / replace / IFFT chain
+    sort and the two-level scatter; and fp64 at its own maximum, 2^27.  The oracle cannot redo a step of this size in
+    test time, so the checks are: the properties that pin L4-L6 at any size (exact); the FFT / replace / IFFT chain
     against a library FFT in fp64 (torch.fft on the GPU's own arrays): |rfft(x_adj)| = A_norm and the phases of x_adj
     are those of x_sim; S2 by sampled Fourier coefficients of x_norm against the oracle's normals and Eq. 3."""
     import paper_1909_06374_b200 as ag
@@ -175,7 +176,7 @@ def test_beyond_the_papers_cap(orc, logn):
     cfg = workloads.config("C4", B=1)
     N, p, seed, dt = 2 ** logn, cfg["psd"][0], cfg["seed"], cfg["dt"]
     # ---- S2
-    xn, an = ag.agnvar_tk_generate(cfg["psd"], 1, N, dt, 1, "f32", seed, 0)
+    xn, an = ag.agnvar_tk_generate(cfg["psd"], 1, N, dt, 1, dtype, seed, 0)
     X = torch.fft.rfft(xn[0].double())
     rel_a = float(torch.linalg.norm(X.abs() - an[0].double()) / torch.linalg.norm(an[0].double()))
     A = orc.psd_unit_variance_A(N, dt, p["f_b"], p["alpha_low"], p["alpha_high"])
@@ -187,11 +188,12 @@ def test_beyond_the_papers_cap(orc, logn):
     got = X[torch.tensor(js, device="cuda")].cpu().numpy()
     rel_x = float(np.linalg.norm(got - want) / np.linalg.norm(want))
     print(f"N=2^{logn} S2: |rfft(x_norm)| vs A_norm rel L2 {rel_a:.2e}; {js.size} sampled coefficients vs the oracle rel L2 {rel_x:.2e}")
-    assert rel_a <= 1e-5 and rel_x <= 1e-4
+    tol = 1e-5 if dtype == "f32" else 1e-12
+    assert rel_a <= tol and rel_x <= 10 * tol
     del X, xn
     torch.cuda.empty_cache()
     # ---- S1 + two iterations
-    srt, perm, _ = ag.agnvar_erdf_sample_sorted(cfg["erdf"], 1, N, "f32", seed, 0, cfg["grid_points"])
+    srt, perm, _ = ag.agnvar_erdf_sample_sorted(cfg["erdf"], 1, N, dtype, seed, 0, cfg["grid_points"])
     assert bool((srt[:, 1:] >= srt[:, :-1]).all())
     o = ag.agnvar_e13_iterate(an, srt, perm, 1)
     perm_prev, x_prev = perm.clone(), o["x"].clone()
@@ -220,5 +222,5 @@ def test_beyond_the_papers_cap(orc, logn):
     ref = an[0].double() * Xs / Xs.abs().clamp_min(1e-300)
     rel_ph = float(torch.linalg.norm(Xa - ref) / torch.linalg.norm(ref))
     print(f"N=2^{logn} E13 step: amplitudes rel L2 {rel_amp:.2e}, spectrum (amplitude replaced, phase kept) rel L2 {rel_ph:.2e}")
-    assert rel_amp <= 1e-5 and rel_ph <= 1e-5
+    assert rel_amp <= tol and rel_ph <= tol
     ag.free_workspace()

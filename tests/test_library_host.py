@@ -39,6 +39,7 @@ def test_workspace_query_and_validation(L):
     assert b.workspace_bytes(b.OP_E13_ITERATE, 4, 2, "f32") == 0
     assert b.workspace_bytes(b.OP_E13_ITERATE, 1, 2 ** 30, "f32") > 2 ** 30 * 4 * 4     # the largest series accepted
     assert b.workspace_bytes(b.OP_E13_ITERATE, 1, 2 ** 31, "f32") == 0
+    assert b.workspace_bytes(b.OP_E13_ITERATE, 1, 2 ** 27, "f64") > 0 and b.workspace_bytes(b.OP_E13_ITERATE, 1, 2 ** 28, "f64") == 0
     assert b.workspace_bytes(b.OP_TK_GENERATE, 4, 4096, "f64", 3) == 0
     assert b.workspace_bytes(b.OP_TK_GENERATE, 4, 4096, "f64", 10) > 0
     assert b.workspace_bytes(b.OP_ERDF_SAMPLE_SORTED, 4, 4096, "f64", 1, 1) == 0
@@ -51,6 +52,8 @@ def test_workspace_query_and_validation(L):
     assert L.agnvar_tk_generate(C.byref(good), 1, 1, 1000, 1.0, 1, 0, 0, 0, one, one, one, 1 << 40, None) == 1
     assert L.agnvar_tk_generate(C.byref(good), 1, 1, 1024, 1.0, 1, 0, 0, 0, None, None, one, 1 << 40, None) == 1
     assert L.agnvar_tk_generate(C.byref(good), 1, 1, 2 ** 29, 1.0, 4, 0, 0, 0, one, one, one, 1 << 40, None) == 4
+    assert L.agnvar_tk_generate(C.byref(good), 1, 1, 2 ** 28, 1.0, 1, 1, 0, 0, one, one, one, 1 << 40, None) == 4      # fp64 beyond 2^27
+    assert L.agnvar_e13_iterate(1, 2 ** 28, 1, one, one, one, one, 1, None, None, None, None, one, 1 << 40, None) == 4
     assert L.agnvar_e13_iterate(1, 1024, 0, one, one, one, one, 0, None, None, None, None, one, 1 << 40, None) == 1
     assert L.agnvar_e13_iterate(1, 1024, 7, one, one, one, one, 1, None, None, None, None, one, 1 << 40, None) == 1
     assert L.agnvar_e13_iterate(1, 1024, 0, one, one, one, one, 1, None, None, None, None, one, 16, None) == 2
