@@ -472,7 +472,7 @@ template <typename T> struct Fft2Plan {
     }
 };
 
-inline bool fft2_applicable(size_t elem_size, int logL) { return elem_size == 4 && logL >= kLogR1 + 1 && logL <= kLogR1 + 13; }
+inline bool fft2_applicable(size_t elem_size, int logL) { return elem_size == 4 && logL >= kLogR1 + 1 && logL <= kLogR1 + 16; }   // N = 2^15 .. 2^30 (three column phases of radix <= 64 reach R0 = 2^18)
 
 template <typename T>
 inline Fft2Plan<T> fft2_plan_init(int logL, typename Cx<T>::type* tables, unsigned int* counters, cudaStream_t st) {
