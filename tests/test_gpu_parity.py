@@ -321,7 +321,7 @@ def test_e13_ties_and_zero_amplitude(ag, orc):
         assert out["changed_hist"][b, 0].item() == np.count_nonzero(pnew[b] != perm0[b])
 
 
-@pytest.mark.parametrize("N", [2 ** 18, 2 ** 22])
+@pytest.mark.parametrize("N", [2 ** 15, 2 ** 18, 2 ** 22])
 @pytest.mark.parametrize("case", ["red_noise", "quantised", "all_equal", "one_outlier", "mixed", "tone64", "tone4096",
                                   "red_plus_tone"])
 def test_long_curve_argsort_paths(ag, orc, N, case):
@@ -370,8 +370,9 @@ def test_long_curve_argsort_paths(ag, orc, N, case):
         assert out["changed_hist"][b, 0].item() == np.count_nonzero(pnew[b] != perm0[b])
     if case in ("red_noise", "mixed", "quantised"):
         fb = out["sort_fallbacks"].cpu().numpy()
-        assert fb[0] == (1 if case == "quantised" else 0)
-        assert fb[1] == (0 if case == "red_noise" else 1)
+        overflows = N // 8 > 12288        # "quantised": 8 distinct values, N/8 copies each, against the slab capacity
+        assert fb[0] == (1 if case == "quantised" and overflows else 0)
+        assert fb[1] == (0 if case == "red_noise" or not overflows else 1)
 
 
 # ---- boundary behaviour ---------------------------------------------------------------------------
