@@ -41,7 +41,8 @@ typedef enum {
     AGNVAR_EINVAL = 1,       /* bad argument (see each call) */
     AGNVAR_EWORKSPACE = 2,   /* ws_bytes too small or d_ws NULL / misaligned */
     AGNVAR_ECUDA = 3,        /* a CUDA launch or API call failed */
-    AGNVAR_EUNSUPPORTED = 4  /* valid request this build does not implement (oversample*N > 2^30; fp64 beyond 2^27) */
+    AGNVAR_EUNSUPPORTED = 4, /* valid request this build does not implement (oversample*N > 2^30; fp64 beyond 2^27) */
+    AGNVAR_ESTATIC_LIMIT = 5 /* agnvar_structure_function_static only: the request needs more than the built-in array */
 } agnvar_status;
 
 typedef enum { AGNVAR_F32 = 0, AGNVAR_F64 = 1 } agnvar_dtype;
@@ -233,6 +234,45 @@ int agnvar_periodogram(int64_t B, int64_t N, int dtype, const void* d_x, double 
 int agnvar_structure_function(int64_t B, int64_t N, int dtype, const void* d_x, const int64_t* h_lags, int nlags, int mag,
                               double* d_sf2, int64_t* d_pairs, double* d_rep_mean, double* d_rep_stderr, void* d_ws,
                               size_t ws_bytes, void* stream);
+
+/* SF without a workspace -- agnvar_structure_function for callers that cannot hand the library any scratch memory.
+ *
+ * Who this is for.  Every other call here works in a buffer the caller allocates.  That is no help to code that cannot
+ * allocate on the device at all: a plug-in that is passed light curves and an output slot and nothing else; a process
+ * whose device memory was handed over wholesale to another component's memory pool when it started, so that a fresh
+ * cudaMalloc either fails or takes what someone else budgeted; a loop with a latency bound that cannot absorb the
+ * device-wide stall an allocation may bring.  For those callers this one entry point keeps its scratch (the lags, the
+ * per-chunk partial sums and, for mag = 1, the magnitudes) in an array that is compiled into the library.  It calls no
+ * cudaMalloc, no cudaFree, no host-to-device copy and no routine that allocates; the caller passes the input and the
+ * output arrays exactly as for agnvar_structure_function (same meaning, same results bit for bit: the same kernels run).
+ *
+ * The limit.  The array is AGNVAR_STATIC_SCRATCH_BYTES = 8 MiB, and every GPU on which the library's code is loaded
+ * holds those 8 MiB until the process ends whether or not this call is ever used.  A request fits when
+ *   agnvar_structure_function_static_bytes(B, N, nlags, mag) <= agnvar_static_scratch_bytes(),
+ * i.e. 256-byte-rounded  8 nlags + (mag ? 8 B N : 0) + 8 B nlags ceil(N / 8192),  and nlags <= AGNVAR_STATIC_MAX_LAGS
+ * (the lags travel as a kernel argument).  Examples that fit: mag = 0, B = 64 curves of 2^20 samples at 64 lags
+ * (4 MiB); mag = 1, B N up to about 10^6 samples.  Anything larger returns AGNVAR_ESTATIC_LIMIT before any launch: use
+ * agnvar_structure_function with a workspace instead.
+ *
+ * First call.  The first call on each device looks up the array's address on that device (the device that is current
+ * when the call is made) and remembers it; that look-up may make the CUDA runtime load the library's code onto the
+ * device.  Make this first call during start-up, outside any stream capture; later calls only enqueue kernels.
+ *
+ * Sharing.  There is one array per device and every call on that device uses it.  Two calls whose kernels can overlap
+ * on the GPU (different streams, or different host threads without ordering between them) overwrite each other's
+ * partial sums and return garbage: order such calls on one stream or with events.  Calls on one stream are safe back
+ * to back.  Whatever a call leaves in the array is never read by the next one (each call writes all it reads), so
+ * nothing needs clearing between calls.
+ *
+ * Returns: AGNVAR_EINVAL as agnvar_structure_function; AGNVAR_ESTATIC_LIMIT (nlags or the scratch need above the
+ * limit); AGNVAR_ECUDA when the address look-up or a launch fails. */
+#define AGNVAR_STATIC_SCRATCH_BYTES (8u << 20)
+#define AGNVAR_STATIC_MAX_LAGS 256
+size_t agnvar_static_scratch_bytes(void);
+size_t agnvar_structure_function_static_bytes(int64_t B, int64_t N, int nlags, int mag);   /* 0 for invalid arguments */
+int agnvar_structure_function_static(int64_t B, int64_t N, int dtype, const void* d_x, const int64_t* h_lags, int nlags,
+                                     int mag, double* d_sf2, int64_t* d_pairs, double* d_rep_mean, double* d_rep_stderr,
+                                     void* stream);
 
 /* dM -- P(|dm| > dm_ref given tau) (Figs 16-17): per curve and lag, the number of pairs (i, i + l)
  * with |m_i - m_{i+l}| > dm_ref divided by the number of pairs considered, m = m_zero - 2.5 log10 x (fp64).

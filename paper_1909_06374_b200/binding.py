@@ -23,6 +23,7 @@ EXPORTS = (
     "agnvar_launch_count", "agnvar_trace_begin", "agnvar_trace_end", "agnvar_kernel_name",
     "agnvar_structure_function", "agnvar_delta_m_prob", "agnvar_ensemble_sf", "agnvar_moments",
     "agnvar_slice_sample_sorted",
+    "agnvar_static_scratch_bytes", "agnvar_structure_function_static_bytes", "agnvar_structure_function_static",
 )
 
 
@@ -93,6 +94,12 @@ def lib():
     L.agnvar_periodogram.argtypes = [i64, i64, i32, vp, dbl, i32, i32, C.POINTER(i64), vp, vp, vp, sz, vp]
     L.agnvar_structure_function.restype = i32
     L.agnvar_structure_function.argtypes = [i64, i64, i32, vp, C.POINTER(i64), i32, i32, vp, vp, vp, vp, vp, sz, vp]
+    L.agnvar_static_scratch_bytes.restype = sz
+    L.agnvar_static_scratch_bytes.argtypes = []
+    L.agnvar_structure_function_static_bytes.restype = sz
+    L.agnvar_structure_function_static_bytes.argtypes = [i64, i64, i32, i32]
+    L.agnvar_structure_function_static.restype = i32
+    L.agnvar_structure_function_static.argtypes = [i64, i64, i32, vp, C.POINTER(i64), i32, i32, vp, vp, vp, vp, vp]
     L.agnvar_delta_m_prob.restype = i32
     L.agnvar_delta_m_prob.argtypes = [i64, i64, i32, vp, C.POINTER(i64), i32, C.POINTER(dbl), i32, dbl, i32, dbl, vp, vp,
                                       vp, sz, vp]
@@ -383,6 +390,56 @@ def agnvar_structure_function(x, lags, mag=False, want_rep=False):
                                                _ptr(mean), _ptr(se), _ptr(ws), ws.numel(), _stream()),
                "agnvar_structure_function")
     return {"sf2": sf2, "pairs": pairs, "rep_mean": mean, "rep_stderr": se}
+
+
+AGNVAR_ESTATIC_LIMIT = 5
+
+
+def agnvar_structure_function_static(x, lags, mag=False, want_rep=False, out=None):
+    """agnvar_structure_function for a caller that has no scratch memory to offer (include/agnvar.h, "SF without a
+    workspace").
+
+    Use it where device allocation is not an option -- a plug-in that only receives tensors, a process whose device
+    memory already belongs to somebody else's pool, a loop that cannot afford the stall an allocation may cause.  The
+    library then works in an 8 MiB array that is part of libagnvar.so (every GPU that loads the library holds it until
+    the process exits); this call allocates nothing on the device when `out` is given.
+
+    x [B][N] float32 / float64 on the GPU; at most 256 lags; the request must fit the array
+    (static_scratch_need(...) <= static_scratch_bytes(), e.g. 64 curves x 2^20 samples x 64 lags without magnitudes,
+    about 10^6 samples in total with mag=True) or AgnvarError(status AGNVAR_ESTATIC_LIMIT) is raised and nothing runs.
+    out: the dict a previous call returned (its tensors are overwritten), so that a caller that may not allocate can
+    create the outputs once at start-up; None lets torch allocate them.
+    Make the first call on each device at start-up (it looks up the array's device address).  All calls on a device
+    share the one array: keep them on one stream, or order them with events; calls that overlap on the GPU corrupt
+    each other's sums.  Results are identical to agnvar_structure_function's (same kernels)."""
+    B, N = x.shape
+    code, _ = _dt(x.dtype)
+    dev = x.device
+    nl = len(lags)
+    arr = (C.c_int64 * nl)(*[int(l) for l in lags])
+    with _on(dev):
+        if out is None:
+            out = {"sf2": torch.empty((B, nl), dtype=torch.float64, device=dev),
+                   "pairs": torch.empty((nl,), dtype=torch.int64, device=dev),
+                   "rep_mean": torch.empty((nl,), dtype=torch.float64, device=dev) if want_rep else None,
+                   "rep_stderr": torch.empty((nl,), dtype=torch.float64, device=dev) if want_rep else None}
+        elif tuple(out["sf2"].shape) != (B, nl) or out["pairs"].numel() != nl:
+            raise ValueError("out does not have the shapes of this request")
+        _check(lib().agnvar_structure_function_static(B, N, code, _ptr(x), arr, nl, 1 if mag else 0, _ptr(out["sf2"]),
+                                                      _ptr(out["pairs"]), _ptr(out["rep_mean"]), _ptr(out["rep_stderr"]),
+                                                      _stream()),
+               "agnvar_structure_function_static")
+    return out
+
+
+def static_scratch_bytes():
+    """Size of the array agnvar_structure_function_static works in (bytes held on every GPU that loads the library)."""
+    return int(lib().agnvar_static_scratch_bytes())
+
+
+def static_scratch_need(B, N, nlags, mag=False):
+    """Bytes of that array a request would use (0 for invalid arguments); it runs iff this is <= static_scratch_bytes()."""
+    return int(lib().agnvar_structure_function_static_bytes(int(B), int(N), int(nlags), 1 if mag else 0))
 
 
 def agnvar_delta_m_prob(x, lags, dm_ref, m_zero=0.0, m_cut=None):

@@ -15,6 +15,7 @@
 
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 using namespace agn;
@@ -575,6 +576,7 @@ const char* agnvar_strerror(int status) {
         case AGNVAR_EWORKSPACE: return "workspace too small, NULL or misaligned";
         case AGNVAR_ECUDA: return "CUDA launch or API failure";
         case AGNVAR_EUNSUPPORTED: return "unsupported configuration";
+        case AGNVAR_ESTATIC_LIMIT: return "request does not fit the library's built-in scratch array (agnvar_static_scratch_bytes)";
         default: return "unknown status";
     }
 }
@@ -857,6 +859,109 @@ int agnvar_periodogram(int64_t B, int64_t N, int dtype, const void* d_x, double 
                                  (cudaStream_t)stream);
     return pgram_impl<double>(B, N, d_x, dt, norm, nbins, h_bin_edges_j, d_out, d_counts, d_ws, ws_bytes,
                               (cudaStream_t)stream);
+}
+
+}  // extern "C"
+
+// =====================================================================================================
+// agnvar_structure_function_static -- the structure function for callers that have no scratch to give
+// =====================================================================================================
+// Every other call of this library works in a scratch buffer the caller allocates (d_ws).  Some callers cannot
+// produce one: a plug-in that is handed the light curves and an output slot but no allocator; a serving process whose
+// device memory was given, whole, to another component's pool at start-up, so that a cudaMalloc made now fails or eats
+// into somebody else's budget; a latency-bound loop that must not pay the device-wide wait an allocation can imply.
+// For them the partial sums, the lags and (mag = 1) the magnitudes live in the array below.  It is part of the
+// library's image: every GPU that loads libagnvar.so gives up AGNVAR_STATIC_SCRATCH_BYTES of memory for it when the
+// module is loaded there and keeps it until the process exits, which is why it is small.
+//
+// The name `g_sf_static_scratch` means two different things.  In device code it is the array.  In host code it is only
+// a handle by which the runtime finds the array: it is NOT an address a kernel can use (passing it would make the
+// kernel fault or, on a system where the GPU can read host memory, quietly work in the wrong place).  The host asks for
+// the real address with cudaGetSymbolAddress, once per device, with that device current (sf_static_base below), and
+// hands that pointer to the kernels -- the same sf_partial / sf_final / sf_rep kernels the workspace path launches.
+static __device__ __align__(256) unsigned char g_sf_static_scratch[AGNVAR_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+struct StaticLags { long long l[AGNVAR_STATIC_MAX_LAGS]; };
+
+// the lags arrive as a kernel argument (2 KB) and are written to the head of the scratch, where the pair kernels read
+// them: no host-to-device copy, hence no staging buffer of any kind
+__global__ void __launch_bounds__(AGNVAR_STATIC_MAX_LAGS) sf_static_lags_kernel(StaticLags h, int nlags, long long* __restrict__ lags) {
+    if ((int)threadIdx.x < nlags) lags[threadIdx.x] = h.l[threadIdx.x];
+}
+
+// bytes of the array a request uses: lags | magnitudes (mag only) | per-chunk partial sums
+inline size_t sf_static_need(int64_t B, int64_t N, int nlags, int mag) {
+    Carver c(nullptr);
+    c.take<long long>((size_t)nlags);
+    if (mag) c.take<double>((size_t)B * N);
+    c.take<double>((size_t)B * nlags * sf_chunks(N));
+    return c.off;
+}
+
+// Device address of g_sf_static_scratch on the CURRENT device; looked up on the first call per device and remembered
+// (ordinals >= 64 are looked up every time).  Returns NULL when the runtime refuses.
+void* sf_static_base() {
+    static std::mutex mu;
+    static void* known[64] = {nullptr};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0) return nullptr;
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev < 64 && known[dev]) return known[dev];
+    void* ptr = nullptr;
+    if (cudaGetSymbolAddress((void**)&ptr, g_sf_static_scratch) != cudaSuccess || !ptr) return nullptr;
+    if (dev < 64) known[dev] = ptr;
+    return ptr;
+}
+
+template <typename T>
+int sf_static_impl(int64_t B, int64_t N, const void* d_x, const int64_t* h_lags, int nlags, int mag, double* d_sf2,
+                   int64_t* d_pairs, double* d_mean, double* d_se, cudaStream_t st) {
+    void* base = sf_static_base();
+    if (!base) return AGNVAR_ECUDA;
+    Carver c(base);
+    long long* lags = c.take<long long>((size_t)nlags);
+    double* mags = mag ? c.take<double>((size_t)B * N) : nullptr;
+    const int nch = sf_chunks(N);
+    double* partial = c.take<double>((size_t)B * nlags * nch);
+    // Nothing in the array has to start at zero: the lags, every magnitude and every (curve, lag, chunk) partial sum
+    // are written by this call before anything reads them, so what an earlier call left behind is never seen.
+    StaticLags hl;
+    for (int q = 0; q < AGNVAR_STATIC_MAX_LAGS; ++q) hl.l[q] = q < nlags ? (long long)h_lags[q] : 0;
+    AGN_LAUNCH(K_SF, st, (sf_static_lags_kernel<<<1, AGNVAR_STATIC_MAX_LAGS, 0, st>>>(hl, nlags, lags)));
+    const dim3 grid((unsigned)nch, (unsigned)nlags, (unsigned)B);
+    if (mag) {
+        AGN_LAUNCH(K_SF, st, (sf_mag_kernel<T><<<cdiv(B * N, 256), 256, 0, st>>>((const T*)d_x, (long long)B * N, 0.0, 0, 0.0, mags, nullptr)));
+        AGN_LAUNCH(K_SF, st, (sf_partial_kernel<double><<<grid, 256, 0, st>>>(mags, N, lags, nlags, partial, nch, (int)B)));
+    } else {
+        AGN_LAUNCH(K_SF, st, (sf_partial_kernel<T><<<grid, 256, 0, st>>>((const T*)d_x, N, lags, nlags, partial, nch, (int)B)));
+    }
+    AGN_LAUNCH(K_SF, st, (sf_final_kernel<<<dim3((unsigned)nlags, (unsigned)B), 256, 0, st>>>(partial, nch, N, lags, nlags, d_sf2, (long long*)d_pairs)));
+    if (d_mean || d_se) AGN_LAUNCH(K_SF, st, (sf_rep_kernel<<<(unsigned)nlags, 256, 0, st>>>(d_sf2, (int)B, nlags, d_mean, d_se)));
+    return cuda_status(cudaGetLastError());
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t agnvar_static_scratch_bytes(void) { return (size_t)AGNVAR_STATIC_SCRATCH_BYTES; }
+
+size_t agnvar_structure_function_static_bytes(int64_t B, int64_t N, int nlags, int mag) {
+    if (!valid_BN(B, N) || B > 65535 || nlags < 1 || nlags > AGNVAR_STATIC_MAX_LAGS) return 0;
+    return sf_static_need(B, N, nlags, mag);
+}
+
+int agnvar_structure_function_static(int64_t B, int64_t N, int dtype, const void* d_x, const int64_t* h_lags, int nlags,
+                                     int mag, double* d_sf2, int64_t* d_pairs, double* d_rep_mean, double* d_rep_stderr,
+                                     void* stream) {
+    if (!valid_BN(B, N) || B > 65535 || !valid_dtype(dtype) || !d_x || !d_sf2 || !valid_lags(h_lags, nlags)) return AGNVAR_EINVAL;
+    if (nlags > AGNVAR_STATIC_MAX_LAGS) return AGNVAR_ESTATIC_LIMIT;
+    if (sf_static_need(B, N, nlags, mag) > (size_t)AGNVAR_STATIC_SCRATCH_BYTES) return AGNVAR_ESTATIC_LIMIT;
+    if (dtype == AGNVAR_F32)
+        return sf_static_impl<float>(B, N, d_x, h_lags, nlags, mag, d_sf2, d_pairs, d_rep_mean, d_rep_stderr, (cudaStream_t)stream);
+    return sf_static_impl<double>(B, N, d_x, h_lags, nlags, mag, d_sf2, d_pairs, d_rep_mean, d_rep_stderr, (cudaStream_t)stream);
 }
 
 }  // extern "C"
