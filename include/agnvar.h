@@ -14,6 +14,9 @@
  *     stream) and returns without synchronising.
  *   - Every call returns an agnvar_status; nothing throws or aborts.  AGNVAR_EINVAL is returned
  *     before any launch.  AGNVAR_ECUDA wraps a failed launch (sticky CUDA errors are not cleared).
+ *   - Threads: the library keeps small per-device host tables (kernel attributes set, grid sizes, the launch trace)
+ *     that are not locked.  Host threads that drive DIFFERENT devices may call concurrently; calls on the SAME device
+ *     must be serialised by the caller (one thread inside the library per device at a time).
  *   - Arrays are row-major [B][N], one light curve contiguous.  N is a power of two,
  *     4 <= N <= 2^30 (the paper's own cap is 2^27, "set by memory limitations"; a 180 GB B200 holds
  *     the loop's working set, ~45 bytes per sample, well beyond it).  The fastest paths cover fp32 up to 2^26
@@ -80,8 +83,8 @@ typedef struct {
 /* Bytes of scratch the given op needs.  `oversample` matters for AGNVAR_OP_TK_GENERATE only
  * (pass 1 otherwise); `aux` = grid_points for ERDF_SAMPLE_SORTED, nbins for PERIODOGRAM, 1 for E13_ITERATE
  * with the delta_i rule / history (see agnvar_e13_opts), nlags for STRUCTURE_FUNCTION, DELTA_M_PROB and
- * ENSEMBLE_SF (pass n_sub as N for ENSEMBLE_SF), else 0 (SLICE_SAMPLE_SORTED: 0).
- * Returns 0 for invalid arguments. */
+ * ENSEMBLE_SF (pass n_sub as N for ENSEMBLE_SF: any 2 <= n_sub <= 2^30, not only powers of two), else 0
+ * (SLICE_SAMPLE_SORTED: 0).  Returns 0 for invalid arguments. */
 size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int oversample, int64_t aux);
 
 /* S0 -- Eq. 3 at n given frequencies (fp64 in, fp64 out; d_out[i] = A * bracket(d_f[i])).
@@ -197,7 +200,8 @@ typedef struct {
  *                                        Feeding the output back resumes the run.
  *   d_x            out [B][N] dtype      final x_sim  (x[perm[r]] = sorted[r])
  *   d_iters_used   out [B] i32 or NULL
- *   d_changed_hist out [B][max_iter] i64 or NULL: changed count of every iteration
+ *   d_changed_hist out [B][max_iter] i64 or NULL: changed count of every executed iteration (entries of iterations that
+ *                  did not run -- early return with check_every > 0, on-chip early exit -- are 0)
  *   d_xadj_dbg     out [B][N] dtype or NULL: x_adj of the last iteration (for lock-step checks: call
  *                  with max_iter = 1 to step the product kernels one iteration at a time)
  *   h_opts         NULL or options (above).  Workspace: query with aux = 1 when delta_threshold > 0 or

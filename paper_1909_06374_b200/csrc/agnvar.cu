@@ -219,6 +219,8 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
     CK(cudaMemsetAsync(cursor, 0, (size_t)B * kRadix * sizeof(uint32_t), st));
     if (opt.d_sort_fallbacks) CK(cudaMemsetAsync(opt.d_sort_fallbacks, 0, (size_t)B * sizeof(int32_t), st));
     if (opt.d_delta_hist) CK(cudaMemsetAsync(opt.d_delta_hist, 0, (size_t)B * max_iter * sizeof(double), st));
+    // entries of iterations that never run (early return with check_every > 0) read 0, as on the on-chip path
+    if (d_changed_hist) CK(cudaMemsetAsync(d_changed_hist, 0, (size_t)B * max_iter * sizeof(int64_t), st));
     AGN_LAUNCH(K_PERM_ANORM, st, (perm_anorm_kernel<T><<<bgrid(cdiv(L + 1, 256), B), 256, 0, st>>>((const T*)d_anorm, Ap, plan.dg, (int)B)));
     const unsigned sg = (unsigned)std::min<long long>((N + 1023) / 1024, 148 * 16);
     // working buffers: x_sim in the caller's d_x and the permutations in (d_perm, P1) -- or, when delta_k is wanted,
@@ -619,6 +621,10 @@ int agnvar_trace_end(int64_t cap, int32_t* h_ids, float* h_ms, int64_t* h_n) {
 const char* agnvar_kernel_name(int id) { return (id >= 0 && id < K_NIDS) ? kKernelNames[id] : nullptr; }
 
 size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int oversample, int64_t aux) {
+    if (op == AGNVAR_OP_ENSEMBLE_SF) {   // N is n_sub here: any length agnvar_ensemble_sf accepts, not only powers of two
+        if (B < 1 || B > 65535 || N < 2 || N > ((int64_t)1 << 30) || !valid_dtype(dtype) || aux < 1 || aux > 4096) return 0;
+        return ws_ens(B, N, aux);
+    }
     if (!valid_BN(B, N) || !valid_dtype(dtype) || !size_supported(dtype, N)) return 0;
     const bool f32 = dtype == AGNVAR_F32;
     switch (op) {
@@ -641,9 +647,6 @@ size_t agnvar_workspace_bytes(int op, int64_t B, int64_t N, int dtype, int overs
         case AGNVAR_OP_DELTA_M_PROB:
             if (aux < 1 || aux > 4096 || B > 65535) return 0;
             return ws_sf(B, N, aux, true);
-        case AGNVAR_OP_ENSEMBLE_SF:
-            if (aux < 1 || aux > 4096 || B > 65535) return 0;
-            return ws_ens(B, N, aux);
         default: return 0;
     }
 }

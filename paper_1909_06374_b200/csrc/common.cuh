@@ -5,6 +5,7 @@
 #include <stdint.h>
 #include <stddef.h>
 #include <stdlib.h>
+#include <mutex>
 
 namespace agn {
 
@@ -127,16 +128,20 @@ struct DevCache {
     int sms = 0;
     int grid[16] = {0};                 // persistent-kernel grid sizes, by kernel slot
 };
+// Threading contract (include/agnvar.h, "Threads"): the slot's first-use initialisation is serialised here, but the
+// entries (attrs, grid) are then read and written without locks -- host threads that drive the SAME device must not
+// be inside the library at the same time; threads on different devices are independent.
 inline DevCache& dev_cache() {
     static DevCache tab[64];
+    static std::mutex mu;
     int dev = 0;
-    cudaGetDevice(&dev);
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0) dev = 0;   // no usable device: the first launch reports the error
     DevCache& c = tab[dev & 63];
+    std::lock_guard<std::mutex> lock(mu);
     if (c.dev != dev) {                 // first use of this ordinal (or an ordinal >= 64 aliasing a slot): start over
         c = DevCache();
         c.dev = dev;
-        cudaDeviceGetAttribute(&c.sms, cudaDevAttrMultiProcessorCount, dev);
-        if (c.sms < 1) c.sms = 1;
+        if (cudaDeviceGetAttribute(&c.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c.sms < 1) c.sms = 1;
     }
     return c;
 }

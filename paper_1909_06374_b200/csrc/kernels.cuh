@@ -21,8 +21,11 @@ __global__ void philox_words_kernel(uint64_t seed, uint64_t i0, long long n, uin
 // (r^a as exp2(a log2 r): one logarithm for both powers; the exponent a log2 r stays below ~100 in magnitude, so the
 //  result is within ~1e-14 relative of pow(): PSD values are gated at 1e-13 against the oracle)
 __device__ __forceinline__ double psd_shape(double f, double f_b, double a_lo, double a_hi) {
+    // a slope of exactly 0 gives the term 1 at every f, f = 0 included (pow(0, 0) = 1; 0 * log2(0) would be NaN)
     const double l = log2(f / f_b);
-    return 1.0 / (exp2(a_lo * l) + exp2(a_hi * l));
+    const double t_lo = a_lo == 0.0 ? 1.0 : exp2(a_lo * l);
+    const double t_hi = a_hi == 0.0 ? 1.0 : exp2(a_hi * l);
+    return 1.0 / (t_lo + t_hi);
 }
 
 __global__ void psd_bpl_kernel(const double* __restrict__ f, long long n, PsdDev p, double* __restrict__ out) {

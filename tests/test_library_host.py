@@ -44,6 +44,12 @@ def test_workspace_query_and_validation(L):
     assert b.workspace_bytes(b.OP_TK_GENERATE, 4, 4096, "f64", 10) > 0
     assert b.workspace_bytes(b.OP_ERDF_SAMPLE_SORTED, 4, 4096, "f64", 1, 1) == 0
     assert b.workspace_bytes(99, 4, 4096, "f64") == 0
+    # ENSEMBLE_SF: N is n_sub, any 2 <= n_sub <= 2^30 (values, flags, lags, counts, per-chunk partials)
+    assert b.workspace_bytes(b.OP_ENSEMBLE_SF, 40, 1000, "f32", 1, 9) >= 40 * 1000 * 9
+    assert b.workspace_bytes(b.OP_ENSEMBLE_SF, 40, 1024, "f64", 1, 9) >= 40 * 1024 * 9
+    assert b.workspace_bytes(b.OP_ENSEMBLE_SF, 40, 1, "f32", 1, 9) == 0
+    assert b.workspace_bytes(b.OP_ENSEMBLE_SF, 40, 1000, "f32", 1, 0) == 0
+    assert b.workspace_bytes(b.OP_ENSEMBLE_SF, 70000, 1000, "f32", 1, 9) == 0
     # EINVAL is returned before any launch, so these are safe without a device
     psd = b.agnvar_psd(0.0, -1.0, 1.0, 2.0)
     one = C.c_void_p(256)
