@@ -195,11 +195,24 @@ def oracle_all_cores(cfg, logn, iters):
     return cores * (1 << logn) * iters / dt, dt, cores
 
 
+REF_LOGN_CAP = 22      # the bounded CPU sample: one curve of the workload's parameters at N = 2^22 (1.5 s per iteration)
+
+
+def reference_sample(cfg):
+    """The ONE bounded sample both CPU legs time (--impl reference and the product line's cpu_baseline.value): one curve
+    of the workload's PSD / ERDF parameters at N = min(2^22, the workload's N), inputs from the oracle's own S1 + S2, one
+    E13 iteration (L1-L6) per repetition, fp64, one thread."""
+    logn = min(REF_LOGN_CAP, cfg["N"].bit_length() - 1)
+    sample = (f"1 curve of {cfg['name']}'s PSD/ERDF parameters at N=2^{logn}, 1 E13 iteration per step "
+              f"(fp64 CPU oracle, 1 thread)")
+    return logn, sample
+
+
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    logn = min(22, cfg["N"].bit_length() - 1)
+    logn, _ = reference_sample(cfg)
     iters = 1
     inputs = oracle_sample_inputs(cfg, logn)
     for _ in range(args.warmup):
@@ -209,8 +222,7 @@ def run_reference(args, cfg):
         oracle_time(logn, iters, inputs)
     dt = time.perf_counter() - t0
     value = args.steps * (1 << logn) * iters / dt
-    sample = (f"1 curve of {cfg['name']}'s PSD/ERDF parameters at N=2^{logn}, {iters} E13 iteration per step "
-              f"(fp64 CPU oracle, 1 thread)")
+    sample = reference_sample(cfg)[1]
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -259,6 +271,55 @@ def fp32_context(ag, cfg, dev):
 
 
 # ------------------------------------------------------------------------------------------------------
+# the other configurations (C1, C2, C3, C5), timed briefly after the headline's regions
+# ------------------------------------------------------------------------------------------------------
+def time_other_config(ag, torch, workloads, name, dev, peak, steps=3, warmup=2):
+    """`steps` steps of the whole path (S1 + S2 + loop + P) of configuration `name`, CUDA events, untraced; then one traced
+    step for the kernel time of the E13 call and, where the loop runs on chip, its rate on SURVEY 8(d)'s byte model."""
+    cfg = workloads.config(name)
+    B, N, iters = cfg["B"], cfg["N"], cfg["max_iter"]
+    for _ in range(warmup):
+        out = ag.generate_light_curves(cfg, device=dev)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        out = ag.generate_light_curves(cfg, device=dev)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    executed = int(out["iters_used"].sum().item())
+    del out
+    ag.trace_begin()
+    marks = []
+    out = ag.generate_light_curves(cfg, device=dev, phase_hook=lambda nm: marks.append((nm, ag.launch_count())))
+    torch.cuda.synchronize()
+    trace = ag.trace_end()
+    del out
+    lc0 = marks[0][1]
+    idx = {nm: c - lc0 for nm, c in marks}
+    order = [nm for nm, _ in marks]
+    e13 = trace[idx["E13"]:idx[order[order.index("E13") + 1]]] if order.index("E13") + 1 < len(order) else trace[idx["E13"]:]
+    e13_ms = sum(t for _, t in e13)
+    onchip = any(nm == "e13_onchip_loop" for nm, _ in e13)
+    model = sum(STAGE_MODEL_BYTES.values())
+    res = {"workload": workload_label(cfg), "steps": steps, "warmup": warmup, "ms_per_step": ms,
+           "value": N * executed / (ms * 1e-3), "unit": UNIT,
+           "iterations_executed_per_curve_mean": executed / B,
+           "nominal_value_at_max_iter": B * N * iters / (ms * 1e-3),
+           "e13_call_kernel_ms_traced": e13_ms, "e13_launches": len(e13),
+           "loop": "whole loop inside one CTA per curve (e13_onchip_loop)" if onchip else "multi-kernel loop",
+           "loop_samples_x_iterations_per_s": N * executed / (e13_ms * 1e-3) if e13_ms > 0 else None,
+           "l2": "inputs larger than L2" if B * N * (4 if cfg["dtype"] == "f32" else 8) > 2 ** 28 else
+                 "arrays smaller than L2: not flushed between steps"}
+    if e13_ms > 0:
+        res["hbm_equivalent_frac_of_peak"] = model * (2 if cfg["dtype"] == "f64" else 1) * N * executed / (e13_ms * 1e-3) / 1e9 / peak
+        res["hbm_equivalent_note"] = ("SURVEY 8(d)'s two-level model (86 B per sample per iteration in fp32, twice that in fp64) "
+                                      "over the E13 call's kernel time; for the on-chip loop this is NOT its HBM traffic")
+    return res
+
+
+# ------------------------------------------------------------------------------------------------------
 def respawn_under_torchrun(args):
     """`python bench.py --gpus N` without torchrun: run the same command line as N ranks on this node."""
     s = socket.socket()
@@ -284,6 +345,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-context", action="store_true", help="skip the fp32 free-running context numbers")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the short timings of C1, C2, C3 and C5")
     ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
                     help="process-group backend of the N > 1 plumbing (gloo: host-side tests of the spawn path)")
     ap.add_argument("--dry-ranks", action="store_true",
@@ -498,6 +560,22 @@ def main():
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
         del host
 
+    # ---- the other configurations of BASELINE.json (parity-test cases, not bench lines): a short timing of each, so
+    # that DESIGN.md section 11's table is driver-run.  Rank 0, N = 1, default workload only.
+    other = None
+    if rank == 0 and world == 1 and args.workload == "C4" and not args.no_other_configs and args.batch is None \
+            and args.max_iter is None and args.sampler == "inverse_cdf":
+        ag.free_workspace()
+        torch.cuda.empty_cache()
+        other = {}
+        for name in ("C1", "C2", "C3", "C5"):
+            try:
+                other[name] = time_other_config(ag, torch, workloads, name, dev, peak)
+            except Exception as exc:          # context only: never fails the bench line
+                other[name] = {"error": repr(exc)}
+            ag.free_workspace()
+            torch.cuda.empty_cache()
+
     # ---- the oracle on this box's host cores (rank 0, N = 1 only) ---------------------------------------
     cpu = None
     context = None
@@ -509,14 +587,26 @@ def main():
                 context = {"error": repr(exc)}
         ag.free_workspace()
         if not args.no_cpu_baseline:
-            logn = N.bit_length() - 1                  # the workload's own N (C4: 2^26, one iteration, about a minute)
+            # `value`: the sample the reference arm times (one CPU figure per record); then, as context, the same loop at
+            # the workload's own N (C4: 2^26, one iteration, about 40 s) and one curve per host thread
+            lr, sample = reference_sample(cfg)
+            inputs = oracle_sample_inputs(cfg, lr)
+            oracle_time(lr, 1, inputs)
+            reps, t_ref = 0, 0.0
+            while reps < 3 or (t_ref < 8.0 and reps < 64):
+                t_ref += oracle_time(lr, 1, inputs)[1]
+                reps += 1
+            logn = N.bit_length() - 1
             v, dt = oracle_time(logn, 1, synthetic_loop_inputs(logn))
             la = min(22, logn)
             va, dta, cores = oracle_all_cores(cfg, la, 1)
-            cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-                   "sample": f"1 curve at the workload's own N=2^{logn}, 1 E13 iteration (L1-L6), fp64, 1 thread, {dt:.1f} s; "
-                             f"inputs of that size from numpy (sorted log-normal draw, random permutation, red-noise amplitudes)",
+            cpu = {"value": reps * (1 << lr) / t_ref, "unit": UNIT, "cores": 1, "kind": "oracle",
+                   "sample": f"{sample}; {reps} repetitions, {t_ref:.1f} s (the sample `--impl reference` times)",
                    "host_cores_available": os.cpu_count(),
+                   "full_size": {"value": v, "unit": UNIT, "cores": 1,
+                                 "sample": f"1 curve at the workload's own N=2^{logn}, 1 E13 iteration (L1-L6), fp64, 1 thread, "
+                                           f"{dt:.1f} s; inputs of that size from numpy (sorted log-normal draw, random "
+                                           f"permutation, red-noise amplitudes)"},
                    "all_cores": {"value": va, "unit": UNIT, "cores": cores,
                                  "sample": f"{cores} curves at N=2^{la}, one per host thread, 1 E13 iteration each, {dta:.1f} s"}}
 
@@ -534,7 +624,7 @@ def main():
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "stages": stages,
                 "traffic_model": traffic_model, "sort_fallbacks": fallbacks, "ms_traced_step": ms_traced,
                 "ms_by_call_traced": phase_ms,   # S1 / S2 / E13 / P: kernel time of each C-ABI call in the traced step
-                "cpu_baseline": cpu, "fp32_free_running_context": context, "kernels": kernels}
+                "cpu_baseline": cpu, "fp32_free_running_context": context, "other_configs": other, "kernels": kernels}
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
