@@ -143,6 +143,8 @@ def workload_label(cfg):
          f"max_iter={cfg['max_iter']}, oversample={cfg['oversample']}")
     if cfg.get("sampler") == "slice":
         s += f", S1 by slice sampling {cfg['slice']} (NOT the headline configuration)"
+    if cfg.get("delta_threshold"):
+        s += f", stopping rule delta_i <= {cfg['delta_threshold']:g} (Eq. 4; NOT the headline configuration)"
     return s
 
 
@@ -320,6 +322,58 @@ def time_other_config(ag, torch, workloads, name, dev, peak, steps=3, warmup=2):
 
 
 # ------------------------------------------------------------------------------------------------------
+# NEXT-2: the structure function (Eq. A6) of the curves the path generates -- its own line, not the headline
+# ------------------------------------------------------------------------------------------------------
+def run_sf(args, cfg, ag, torch, dev, step):
+    import numpy as np
+    B, N = cfg["B"], cfg["N"]
+    x = step()["x"]
+    lags = sorted({int(round(v)) for v in np.logspace(0, np.log10(N // 2), 64)})
+    for _ in range(max(args.warmup, 1)):
+        ag.agnvar_structure_function(x, lags, want_rep=True)
+    torch.cuda.synchronize()
+    ag.trace_begin()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        ag.agnvar_structure_function(x, lags, want_rep=True)
+    e1.record()
+    torch.cuda.synchronize()
+    trace = ag.trace_end()
+    ms = e0.elapsed_time(e1) / args.steps
+    pairs = B * sum(N - l for l in lags)                       # pair differences per call
+    peak_hbm, peak_src = measured_peaks()
+    w = 4 if cfg["dtype"] == "f32" else 8
+    # What bounds it (profiles/r3_next_kernels_summary.md): not HBM -- the 60 lags of a curve run close together and find
+    # it in L2, DRAM sees one pass over x -- but the float -> double conversions, which issue on the XU pipe at 16 lanes
+    # per clock per SM (ncu: two conversions per pair at 1.77e12 pairs / s = 78 % of that pipe).  The kernel converts a
+    # first member once per kSfLagGroup = 8 lags and the partner once per pair: 1.125 conversions per pair.
+    conv = 1.125 * pairs if cfg["dtype"] == "f32" else 0.0
+    try:
+        sm_clock = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["sm_max_mhz"]) * 1e6
+    except Exception:
+        sm_clock = 1.965e9
+    peak_conv = 16.0 * 148 * sm_clock
+    top_ms = max(t for _, t in trace)
+    print(json.dumps({"metric": "structure-function pair differences / s", "value": pairs / (ms * 1e-3),
+                      "unit": "pairs/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+                      "higher_is_better": True, "dtype": cfg["dtype"], "data": "synthetic",
+                      "config": {"workload": workload_label(cfg) + f"; agnvar_structure_function at {len(lags)} log-spaced lags, "
+                                 "L/L_Edd units, with the representative SF (Eq. 6)", "lags": len(lags)},
+                      "roofline": {"bound": "alu", "kernel": "sf_partial_kernel",
+                                   "achieved": conv / (ms * 1e-3) / 1e9, "peak": peak_conv / 1e9, "unit": "G conversions/s",
+                                   "frac": conv / (ms * 1e-3) / peak_conv if conv else None,
+                                   "peak_source": "16 float->double conversions per clock per SM (XU pipe) x 148 SMs x the maximum SM "
+                                                  "clock; fp32 input only (fp64 input needs no conversion: fp64-pipe / L2 bound)",
+                                   "hbm_one_pass_bytes": float(w) * B * N,
+                                   "hbm_frac_on_one_pass": float(w) * B * N / (ms * 1e-3) / 1e9 / peak_hbm,
+                                   "hbm_peak": peak_hbm, "hbm_peak_source": peak_src,
+                                   "longest_launch_ms": top_ms, "traffic": None},
+                      "gpu_launches": len(trace)}), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------------
 def respawn_under_torchrun(args):
     """`python bench.py --gpus N` without torchrun: run the same command line as N ranks on this node."""
     s = socket.socket()
@@ -342,6 +396,11 @@ def main():
     ap.add_argument("--max-iter", type=int, default=None, help="override max_iter (NOT the headline configuration)")
     ap.add_argument("--sampler", default="inverse_cdf", choices=["inverse_cdf", "slice"],
                     help="S1 by the inverse-CDF table (north_star, the headline) or by the paper's slice sampler (NEXT-3)")
+    ap.add_argument("--delta", type=float, default=0.0,
+                    help="stop each curve by the paper's delta_i rule (Eq. 4) at this threshold (NOT the headline configuration)")
+    ap.add_argument("--op", default="path", choices=["path", "sf"],
+                    help="path: the hot path (the headline); sf: the structure function of the generated curves at 64 "
+                         "log-spaced lags (NEXT-2, Eq. A6), one JSON line with its own metric and roofline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-context", action="store_true", help="skip the fp32 free-running context numbers")
@@ -359,6 +418,8 @@ def main():
     if args.sampler == "slice":
         cfg["sampler"] = "slice"
         cfg["slice"] = dict(chains=min(cfg["N"], 65536), burn_in=50, thin=1, width=1.0, max_steps=8)
+    if args.delta > 0.0:
+        cfg["delta_threshold"] = args.delta
     if args.impl == "reference":
         run_reference(args, cfg)
         return 0
@@ -407,7 +468,10 @@ def main():
 
     def step(host_out=None, want_fallbacks=False, phase_hook=None):
         return ag.generate_light_curves(cfg, device=dev, host_out=host_out, curve0=curve0, want_fallbacks=want_fallbacks,
-                                        phase_hook=phase_hook)
+                                        phase_hook=phase_hook, delta_threshold=args.delta)
+
+    if args.op == "sf":
+        return run_sf(args, cfg, ag, torch, dev, step)
 
     # ---- (1) device-resident timing, untraced ----------------------------------------------------------
     for _ in range(args.warmup):
@@ -564,7 +628,7 @@ def main():
     # that DESIGN.md section 11's table is driver-run.  Rank 0, N = 1, default workload only.
     other = None
     if rank == 0 and world == 1 and args.workload == "C4" and not args.no_other_configs and args.batch is None \
-            and args.max_iter is None and args.sampler == "inverse_cdf":
+            and args.max_iter is None and args.sampler == "inverse_cdf" and args.delta <= 0.0:
         ag.free_workspace()
         torch.cuda.empty_cache()
         other = {}

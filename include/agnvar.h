@@ -170,6 +170,9 @@ int agnvar_tk_generate(const agnvar_psd* h_psd, int64_t n_psd, int64_t B, int64_
  *                    (or changed = 0): iters_used[b] = k and d_x / d_perm receive the state after iteration k.
  *                    The batch keeps running until every curve has stopped or k = max_iter (see check_every);
  *                    <= 0: only the exact rank-change rule below.  Needs positive values in d_sorted.
+ *                    Short curves (fp32 N <= 2^14, fp64 N <= 2^13) keep their one-CTA-per-curve loop under this rule
+ *                    (delta_k is evaluated on chip; each curve leaves the loop at its own k); d_x serves as scratch
+ *                    for x_sim,k while the call runs and holds the result when it has finished.
  *   d_delta_hist     out [B][max_iter] fp64 or NULL: delta_k of every executed iteration (later entries 0)
  *   d_sort_fallbacks out [B] i32 or NULL: number of iterations in which curve b's argsort left the distribution
  *                    sort for the LSD fallback (slab overflow: massive ties, adversarial keys); 0 in a normal run

@@ -187,16 +187,18 @@ int e13_impl(int64_t B, int64_t N, const void* d_anorm, const void* d_sorted, ui
 
     // short curves (fp32 to 2^14, fp64 to 2^13): the whole loop inside one CTA per curve (onchip.cuh); per-curve early exit
     // at changed = 0.
-    // (The delta_i rule keeps the generic path: it needs x_sim,k and x_sim,k+1 side by side.)
-    if (onchip_applicable(sizeof(T), N) && !dmode) {
+    // The delta_i rule (Eq. 4) runs there too: x_sim,k is parked in d_x during an iteration (onchip.cuh).
+    if (onchip_applicable(sizeof(T), N)) {
         AGN_LAUNCH(K_TABLES, st, (tw_init_kernel<T><<<(1 << kLogTw) / 256, 256, 0, st>>>(tables, 1 << kLogTw, kLogTw)));
         CK(cudaMemsetAsync(counters, 0, sizeof(unsigned int), st));
         if (d_changed_hist) CK(cudaMemsetAsync(d_changed_hist, 0, (size_t)B * max_iter * sizeof(int64_t), st));
         if (opt.d_sort_fallbacks) CK(cudaMemsetAsync(opt.d_sort_fallbacks, 0, (size_t)B * sizeof(int32_t), st));
+        if (opt.d_delta_hist) CK(cudaMemsetAsync(opt.d_delta_hist, 0, (size_t)B * max_iter * sizeof(double), st));
         OnchipArgs<T> oa;
         oa.anorm = (const T*)d_anorm; oa.sorted = (const T*)d_sorted; oa.perm = d_perm; oa.x = (T*)d_x;
         oa.xadj_dbg = (T*)d_xadj_dbg; oa.iters_used = d_iters_used; oa.hist = (long long*)d_changed_hist;
         oa.tw14 = (const C*)tables; oa.ticket = counters; oa.max_iter = max_iter; oa.B = B;
+        oa.delta_threshold = opt.delta_threshold; oa.delta_hist = opt.d_delta_hist;
         if (onchip_run<T>(ilog2_u64((uint64_t)N), oa, st) != cudaSuccess) return AGNVAR_ECUDA;
         return cuda_status(cudaGetLastError());
     }
@@ -498,7 +500,7 @@ int sf_impl(int64_t B, int64_t N, const void* d_x, const int64_t* h_lags, int nl
     const int nch = sf_chunks(N);
     double* partial = c.take<double>((size_t)B * nlags * nch);
     CK(cudaMemcpyAsync(lags, h_lags, (size_t)nlags * sizeof(int64_t), cudaMemcpyHostToDevice, st));
-    const dim3 grid((unsigned)nch, (unsigned)nlags, (unsigned)B);
+    const dim3 grid((unsigned)nch, sf_lag_groups(nlags), (unsigned)B);
     if (mag) {
         AGN_LAUNCH(K_SF, st, (sf_mag_kernel<T><<<cdiv(B * N, 256), 256, 0, st>>>((const T*)d_x, (long long)B * N, 0.0, 0, 0.0, mags, nullptr)));
         AGN_LAUNCH(K_SF, st, (sf_partial_kernel<double><<<grid, 256, 0, st>>>(mags, N, lags, nlags, partial, nch, (int)B)));
@@ -933,7 +935,7 @@ int sf_static_impl(int64_t B, int64_t N, const void* d_x, const int64_t* h_lags,
     StaticLags hl;
     for (int q = 0; q < AGNVAR_STATIC_MAX_LAGS; ++q) hl.l[q] = q < nlags ? (long long)h_lags[q] : 0;
     AGN_LAUNCH(K_SF, st, (sf_static_lags_kernel<<<1, AGNVAR_STATIC_MAX_LAGS, 0, st>>>(hl, nlags, lags)));
-    const dim3 grid((unsigned)nch, (unsigned)nlags, (unsigned)B);
+    const dim3 grid((unsigned)nch, sf_lag_groups(nlags), (unsigned)B);
     if (mag) {
         AGN_LAUNCH(K_SF, st, (sf_mag_kernel<T><<<cdiv(B * N, 256), 256, 0, st>>>((const T*)d_x, (long long)B * N, 0.0, 0, 0.0, mags, nullptr)));
         AGN_LAUNCH(K_SF, st, (sf_partial_kernel<double><<<grid, 256, 0, st>>>(mags, N, lags, nlags, partial, nch, (int)B)));

@@ -126,7 +126,7 @@ struct DevCache {
     int dev = -1;
     bool attrs[2] = {false, false};     // by element size (4, 8)
     int sms = 0;
-    int grid[16] = {0};                 // persistent-kernel grid sizes, by kernel slot
+    int grid[32] = {0};                 // persistent-kernel grid sizes, by kernel slot
 };
 // Threading contract (include/agnvar.h, "Threads"): the slot's first-use initialisation is serialised here, but the
 // entries (attrs, grid) are then read and written without locks -- host threads that drive the SAME device must not

@@ -17,7 +17,9 @@
 //       out by ascending time index (O6 step 4), bit-identical to std::stable_sort.  Cost grows with the square of a
 //       slot's population: an input with massive ties (all keys equal) is still sorted exactly, slowly.
 //   L5  changed += (idx_new[r] != idx_old[r]);  x_sim[idx_new[r]] = sorted[r]
-//   L6  changed = 0 -> converged (iters_used = k)
+//   L6  changed = 0 -> converged (iters_used = k); with the paper's delta_i rule (Eq. 4) switched on, also
+//       delta_k <= threshold.  delta_k costs one more pass over the curve per iteration: x_sim,k goes to the curve's
+//       output row in global memory at the start of the iteration (L2-resident) and is compared with x_sim,k+1 at the end.
 #pragma once
 #include "common.cuh"
 #include "fft.cuh"
@@ -68,6 +70,10 @@ template <typename T> struct OnchipArgs {
     unsigned int* ticket;       // zero on entry
     int max_iter;
     long long B;
+    // the paper's stopping rule (Eq. 4; NEXT-1), off when both are unset: delta_k = rms over the
+    // samples of log10(x_sim,k+1 / x_sim,k); a curve also stops at the first k with delta_k <= delta_threshold
+    double delta_threshold;     // <= 0: exact rank-change rule only
+    double* delta_hist;         // [B][max_iter] or NULL (zeroed by the host)
 };
 
 // float index of time sample j inside the padded complex row
@@ -87,7 +93,8 @@ __device__ __forceinline__ void onchip_fft(typename Cx<T>::type* s, int logL, in
     else if (logL - logNs == 1) fft_stage<T, 2, THREADS, EPT, true>(s, logL, logNs, 0, Rp, tw14);
 }
 
-template <typename T, int LOGN>
+// DM: with the delta_i rule (a separate instantiation, so that the plain loop's code and register use stay as they were)
+template <typename T, int LOGN, bool DM>
 __global__ void __launch_bounds__(OnchipCfg<T, LOGN>::THREADS) e13_onchip_kernel(OnchipArgs<T> a) {
     typedef OnchipCfg<T, LOGN> Cfg;
     typedef typename Cx<T>::type C;
@@ -104,7 +111,11 @@ __global__ void __launch_bounds__(OnchipCfg<T, LOGN>::THREADS) e13_onchip_kernel
     __shared__ unsigned int s_curve;
     __shared__ T s_lo, s_scale;
     __shared__ unsigned int s_changed;
+    __shared__ int s_stop;
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    // delta_k wanted: x_sim,k is parked in the curve's output row a.x (every thread stores and later re-reads its own
+    // samples, so no ordering between threads is involved), and compared with x_sim,k+1 once that sits in region A
+    constexpr bool dm = DM;
 
     for (;;) {
     __syncthreads();
@@ -124,7 +135,12 @@ __global__ void __launch_bounds__(OnchipCfg<T, LOGN>::THREADS) e13_onchip_kernel
     int used = a.max_iter;
     for (int k = 1; k <= a.max_iter; ++k) {
         __syncthreads();
-        // ---- L1 forward FFT
+        if (dm) {
+            T* xo = a.x + b * N;
+#pragma unroll
+            for (int i = 0; i < KPT; ++i) { const int j = i * THREADS + t; xo[j] = Zf[xpos(j)]; }
+        }
+        // ---- L1 forward FFT (a stage reads, synchronises, then writes: the reads above are done before any write)
         onchip_fft<T, THREADS, Cfg::EPT>(Z, LOGN - 1, RP, a.tw14);
         // ---- L2 untangle + amplitude replace + re-tangle (the stage's trailing barrier has been passed)
         for (int kk = t; kk <= L / 2; kk += THREADS) {
@@ -278,7 +294,36 @@ __global__ void __launch_bounds__(OnchipCfg<T, LOGN>::THREADS) e13_onchip_kernel
         const uint32_t changed = s_changed;
         if (t == 0 && a.hist) a.hist[b * a.max_iter + (k - 1)] = (long long)changed;
         // ---- L6
-        if (changed == 0u) { used = k; break; }
+        bool stop = changed == 0u;
+        if (dm) {
+            // Eq. 4 on chip: sum of squares in fp64, fixed order (per thread by ascending sample, warp tree, warps in order)
+            __syncthreads();                    // x_sim,k+1 is complete in region A
+            const T* xo = a.x + b * N;
+            double acc = 0.0;
+#pragma unroll
+            for (int i = 0; i < KPT; ++i) {
+                const int j = i * THREADS + t;
+                const T xn = Zf[xpos(j)], xp = xo[j];
+                if (xn != xp) {                 // an unchanged sample contributes log10(1) = 0 exactly: skip the division and the log
+                    const double d = log10_ratio(xn, xp);
+                    acc = fma(d, d, acc);
+                }
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+            if (lane == 0) red[warp] = acc;
+            __syncthreads();
+            if (t == 0) {
+                double tot = 0.0;
+                for (int w = 0; w < WARPS; ++w) tot += red[w];
+                const double delta = sqrt(tot / (double)N);
+                if (a.delta_hist) a.delta_hist[b * a.max_iter + (k - 1)] = delta;
+                s_stop = (a.delta_threshold > 0.0 && delta <= a.delta_threshold) ? 1 : 0;
+            }
+            __syncthreads();
+            stop = stop || s_stop != 0;
+        }
+        if (stop) { used = k; break; }
     }
     __syncthreads();
     // results: x_sim and the final permutation
@@ -294,22 +339,27 @@ inline bool onchip_applicable(size_t elem_size, long long N) {
     return N >= 256 && ((elem_size == 4 && N <= 16384) || (elem_size == 8 && N <= 8192));
 }
 
-template <typename T, int LOGN> inline cudaError_t onchip_launch(const OnchipArgs<T>& a, int slot, cudaStream_t st) {
+template <typename T, int LOGN, bool DM> inline cudaError_t onchip_launch_dm(const OnchipArgs<T>& a, int slot, cudaStream_t st) {
     typedef OnchipCfg<T, LOGN> Cfg;
     int& grid = dev_cache().grid[slot];
     if (!grid) {
-        cudaError_t e = cudaFuncSetAttribute(e13_onchip_kernel<T, LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem);
+        cudaError_t e = cudaFuncSetAttribute(e13_onchip_kernel<T, LOGN, DM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem);
         if (e != cudaSuccess) return e;
-        cudaFuncSetAttribute(e13_onchip_kernel<T, LOGN>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        cudaFuncSetAttribute(e13_onchip_kernel<T, LOGN, DM>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
         int per = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, e13_onchip_kernel<T, LOGN>, Cfg::THREADS, Cfg::smem);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, e13_onchip_kernel<T, LOGN, DM>, Cfg::THREADS, Cfg::smem);
         if (e != cudaSuccess) return e;
         if (per < 1) return cudaErrorInvalidConfiguration;
         grid = dev_cache().sms * per;
     }
     const unsigned g = (unsigned)std::min<long long>(a.B, grid);
-    AGN_LAUNCH(K_E13_ONCHIP, st, (e13_onchip_kernel<T, LOGN><<<g, Cfg::THREADS, Cfg::smem, st>>>(a)));
+    AGN_LAUNCH(K_E13_ONCHIP, st, (e13_onchip_kernel<T, LOGN, DM><<<g, Cfg::THREADS, Cfg::smem, st>>>(a)));
     return cudaGetLastError();
+}
+// slot: dev_cache().grid index of the plain instantiation (3 .. 15); the delta instantiation keeps its own 13 slots above
+template <typename T, int LOGN> inline cudaError_t onchip_launch(const OnchipArgs<T>& a, int slot, cudaStream_t st) {
+    if (a.delta_hist != nullptr || a.delta_threshold > 0.0) return onchip_launch_dm<T, LOGN, true>(a, slot + 13, st);
+    return onchip_launch_dm<T, LOGN, false>(a, slot, st);
 }
 
 template <typename T> inline cudaError_t onchip_run(int logN, const OnchipArgs<T>& a, cudaStream_t st) {

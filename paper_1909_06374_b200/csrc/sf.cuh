@@ -30,25 +30,56 @@ __global__ void __launch_bounds__(256) sf_mag_kernel(const T* __restrict__ x, lo
 }
 
 // partial[b][q][chunk] = sum over the chunk's pairs of (v_i - v_{i+l})^2.  V = T (raw series) or double (magnitudes).
+// A CTA owns one chunk of first members i and kSfLagGroup consecutive lags: a thread converts its 32 first members to
+// fp64 ONCE and keeps them in registers, so a pair costs one load and one float -> double conversion instead of two
+// (ncu, round 3: with two conversions per pair the kernel sat at 78 % of the conversion (XU) pipe, fp64 pipe 22 %,
+// DRAM one pass over x -- a curve's lags run close together and find it in L2).  Order of the additions per (b, q,
+// chunk) is fixed: per thread by ascending i, then the block tree.
+constexpr int kSfLagGroup = 8;
+constexpr int kSfSub = 8;                 // first members held in registers at a time
 template <typename V>
-__global__ void __launch_bounds__(256) sf_partial_kernel(const V* __restrict__ v, long long N, const long long* __restrict__ lags,
-                                                         int nlags, double* __restrict__ partial, int nchunks, int B) {
+__global__ void __launch_bounds__(256, 4) sf_partial_kernel(const V* __restrict__ v, long long N, const long long* __restrict__ lags,
+                                                            int nlags, double* __restrict__ partial, int nchunks, int B) {
     __shared__ double sh[256];
+    constexpr int PER = kSfChunk / 256;
     const long long b = blockIdx.z;
-    const int q = blockIdx.y;
-    const long long l = lags[q];
-    const long long P = N - l;                              // number of pairs (<= 0: none)
-    const long long beg = (long long)blockIdx.x * kSfChunk;
-    const long long end = beg + kSfChunk < P ? beg + kSfChunk : P;
+    const int q0 = blockIdx.y * kSfLagGroup;
+    const long long beg = (long long)blockIdx.x * kSfChunk + threadIdx.x;
     const V* vb = v + b * N;
-    double acc = 0.0;
-    for (long long i = beg + threadIdx.x; i < end; i += 256) {
-        const double d = (double)vb[i] - (double)vb[i + l];
-        acc += d * d;
+    long long lag[kSfLagGroup];
+    double acc[kSfLagGroup];
+#pragma unroll
+    for (int g = 0; g < kSfLagGroup; ++g) {
+        lag[g] = q0 + g < nlags ? lags[q0 + g] : N;          // a lag of N has no pair
+        acc[g] = 0.0;
     }
-    const double tot = block_sum<256>(acc, sh);
-    if (threadIdx.x == 0) partial[(b * nlags + q) * nchunks + blockIdx.x] = tot;
+    for (int k0 = 0; k0 < PER; k0 += kSfSub) {
+        double own[kSfSub];
+#pragma unroll
+        for (int k = 0; k < kSfSub; ++k) {
+            const long long i = beg + 256ll * (k0 + k);
+            own[k] = i < N ? (double)vb[i] : 0.0;
+        }
+#pragma unroll
+        for (int g = 0; g < kSfLagGroup; ++g) {
+            const long long P = N - lag[g];                  // number of pairs (<= 0: none)
+#pragma unroll
+            for (int k = 0; k < kSfSub; ++k) {
+                const long long i = beg + 256ll * (k0 + k);
+                if (i < P) {
+                    const double d = own[k] - (double)vb[i + lag[g]];
+                    acc[g] += d * d;
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int g = 0; g < kSfLagGroup; ++g) {
+        const double tot = block_sum<256>(acc[g], sh);
+        if (threadIdx.x == 0 && q0 + g < nlags) partial[(b * nlags + q0 + g) * nchunks + blockIdx.x] = tot;
+    }
 }
+inline unsigned sf_lag_groups(int nlags) { return (unsigned)((nlags + kSfLagGroup - 1) / kSfLagGroup); }
 
 // sf2[b][q] = (sum of the partials) / (N - l); pairs[q] = N - l
 __global__ void __launch_bounds__(256) sf_final_kernel(const double* __restrict__ partial, int nchunks, long long N,

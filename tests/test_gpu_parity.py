@@ -488,7 +488,7 @@ def test_delta_fp64_trajectory_and_threshold(ag, orc, N, os_):
     assert (ch[:, kmax + 2:] == 0).all() and (early["delta_hist"].cpu().numpy()[:, kmax + 2:] == 0).all()
 
 
-@pytest.mark.parametrize("N,erdf", [(1024, BPL), (2 ** 15, LOGN), (2 ** 18, BPL), (2 ** 22, BPL)])
+@pytest.mark.parametrize("N,erdf", [(256, LOGN), (1024, BPL), (2 ** 14, BPL), (2 ** 15, LOGN), (2 ** 18, BPL), (2 ** 22, BPL)])
 def test_delta_fp32_lockstep(ag, orc, N, erdf):
     """fp32: delta_k is a function of the two consecutive series the GPU itself produced (exact fp32 values), so it is
     compared with the oracle's Eq. 4 evaluated on those very series: <= 1e-6 relative."""
@@ -511,6 +511,44 @@ def test_delta_fp32_lockstep(ag, orc, N, erdf):
     srt2, perm2, an2 = _inputs(ag, erdf, PSD, B, N, 1, "f32", 8)
     plain = ag.agnvar_e13_iterate(an2, srt2, perm2, K)
     assert torch.equal(plain["x"], out["x"]) and torch.equal(perm2, perm)
+
+
+@pytest.mark.parametrize("dtype,N", [("f32", 1024), ("f32", 2 ** 14), ("f64", 4096)])
+def test_delta_rule_stays_on_chip_for_short_curves(ag, orc, dtype, N):
+    """The paper's own stopping rule (Eq. 4) must not cost short curves their on-chip loop: with a threshold the call is
+    still the one-CTA-per-curve kernel, every curve stops at the first k with delta_k <= threshold (or changed = 0),
+    delta_k equals Eq. 4 evaluated on the two series around that iteration, and entries after the stop read 0."""
+    B, max_iter = 6, 40
+    srt, perm0, an = _inputs(ag, BPL, PSD, B, N, 1, dtype, 21)
+    free = ag.agnvar_e13_iterate(an, srt, perm0.clone(), max_iter, want_hist=True, want_delta=True)
+    dh = free["delta_hist"].cpu().numpy()
+    thr = float(np.sqrt(dh[0][3] * dh[0][4]))
+    ag.trace_begin()
+    perm = perm0.clone()
+    out = ag.agnvar_e13_iterate(an, srt, perm, max_iter, want_hist=True, want_delta=True, delta_threshold=thr)
+    torch.cuda.synchronize()
+    names = [n for n, _ in ag.trace_end()]
+    assert "e13_onchip_loop" in names and not any(n.startswith("sort_") or n.startswith("fft_") for n in names)
+    it = out["iters_used"].cpu().numpy()
+    d, ch = out["delta_hist"].cpu().numpy(), out["changed_hist"].cpu().numpy()
+    assert len(set(it.tolist())) > 1 or B == 1          # curves stop at their own iteration
+    for b in range(B):
+        k = int(it[b])
+        assert k == max_iter or d[b][k - 1] <= thr or ch[b][k - 1] == 0
+        assert (d[b][:k - 1] > thr).all() and (ch[b][:k - 1] > 0).all()             # not earlier
+        assert (d[b][k:] == 0).all() and (ch[b][k:] == 0).all()
+        # the same curve alone, stepped k - 1 iterations and then one more: delta of that last step against Eq. 4
+        p1 = perm0[b:b + 1].clone()
+        if k > 1:
+            prev = ag.agnvar_e13_iterate(an[b:b + 1], srt[b:b + 1], p1, k - 1)["x"].cpu().numpy()[0]
+        else:
+            prev = np.empty(N, dtype=srt.cpu().numpy().dtype)
+            prev[u32(perm0)[b]] = srt[b].cpu().numpy()
+        last = ag.agnvar_e13_iterate(an[b:b + 1], srt[b:b + 1], p1, 1, want_delta=True)
+        assert torch.equal(last["x"][0], out["x"][b]) and torch.equal(p1[0], perm[b])
+        want = orc.delta_rms(last["x"].cpu().numpy()[0].astype(np.float64), prev.astype(np.float64))
+        assert d[b][k - 1] == pytest.approx(want, rel=1e-6 if dtype == "f32" else 1e-12)
+        assert float(last["delta_hist"][0, 0]) == d[b][k - 1]
 
 
 # ---- NEXT-2: structure function (Eq. A6), representative SF (Eq. 6), P(|dm| > dm_ref | tau) ------------
