@@ -555,7 +555,7 @@ inline cudaError_t bucket1_sort(const float* vals, uint32_t* idx_out, float* sor
     const uint32_t nsamp = (uint32_t)(N >> kBkSampleLog);
     const uint32_t M = bucket1_magic(nb, bl);
     const unsigned chunks = cdf_chunks(bl);
-    AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B, bl)));
+    AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid(cdf_sample_grid(nsamp), B), 256, 0, st>>>(vals, hist, (uint32_t)N, B, bl)));
     AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)(B * chunks), 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog), bl, chunks)));
     AGN_LAUNCH(K_SORT_CDF, st, (bucket_bounds_kernel<<<bgrid((nb + 256) / 256, B), 256, 0, st>>>(tab, klo, nb, M, kB1SlotLog, B, bl)));
     Part1Args a;

@@ -62,20 +62,31 @@ inline uint32_t bucket32_magic(uint32_t nb) {
     return (uint32_t)((((unsigned __int128)nb) << (32 + kBkSlotLog + 9)) / (kBkTotalW << 16));
 }
 
+// (kCdfSampleIlp samples per thread, all loads issued before the first histogram update: the kernel is bound by DRAM
+//  latency -- every sample costs a 32-byte sector -- and one load in flight per thread left the memory system at 3 TB/s)
+constexpr int kCdfSampleIlp = 4;
 __global__ void __launch_bounds__(256) cdf_sample_kernel(const float* __restrict__ vals, uint32_t* __restrict__ hist,
                                                          uint32_t N, long long B, int bl = kBkBinLog) {
     const long long b = bidx();
     if (b >= B) return;
-    const uint32_t i = blockIdx.x * 256 + threadIdx.x;          // sample number
-    const bool in = i < (N >> kBkSampleLog);
-    // the sample of block i of 64 keys sits at a position that varies with i (no fixed phase)
-    const uint32_t e = (i << kBkSampleLog) + ((i * 0x9E3779B1u) >> (32 - kBkSampleLog));
-    const uint32_t bin = in ? (key_of(vals[(size_t)b * N + e]) >> (32 - bl)) : 0xffffffffu;
-    // neighbouring samples of a smooth series share their bin: one atomic per distinct bin and warp
-    const uint32_t peers = __match_any_sync(0xffffffffu, bin);
-    if (in && (threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1))
-        atomicAdd(&hist[((size_t)b << bl) + bin], (uint32_t)__popc(peers));
+    const uint32_t nsamp = N >> kBkSampleLog;
+    uint32_t bin[kCdfSampleIlp];
+#pragma unroll
+    for (int u = 0; u < kCdfSampleIlp; ++u) {
+        const uint32_t i = (blockIdx.x * kCdfSampleIlp + u) * 256 + threadIdx.x;          // sample number
+        // the sample of block i of 64 keys sits at a position that varies with i (no fixed phase)
+        const uint32_t e = (i << kBkSampleLog) + ((i * 0x9E3779B1u) >> (32 - kBkSampleLog));
+        bin[u] = i < nsamp ? (key_of(vals[(size_t)b * N + e]) >> (32 - bl)) : 0xffffffffu;
+    }
+#pragma unroll
+    for (int u = 0; u < kCdfSampleIlp; ++u) {
+        // neighbouring samples of a smooth series share their bin: one atomic per distinct bin and warp
+        const uint32_t peers = __match_any_sync(0xffffffffu, bin[u]);
+        if (bin[u] != 0xffffffffu && (threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1))
+            atomicAdd(&hist[((size_t)b << bl) + bin[u]], (uint32_t)__popc(peers));
+    }
 }
+inline unsigned cdf_sample_grid(uint32_t nsamp) { return (nsamp + 256 * kCdfSampleIlp - 1) / (256 * kCdfSampleIlp); }
 
 // tab[bin] = (exclusive cumulative weight << 7, weight), weight = (cnt << logK) + 1.  kCdfChunks CTAs per curve, each
 // owning 65536 / kCdfChunks consecutive bins: a CTA first adds up the weights of all bins before its chunk (the
@@ -532,7 +543,7 @@ inline cudaError_t bucket32_sort(const float* vals, uint32_t* idx_out, float* so
     e = cudaMemsetAsync(hist, 0, zero_bytes, st);
     if (e != cudaSuccess) return e;
     const uint32_t nsamp = (uint32_t)(N >> kBkSampleLog);
-    AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid((nsamp + 255) / 256, B), 256, 0, st>>>(vals, hist, (uint32_t)N, B)));
+    AGN_LAUNCH(K_SORT_CDF, st, (cdf_sample_kernel<<<bgrid(cdf_sample_grid(nsamp), B), 256, 0, st>>>(vals, hist, (uint32_t)N, B)));
     AGN_LAUNCH(K_SORT_CDF, st, (cdf_table_kernel<<<(unsigned)(B * kCdfChunks), 1024, 0, st>>>(hist, tab, 24 - (ilog2_u64((uint64_t)N) - kBkSampleLog))));
     AGN_LAUNCH(K_SORT_CDF, st, (bucket_bounds_kernel<<<bgrid((g.nb + 256) / 256, B), 256, 0, st>>>(tab, klo, g.nb, bucket32_magic(g.nb), kBkSlotLog, B)));
     PartArgs a;
