@@ -252,6 +252,7 @@ __global__ void __launch_bounds__(kS32Threads, 4) sweep32_kernel(Sweep32Args a) 
 // ------------------------------------------------------------------------------------------------
 // L5 two-level: place step (the bin step is bucket_part_kernel<2> of bucket32.cuh)
 // ------------------------------------------------------------------------------------------------
+template <int kPlaceElems>
 __global__ void __launch_bounds__(256) scatter_place32_kernel(const uint4* __restrict__ pairs2, float* __restrict__ x,
                                                               uint32_t N, uint32_t* __restrict__ cursor, long long B,
                                                               const uint32_t* __restrict__ gate) {
@@ -261,9 +262,12 @@ __global__ void __launch_bounds__(256) scatter_place32_kernel(const uint4* __res
     if (blockIdx.x == 0) cursor[b * kRadix + threadIdx.x] = 0u;      // ready for the next iteration's bin pass
     const size_t seg = (size_t)b * N;
     float* xs = x + seg;
-    const uint4* p = pairs2 + (seg >> 1) + (size_t)blockIdx.x * 1024 + threadIdx.x;     // 2 pairs per uint4
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
+    // kPlaceElems pairs per CTA (2 per uint4): 2048 where the kernel does the work (1.45 ms per 2^28 pairs; 8192 measured
+    // 1.99 ms), 8192 where it is the gated fallback of the write-back sort and normally exits at once -- its cost is then
+    // the number of CTAs (131072 CTAs of 2048 pairs took 70 us per C4 iteration doing nothing).
+    const uint4* p = pairs2 + (seg >> 1) + (size_t)blockIdx.x * (kPlaceElems / 2) + threadIdx.x;
+#pragma unroll 4
+    for (int i = 0; i < kPlaceElems / 512; ++i) {
         const uint4 q = __ldcs(p + i * 256);
         xs[q.y] = __uint_as_float(q.x);
         xs[q.w] = __uint_as_float(q.z);
@@ -395,8 +399,12 @@ inline cudaError_t rank_scatter_two_level32(const uint32_t* idx_new, const uint3
     a.cap_out = (uint32_t)(N >> kRadixBits); a.B = B; a.gate = gate;
     // with a gate these two launches are the fallback of the write-back sort: they exit at once for every other curve
     AGN_LAUNCH(gate ? K_SORT_FALLBACK : K_SCATTER_BIN, st, (bucket_part_kernel<2><<<bgrid((unsigned)(N / bk_part_tile(2)), B), kBkPartThreads, sizeof(PartSmem<2>), st>>>(a)));
-    AGN_LAUNCH(gate ? K_SORT_FALLBACK : K_SCATTER_PLACE, st, (scatter_place32_kernel<<<bgrid((unsigned)(N / 2048), B), 256, 0, st>>>(
-        (const uint4*)pairs, x, (uint32_t)N, cursor, B, gate)));
+    if (gate)
+        AGN_LAUNCH(K_SORT_FALLBACK, st, (scatter_place32_kernel<8192><<<bgrid((unsigned)(N / 8192), B), 256, 0, st>>>(
+            (const uint4*)pairs, x, (uint32_t)N, cursor, B, gate)));
+    else
+        AGN_LAUNCH(K_SCATTER_PLACE, st, (scatter_place32_kernel<2048><<<bgrid((unsigned)(N / 2048), B), 256, 0, st>>>(
+            (const uint4*)pairs, x, (uint32_t)N, cursor, B, gate)));
     return cudaGetLastError();
 }
 
